@@ -1,0 +1,184 @@
+"""ORACLE — test infrastructure only (see oracle/treecode_oracle.cpp header).
+
+Only tests/, ``__graft_entry__.smoke()`` and ``bench.py``'s ``cpu_baseline`` /
+``--impl reference`` legs may import this package.  It never imports the CUDA
+binding and shares no code with ``paper_1005_5384_b200/csrc``.
+
+``build()`` compiles the plain C++ oracle with g++ (``-ffp-contract=off``) into
+``oracle/liboracle_tc.so``; ``Oracle`` is a thin ctypes wrapper.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+import subprocess
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SRC = os.path.join(_HERE, "treecode_oracle.cpp")
+_LIB = os.path.join(_HERE, "liboracle_tc.so")
+_lib = None
+
+
+def build(force: bool = False) -> str:
+    """Compile the oracle if the .so is missing or older than its source."""
+    if (not force and os.path.exists(_LIB)
+            and os.path.getmtime(_LIB) >= os.path.getmtime(_SRC)):
+        return _LIB
+    cmd = ["g++", "-O2", "-std=c++17", "-fPIC", "-shared", "-fopenmp",
+           "-ffp-contract=off", "-fno-fast-math", "-o", _LIB, _SRC]
+    subprocess.run(cmd, check=True)
+    return _LIB
+
+
+def _load():
+    global _lib
+    if _lib is not None:
+        return _lib
+    build()
+    L = C.CDLL(_LIB)
+    vp, i64, i32, f64 = C.c_void_p, C.c_int64, C.c_int, C.c_double
+    L.orc_create.restype = vp
+    L.orc_create.argtypes = [i64, vp, vp, i32, i32]
+    L.orc_destroy.argtypes = [vp]
+    for f in ("orc_n_cells", "orc_n_leaves", "orc_n_groups"):
+        getattr(L, f).restype = i64
+        getattr(L, f).argtypes = [vp]
+    L.orc_depth.restype = i32
+    L.orc_depth.argtypes = [vp]
+    L.orc_get_root.argtypes = [vp, vp, vp]
+    L.orc_get_grid.argtypes = [vp, vp]
+    L.orc_get_perm.argtypes = [vp, vp]
+    L.orc_get_groups.argtypes = [vp, vp]
+    L.orc_get_cells.argtypes = [vp] + [vp] * 13
+    L.orc_walk.restype = i32
+    L.orc_walk.argtypes = [vp, i64, f64, i32, vp, i64, vp, i64, vp, vp, vp, vp, vp]
+    L.orc_forces.restype = i64
+    L.orc_forces.argtypes = [vp, f64, f64, i32, i64, vp, vp, vp, vp, vp, vp, vp, vp]
+    L.orc_direct.argtypes = [i64, vp, vp, f64, i64, vp, vp, vp]
+    L.orc_num_threads.restype = i32
+    _lib = L
+    return L
+
+
+def _p(a):
+    return None if a is None else a.ctypes.data_as(C.c_void_p)
+
+
+def num_threads() -> int:
+    return int(_load().orc_num_threads())
+
+
+class Oracle:
+    """fp64 CPU tree-code: own tree (O1-O4), own walk (O5), own evaluation (O6)."""
+
+    def __init__(self, pos, mass, n_leaf: int = 16, n_group: int | None = None):
+        L = _load()
+        self.pos = np.ascontiguousarray(pos, dtype=np.float32)
+        self.mass = np.ascontiguousarray(mass, dtype=np.float32)
+        assert self.pos.ndim == 2 and self.pos.shape[1] == 3 and self.mass.shape == (self.pos.shape[0],)
+        self.n = self.pos.shape[0]
+        self.n_leaf = int(n_leaf)
+        self.n_group = int(n_group if n_group is not None else n_leaf)
+        self._h = L.orc_create(self.n, _p(self.pos), _p(self.mass), self.n_leaf, self.n_group)
+        if not self._h:
+            raise ValueError("orc_create failed (n, n_leaf, n_group must be >= 1)")
+        self.n_cells = int(L.orc_n_cells(self._h))
+        self.n_leaves = int(L.orc_n_leaves(self._h))
+        self.n_groups = int(L.orc_n_groups(self._h))
+        self.depth = int(L.orc_depth(self._h))
+
+    def __del__(self):
+        if getattr(self, "_h", None) and _lib is not None:
+            _lib.orc_destroy(self._h)
+            self._h = None
+
+    # ---- tree inspection -------------------------------------------------
+    def root(self):
+        org = np.zeros(3)
+        side = np.zeros(1)
+        _lib.orc_get_root(self._h, _p(org), _p(side))
+        return org, float(side[0])
+
+    def grid(self):
+        g = np.zeros((self.n, 3), dtype=np.int32)
+        _lib.orc_get_grid(self._h, _p(g))
+        return g
+
+    def perm(self):
+        p = np.zeros(self.n, dtype=np.int64)
+        _lib.orc_get_perm(self._h, _p(p))
+        return p
+
+    def groups(self):
+        g = np.zeros(self.n_groups, dtype=np.int32)
+        _lib.orc_get_groups(self._h, _p(g))
+        return g
+
+    def cells(self) -> dict:
+        nc = self.n_cells
+        d = dict(level=np.zeros(nc, np.int32), parent=np.zeros(nc, np.int32),
+                 child=np.zeros((nc, 8), np.int32), n_child=np.zeros(nc, np.int32),
+                 begin=np.zeros(nc, np.int64), count=np.zeros(nc, np.int64),
+                 bmin=np.zeros((nc, 3)), bmax=np.zeros((nc, 3)), b=np.zeros((nc, 3)), h=np.zeros(nc),
+                 M=np.zeros(nc), X=np.zeros((nc, 3)), Q=np.zeros((nc, 6)))
+        _lib.orc_get_cells(self._h, *[_p(d[k]) for k in
+                                      ("level", "parent", "child", "n_child", "begin", "count",
+                                       "bmin", "bmax", "b", "h", "M", "X", "Q")])
+        return d
+
+    # ---- walk / forces ---------------------------------------------------
+    def walk(self, group: int, theta: float, shadow32: bool = False):
+        """(cell_list, leaf_list, min_margin, n_flips, n_tests) of one group (O5)."""
+        cap = self.n_cells
+        cl = np.zeros(cap, np.int32)
+        ll = np.zeros(cap, np.int32)
+        nc = np.zeros(1, np.int64)
+        nl = np.zeros(1, np.int64)
+        mm = np.zeros(1)
+        nf = np.zeros(1, np.int64)
+        nt = np.zeros(1, np.int64)
+        rc = _lib.orc_walk(self._h, int(group), float(theta), int(shadow32), _p(cl), cap, _p(ll), cap,
+                           _p(nc), _p(nl), _p(mm), _p(nf), _p(nt))
+        assert rc == 0
+        return cl[: nc[0]].copy(), ll[: nl[0]].copy(), float(mm[0]), int(nf[0]), int(nt[0])
+
+    def forces(self, theta: float, eps: float, shadow32: bool = False, groups=None, stats: bool = False):
+        """acc fp64 [n,3], pot fp64 [n], n_pc int64 [n], n_pp int64 [n] (+ per-group stats).
+
+        ``groups``: optional int64 array of group indices; particles of other
+        groups keep NaN (acc, pot) / -1 (counts).
+        """
+        acc = np.full((self.n, 3), np.nan)
+        pot = np.full(self.n, np.nan)
+        npc = np.full(self.n, -1, np.int64)
+        npp = np.full(self.n, -1, np.int64)
+        sel = None
+        ng = self.n_groups
+        if groups is not None:
+            sel = np.ascontiguousarray(groups, dtype=np.int64)
+            ng = sel.size
+        gm = np.zeros(ng)
+        gf = np.zeros(ng, np.int64)
+        gt = np.zeros(ng, np.int64)
+        total = _lib.orc_forces(self._h, float(theta), float(eps), int(shadow32), ng, _p(sel),
+                                _p(acc), _p(pot), _p(npc), _p(npp), _p(gm), _p(gf), _p(gt))
+        out = dict(acc=acc, pot=pot, n_pc=npc, n_pp=npp, interactions=int(total))
+        if stats:
+            out.update(min_margin=gm, flips=gf, tests=gt)
+        return out
+
+
+def direct(pos, mass, eps: float, targets=None):
+    """fp64 direct summation: (acc [n_t,3], pot [n_t])."""
+    L = _load()
+    pos = np.ascontiguousarray(pos, dtype=np.float32)
+    mass = np.ascontiguousarray(mass, dtype=np.float32)
+    n = pos.shape[0]
+    t = None if targets is None else np.ascontiguousarray(targets, dtype=np.int64)
+    nt = n if t is None else t.size
+    acc = np.zeros((nt, 3))
+    pot = np.zeros(nt)
+    L.orc_direct(n, _p(pos), _p(mass), float(eps), nt, _p(t), _p(acc), _p(pot))
+    return acc, pot
