@@ -1,0 +1,148 @@
+/* ============================================================================
+ *  tc.h — C ABI of the B200-native tree-code force calculation
+ *  (hot path of arXiv 1005.5384, Gaburov, Bedorf & Portegies Zwart, ICCS 2010).
+ *
+ *  What the library computes (citations are /root/reference/PAPER.md lines):
+ *    - host: octree by recursive cubic subdivision down to N_leaf,
+ *      tight bounding boxes -> boundary cubes (Fig. 1), mass, centre
+ *      of mass and quadrupole moments per cell, groups,
+ *      packed into SoA float4 arrays and moved in ONE bulk copy;
+ *    - device (sm_100a): per group, the non-recursive stack walk with the opening
+ *      test on cell boundaries (Sec. 2.2, List 2) fused with the
+ *      evaluation of the interaction lists as particle-cell (monopole + quadrupole)
+ *      and particle-particle softened gravity (Sec. 2.3, Lists 3-4).
+ *  The exact formulae (the paper only cites them) are the readings O1-O6 / R1-R18
+ *  listed in DESIGN.md section 3.
+ *
+ *  Conventions: G = 1; every function is thread-compatible per context (one
+ *  thread at a time per tc_ctx); no function throws or aborts; all int-returning
+ *  functions return TC_OK (0) or a negative TC_E* code and keep a message that
+ *  tc_last_error() returns.  There is NO CPU fallback: without a CUDA device
+ *  tc_create() returns NULL and tc_forces() cannot be reached.
+ * ========================================================================== */
+#ifndef TC_H_
+#define TC_H_
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct tc_ctx tc_ctx;
+
+enum {
+  TC_OK = 0,
+  TC_EINVAL = -1,    /* bad argument (null, out of range, non-finite)            */
+  TC_ESTATE = -2,    /* call order: no particles / no tree / host-only context   */
+  TC_ECUDA = -3,     /* a CUDA runtime call or kernel failed; see tc_last_error  */
+  TC_ENOMEM = -4,    /* host or device allocation failed                         */
+  TC_EOVERFLOW = -5  /* a device-side walk stack exceeded its spill capacity     */
+};
+
+/* tc_create_ex flags */
+#define TC_FLAG_HOST_ONLY 1u /* no device: set_particles/build/get_tree work (host
+                                builder tests); tc_forces returns TC_ESTATE.      */
+
+/* Tree / timing statistics, filled by tc_get_stats.  Times follow the paper's
+ * split T_host / T_GPU plus the copy.                        */
+typedef struct tc_stats {
+  int64_t n;              /* particles                                            */
+  int64_t n_cells;        /* cells in the tree (nodes + leaves, root included)    */
+  int64_t n_leaves;
+  int64_t n_groups;
+  int32_t depth;          /* deepest level (root = 0)                             */
+  int32_t n_leaf;         /* N_leaf of the last tc_build                          */
+  int32_t n_group;        /* N_group of the last tc_build                         */
+  int32_t reserved;
+  int64_t n_pc_total;     /* sum over particles of particle-cell interactions of
+                             the last tc_forces                                   */
+  int64_t n_pp_total;     /* same, particle-particle (self excluded)              */
+  int64_t n_tests_total;  /* opening tests of the last tc_forces (sum over groups)*/
+  int64_t n_spills;       /* walk-stack spills to global memory (last tc_forces)  */
+  double t_host_ms;       /* last tc_build: host tree + moments + pack            */
+  double t_copy_ms;       /* last tc_build: bulk host->device copy (wall)         */
+  double t_gpu_ms;        /* last tc_forces: device time of the force kernel(s),
+                             CUDA events on the context's stream                  */
+  int64_t tree_bytes;     /* bytes of the single bulk H2D copy of tc_build        */
+} tc_stats;
+
+/* Select the current CUDA device, create the context and its stream.
+ * Returns NULL on failure (no device, out of memory).  Multiple contexts are
+ * allowed; there is no global state.                                            */
+tc_ctx* tc_create(void);
+tc_ctx* tc_create_ex(uint32_t flags);
+
+/* Free everything owned by the context.  NULL is a no-op.                       */
+void tc_destroy(tc_ctx* ctx);
+
+/* Particles (the host owns allocation and transfers).
+ *   pos  : n x 3 fp32, row-major (x,y,z)        mass : n fp32
+ * HOST or DEVICE pointers (resolved with cudaPointerGetAttributes).  The data is
+ * COPIED; the caller may free or overwrite it on return.  Invalidates the tree.
+ * Errors: TC_EINVAL (null, n < 1, n > 2^31-1, non-finite position, negative or
+ * non-finite mass).                                                             */
+int tc_set_particles(tc_ctx* ctx, const float* pos, const float* mass, int64_t n);
+
+/* Host octree: root cube, recursive 8-way split until a cell
+ * holds <= n_leaf particles (or level 21), tight bounding boxes, boundary cubes,
+ * fp64 moments rounded to fp32, groups (N_group from tc_set_option, default 64),
+ * SoA float4 packing, one bulk host->device copy.
+ * Errors: TC_ESTATE (no particles), TC_EINVAL (n_leaf < 1), TC_ENOMEM, TC_ECUDA. */
+int tc_build(tc_ctx* ctx, int n_leaf);
+
+/* The hot path: for every group walk the tree with opening
+ * angle theta, evaluate particle-cell (monopole+quadrupole) and particle-particle
+ * Plummer-softened interactions, write accelerations and potentials.
+ *   acc : n x 3 fp32 (ax,ay,az), pot : n fp32 or NULL — CALLER-ALLOCATED, host or
+ *   device, in the CALLER's particle order.
+ * Host pointers: synchronous on return.  Device pointers: stream-ordered on the
+ * context's stream (tc_set_stream); errors of the kernel surface at tc_sync().
+ * Errors: TC_ESTATE (tree not built / host-only), TC_EINVAL (theta < 0, eps < 0,
+ * non-finite, acc NULL), TC_ECUDA, TC_EOVERFLOW.                                 */
+int tc_forces(tc_ctx* ctx, float theta, float eps, float* acc, float* pot);
+
+/* Options (double-valued).  Keys:
+ *   "n_group"     N_group >= 1; takes effect at the next tc_build
+ *   "stack_smem"  walk-stack entries kept in shared memory per warp before
+ *                 spilling to global memory: 512 (default) or 64 (test of the
+ *                 spill path)
+ * Unknown key or bad value -> TC_EINVAL.                                        */
+int tc_set_option(tc_ctx* ctx, const char* key, double value);
+
+/* Per-particle interaction counts of the last tc_forces, caller's order:
+ * n_pc = |cell list of the particle's group|, n_pp = bodies of the opened leaves
+ * minus the particle itself.  HOST pointers, n int32 each; either may be NULL.
+ * Synchronises the context's stream.                                            */
+int tc_get_counts(tc_ctx* ctx, int32_t* n_pc, int32_t* n_pp);
+
+int tc_get_stats(tc_ctx* ctx, tc_stats* out);
+
+/* Use the caller's CUDA stream (a cudaStream_t passed as void*; NULL = the
+ * context's own stream).  The context never destroys a caller's stream.         */
+int tc_set_stream(tc_ctx* ctx, void* cuda_stream);
+
+/* Block until all work queued by this context has finished; returns TC_ECUDA /
+ * TC_EOVERFLOW if the last stream-ordered tc_forces failed.                      */
+int tc_sync(tc_ctx* ctx);
+
+/* Message of the last error of this context ("" if none).  Owned by the context.
+ * ctx == NULL returns the message of the last failed tc_create.                  */
+const char* tc_last_error(const tc_ctx* ctx);
+
+/* Inspection of the packed host tree of the last tc_build (tests of the host
+ * builder; no device needed).  Every pointer is a HOST array or NULL:
+ *   perm      [n]          original index of the i-th particle in tree (Morton) order
+ *   cell_bnd  [n_cells,4]  boundary cube (bx,by,bz,h), h >= 0            (Fig. 1)
+ *   cell_xm   [n_cells,4]  centre of mass and mass (X,Y,Z,M)
+ *   cell_q    [n_cells,6]  traceless quadrupole xx,yy,zz,xy,xz,yz
+ *   cell_link [n_cells,4]  first_child, n_child (0 = leaf), first_body, n_body
+ *   groups    [n_groups]   cell id of every group, Morton order
+ * Sizes come from tc_get_stats.                                                 */
+int tc_get_tree(tc_ctx* ctx, int32_t* perm, float* cell_bnd, float* cell_xm, float* cell_q,
+                int32_t* cell_link, int32_t* groups);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* TC_H_ */

@@ -1,0 +1,216 @@
+"""Thin Python binding of the C ABI in include/tc.h — argument marshalling only.
+
+Same names as the C functions (``tc_create`` ... ``tc_destroy``) plus a small
+``TreeCode`` convenience class.  Every step of the hot path runs inside
+``libtc_b200.so`` (hand-written CUDA for sm_100a); there is no Python or CPU
+fallback: if the library is missing or no CUDA device exists, calls raise.
+
+Arrays may be numpy arrays (host pointers) or torch CUDA tensors (device
+pointers, passed as ``data_ptr()``); PyTorch is used for device memory and
+streams only.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libtc_b200.so")
+
+TC_OK, TC_EINVAL, TC_ESTATE, TC_ECUDA, TC_ENOMEM, TC_EOVERFLOW = 0, -1, -2, -3, -4, -5
+TC_FLAG_HOST_ONLY = 1
+
+#: every symbol include/tc.h declares (checked by tests/test_abi.py)
+SYMBOLS = ["tc_create", "tc_create_ex", "tc_destroy", "tc_set_particles", "tc_build", "tc_forces",
+           "tc_set_option", "tc_get_counts", "tc_get_stats", "tc_set_stream", "tc_sync",
+           "tc_last_error", "tc_get_tree"]
+
+
+class tc_stats(C.Structure):
+    _fields_ = [("n", C.c_int64), ("n_cells", C.c_int64), ("n_leaves", C.c_int64), ("n_groups", C.c_int64),
+                ("depth", C.c_int32), ("n_leaf", C.c_int32), ("n_group", C.c_int32), ("reserved", C.c_int32),
+                ("n_pc_total", C.c_int64), ("n_pp_total", C.c_int64), ("n_tests_total", C.c_int64),
+                ("n_spills", C.c_int64), ("t_host_ms", C.c_double), ("t_copy_ms", C.c_double),
+                ("t_gpu_ms", C.c_double), ("tree_bytes", C.c_int64)]
+
+    def asdict(self):
+        return {k: getattr(self, k) for k, _ in self._fields_ if k != "reserved"}
+
+
+class TcError(RuntimeError):
+    def __init__(self, code, msg):
+        super().__init__(f"tc error {code}: {msg}")
+        self.code = code
+
+
+_lib = None
+
+
+def lib():
+    """Load libtc_b200.so (built by ``paper_1005_5384_b200.build``); fail loudly if absent."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(LIB_PATH):
+        raise ImportError(f"{LIB_PATH} is missing: run `python -m paper_1005_5384_b200.build` "
+                          "(there is no Python/CPU fallback for the CUDA path)")
+    L = C.CDLL(LIB_PATH)
+    vp, i64, i32, f32, f64 = C.c_void_p, C.c_int64, C.c_int, C.c_float, C.c_double
+    L.tc_create.restype = vp
+    L.tc_create.argtypes = []
+    L.tc_create_ex.restype = vp
+    L.tc_create_ex.argtypes = [C.c_uint32]
+    L.tc_destroy.restype = None
+    L.tc_destroy.argtypes = [vp]
+    L.tc_set_particles.argtypes = [vp, vp, vp, i64]
+    L.tc_build.argtypes = [vp, i32]
+    L.tc_forces.argtypes = [vp, f32, f32, vp, vp]
+    L.tc_set_option.argtypes = [vp, C.c_char_p, f64]
+    L.tc_get_counts.argtypes = [vp, vp, vp]
+    L.tc_get_stats.argtypes = [vp, C.POINTER(tc_stats)]
+    L.tc_set_stream.argtypes = [vp, vp]
+    L.tc_sync.argtypes = [vp]
+    L.tc_last_error.restype = C.c_char_p
+    L.tc_last_error.argtypes = [vp]
+    L.tc_get_tree.argtypes = [vp] + [vp] * 6
+    _lib = L
+    return L
+
+
+def _ptr(a):
+    """Raw pointer of a numpy array (host) or a torch tensor (host or device); None -> NULL."""
+    if a is None:
+        return None
+    if isinstance(a, np.ndarray):
+        assert a.flags["C_CONTIGUOUS"], "array must be C-contiguous"
+        return C.c_void_p(a.ctypes.data)
+    if hasattr(a, "data_ptr"):
+        assert a.is_contiguous(), "tensor must be contiguous"
+        return C.c_void_p(a.data_ptr())
+    raise TypeError(f"unsupported buffer type {type(a)}")
+
+
+def _check(ctx, rc):
+    if rc != TC_OK:
+        raise TcError(rc, lib().tc_last_error(ctx).decode())
+
+
+# ---- the C functions, one to one ------------------------------------------------
+def tc_create(flags: int = 0):
+    ctx = lib().tc_create_ex(flags)
+    if not ctx:
+        raise TcError(TC_ECUDA, lib().tc_last_error(None).decode())
+    return ctx
+
+
+def tc_destroy(ctx):
+    lib().tc_destroy(ctx)
+
+
+def tc_set_particles(ctx, pos, mass, n=None):
+    n = int(pos.shape[0]) if n is None else int(n)
+    _check(ctx, lib().tc_set_particles(ctx, _ptr(pos), _ptr(mass), n))
+
+
+def tc_build(ctx, n_leaf: int):
+    _check(ctx, lib().tc_build(ctx, int(n_leaf)))
+
+
+def tc_forces(ctx, theta: float, eps: float, acc, pot=None):
+    _check(ctx, lib().tc_forces(ctx, float(theta), float(eps), _ptr(acc), _ptr(pot)))
+
+
+def tc_set_option(ctx, key: str, value: float):
+    _check(ctx, lib().tc_set_option(ctx, key.encode(), float(value)))
+
+
+def tc_get_counts(ctx, n: int):
+    n_pc = np.zeros(n, np.int32)
+    n_pp = np.zeros(n, np.int32)
+    _check(ctx, lib().tc_get_counts(ctx, _ptr(n_pc), _ptr(n_pp)))
+    return n_pc, n_pp
+
+
+def tc_get_stats(ctx) -> dict:
+    s = tc_stats()
+    _check(ctx, lib().tc_get_stats(ctx, C.byref(s)))
+    return s.asdict()
+
+
+def tc_set_stream(ctx, cuda_stream: int):
+    _check(ctx, lib().tc_set_stream(ctx, C.c_void_p(cuda_stream)))
+
+
+def tc_sync(ctx):
+    _check(ctx, lib().tc_sync(ctx))
+
+
+def tc_get_tree(ctx) -> dict:
+    s = tc_get_stats(ctx)
+    n, nc, ng = s["n"], s["n_cells"], s["n_groups"]
+    out = dict(perm=np.zeros(n, np.int32), bnd=np.zeros((nc, 4), np.float32), xm=np.zeros((nc, 4), np.float32),
+               q=np.zeros((nc, 6), np.float32), link=np.zeros((nc, 4), np.int32), groups=np.zeros(ng, np.int32))
+    _check(ctx, lib().tc_get_tree(ctx, *[_ptr(out[k]) for k in ("perm", "bnd", "xm", "q", "link", "groups")]))
+    return out
+
+
+class TreeCode:
+    """Context manager around one tc_ctx (marshalling only)."""
+
+    def __init__(self, host_only: bool = False, n_group: int | None = None):
+        self.ctx = tc_create(TC_FLAG_HOST_ONLY if host_only else 0)
+        self.n = 0
+        if n_group is not None:
+            self.set_option("n_group", n_group)
+
+    def close(self):
+        if self.ctx:
+            tc_destroy(self.ctx)
+            self.ctx = None
+
+    def __enter__(self):
+        return self
+
+    def __exit__(self, *a):
+        self.close()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def set_option(self, key, value):
+        tc_set_option(self.ctx, key, value)
+
+    def set_particles(self, pos, mass):
+        self.n = int(pos.shape[0])
+        tc_set_particles(self.ctx, pos, mass, self.n)
+
+    def build(self, n_leaf: int = 16):
+        tc_build(self.ctx, n_leaf)
+
+    def forces(self, theta, eps, acc=None, pot=None):
+        """Host path: allocates numpy outputs if none are given and returns (acc, pot)."""
+        if acc is None:
+            acc = np.empty((self.n, 3), np.float32)
+            pot = np.empty(self.n, np.float32)
+        tc_forces(self.ctx, theta, eps, acc, pot)
+        return acc, pot
+
+    def counts(self):
+        return tc_get_counts(self.ctx, self.n)
+
+    def stats(self):
+        return tc_get_stats(self.ctx)
+
+    def tree(self):
+        return tc_get_tree(self.ctx)
+
+    def sync(self):
+        tc_sync(self.ctx)
+
+    def set_stream(self, s):
+        tc_set_stream(self.ctx, s)

@@ -1,0 +1,328 @@
+// C ABI of the tree-code library (include/tc.h): context, particle intake, host
+// build + one bulk copy, launch of the fused walk+evaluate kernel, results.
+// There is no CPU fallback anywhere in this file: without a device tc_create()
+// fails, and a host-only context (tests of the host builder) refuses tc_forces.
+#include <cuda_runtime.h>
+
+#include <chrono>
+#include <cmath>
+#include <cstdio>
+#include <cstdlib>
+#include <cstring>
+#include <string>
+#include <vector>
+
+#include "tc_internal.h"
+
+struct tc_ctx {
+  uint32_t flags = 0;
+  bool host_only = false;
+  int device = 0, n_sm = 148;
+  cudaStream_t own_stream = nullptr, stream = nullptr;
+  cudaEvent_t ev0 = nullptr, ev1 = nullptr;
+  std::string err;
+  // options
+  int n_group = 64;
+  int stack_smem = 512;
+  // particles (host copy, caller order)
+  std::vector<float> pos, mass;
+  int64_t n = 0;
+  // tree
+  tc::HostTree tree;
+  bool built = false;
+  void* d_tree = nullptr;
+  size_t d_tree_cap = 0;
+  tc::DeviceTree dview;
+  // outputs / scratch on the device
+  float* d_acc = nullptr; float* d_pot = nullptr; int64_t out_cap = 0;
+  int32_t* d_npc = nullptr; int32_t* d_npp = nullptr; int64_t cnt_cap = 0;
+  tc::DeviceCounters* d_ctr = nullptr;
+  uint32_t* d_spill = nullptr; size_t spill_elems = 0; int spill_cap = 4096;
+  bool forces_done = false, timing_pending = false;
+  tc_stats stats{};
+};
+
+namespace {
+
+thread_local std::string g_create_err;
+
+int fail(tc_ctx* c, int code, const std::string& m) { if (c) c->err = m; return code; }
+int cuda_fail(tc_ctx* c, cudaError_t e, const char* what) {
+  return fail(c, e == cudaErrorMemoryAllocation ? TC_ENOMEM : TC_ECUDA,
+              std::string(what) + ": " + cudaGetErrorString(e));
+}
+#define TC_CUDA(c, call) do { cudaError_t e_ = (call); if (e_ != cudaSuccess) return cuda_fail(c, e_, #call); } while (0)
+
+bool is_device_ptr(const tc_ctx* c, const void* p) {
+  if (c->host_only || !p) return false;
+  cudaPointerAttributes a;
+  if (cudaPointerGetAttributes(&a, p) != cudaSuccess) { cudaGetLastError(); return false; }
+  return a.type == cudaMemoryTypeDevice || a.type == cudaMemoryTypeManaged;
+}
+
+void* packed_alloc(void* user, size_t bytes) {
+  tc_ctx* c = (tc_ctx*)user;
+  tc::HostTree& T = c->tree;
+  if (T.packed && T.packed_cap >= bytes) return T.packed;
+  if (T.packed) { if (T.packed_pinned) cudaFreeHost(T.packed); else std::free(T.packed); T.packed = nullptr; T.packed_cap = 0; }
+  const size_t cap = bytes + bytes / 8;
+  if (!c->host_only) {
+    void* p = nullptr;
+    if (cudaHostAlloc(&p, cap, cudaHostAllocDefault) == cudaSuccess) { T.packed = p; T.packed_cap = cap; T.packed_pinned = true; return p; }
+    cudaGetLastError();
+  }
+  T.packed = std::malloc(cap); T.packed_pinned = false; T.packed_cap = T.packed ? cap : 0;
+  return T.packed;
+}
+
+double now_ms() {
+  return std::chrono::duration<double, std::milli>(std::chrono::steady_clock::now().time_since_epoch()).count();
+}
+
+// read the device counters + event time of the last tc_forces into stats (stream must be idle)
+int collect(tc_ctx* c) {
+  if (!c->timing_pending) return TC_OK;
+  c->timing_pending = false;
+  tc::DeviceCounters h;
+  TC_CUDA(c, cudaMemcpy(&h, c->d_ctr, sizeof(h), cudaMemcpyDeviceToHost));
+  float ms = 0.f;
+  TC_CUDA(c, cudaEventElapsedTime(&ms, c->ev0, c->ev1));
+  c->stats.t_gpu_ms = ms;
+  c->stats.n_pc_total = (int64_t)h.n_pc_total; c->stats.n_pp_total = (int64_t)h.n_pp_total;
+  c->stats.n_tests_total = (int64_t)h.n_tests_total; c->stats.n_spills = (int64_t)h.n_spills;
+  if (h.overflow) return fail(c, TC_EOVERFLOW, "tc_forces: a walk stack exceeded its global spill capacity");
+  return TC_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+tc_ctx* tc_create_ex(uint32_t flags) {
+  tc_ctx* c = new (std::nothrow) tc_ctx();
+  if (!c) { g_create_err = "tc_create: out of host memory"; return nullptr; }
+  c->flags = flags;
+  c->host_only = (flags & TC_FLAG_HOST_ONLY) != 0;
+  if (c->host_only) return c;
+  cudaError_t e = cudaGetDevice(&c->device);
+  if (e == cudaSuccess) e = cudaFree(0);
+  cudaDeviceProp prop;
+  if (e == cudaSuccess) e = cudaGetDeviceProperties(&prop, c->device);
+  if (e == cudaSuccess && prop.major < 10) {
+    g_create_err = "tc_create: this library is built for sm_100a (B200) only; device is sm_" +
+                   std::to_string(prop.major) + std::to_string(prop.minor);
+    delete c; return nullptr;
+  }
+  if (e == cudaSuccess) { c->n_sm = prop.multiProcessorCount; e = cudaStreamCreateWithFlags(&c->own_stream, cudaStreamNonBlocking); }
+  if (e == cudaSuccess) e = cudaEventCreate(&c->ev0);
+  if (e == cudaSuccess) e = cudaEventCreate(&c->ev1);
+  if (e == cudaSuccess) e = cudaMalloc((void**)&c->d_ctr, sizeof(tc::DeviceCounters));
+  if (e != cudaSuccess) {
+    g_create_err = std::string("tc_create: no usable CUDA device (no CPU fallback exists): ") + cudaGetErrorString(e);
+    cudaGetLastError();
+    tc_destroy(c); return nullptr;
+  }
+  c->stream = c->own_stream;
+  return c;
+}
+
+tc_ctx* tc_create(void) { return tc_create_ex(0); }
+
+void tc_destroy(tc_ctx* c) {
+  if (!c) return;
+  if (!c->host_only) {
+    if (c->stream) cudaStreamSynchronize(c->stream);
+    cudaFree(c->d_tree); cudaFree(c->d_acc); cudaFree(c->d_pot); cudaFree(c->d_npc); cudaFree(c->d_npp);
+    cudaFree(c->d_ctr); cudaFree(c->d_spill);
+    if (c->ev0) cudaEventDestroy(c->ev0);
+    if (c->ev1) cudaEventDestroy(c->ev1);
+    if (c->own_stream) cudaStreamDestroy(c->own_stream);
+  }
+  if (c->tree.packed) { if (c->tree.packed_pinned) cudaFreeHost(c->tree.packed); else std::free(c->tree.packed); }
+  delete c;
+}
+
+const char* tc_last_error(const tc_ctx* c) { return c ? c->err.c_str() : g_create_err.c_str(); }
+
+int tc_set_option(tc_ctx* c, const char* key, double v) {
+  if (!c || !key) return fail(c, TC_EINVAL, "tc_set_option: null argument");
+  if (!std::strcmp(key, "n_group")) {
+    if (!(v >= 1.0) || v > 2147483647.0 || v != std::floor(v)) return fail(c, TC_EINVAL, "tc_set_option: n_group must be an integer >= 1");
+    c->n_group = (int)v; return TC_OK;
+  }
+  if (!std::strcmp(key, "stack_smem")) {
+    if (v != 512.0 && v != 64.0) return fail(c, TC_EINVAL, "tc_set_option: stack_smem must be 512 or 64");
+    c->stack_smem = (int)v; return TC_OK;
+  }
+  return fail(c, TC_EINVAL, std::string("tc_set_option: unknown key '") + key + "'");
+}
+
+int tc_set_stream(tc_ctx* c, void* s) {
+  if (!c) return TC_EINVAL;
+  if (c->host_only) return fail(c, TC_ESTATE, "tc_set_stream: host-only context");
+  TC_CUDA(c, cudaStreamSynchronize(c->stream));
+  c->stream = s ? (cudaStream_t)s : c->own_stream;
+  return TC_OK;
+}
+
+int tc_sync(tc_ctx* c) {
+  if (!c) return TC_EINVAL;
+  if (c->host_only) return TC_OK;
+  TC_CUDA(c, cudaStreamSynchronize(c->stream));
+  return collect(c);
+}
+
+int tc_set_particles(tc_ctx* c, const float* pos, const float* mass, int64_t n) {
+  if (!c) return TC_EINVAL;
+  if (!pos || !mass) return fail(c, TC_EINVAL, "tc_set_particles: null pointer");
+  if (n < 1 || n > 2147483647LL) return fail(c, TC_EINVAL, "tc_set_particles: n must be in [1, 2^31-1]");
+  c->built = false; c->forces_done = false;
+  try { c->pos.resize((size_t)n * 3); c->mass.resize((size_t)n); } catch (...) { return fail(c, TC_ENOMEM, "tc_set_particles: out of host memory"); }
+  if (is_device_ptr(c, pos)) { TC_CUDA(c, cudaMemcpyAsync(c->pos.data(), pos, sizeof(float) * 3 * (size_t)n, cudaMemcpyDeviceToHost, c->stream)); }
+  else std::memcpy(c->pos.data(), pos, sizeof(float) * 3 * (size_t)n);
+  if (is_device_ptr(c, mass)) { TC_CUDA(c, cudaMemcpyAsync(c->mass.data(), mass, sizeof(float) * (size_t)n, cudaMemcpyDeviceToHost, c->stream)); }
+  else std::memcpy(c->mass.data(), mass, sizeof(float) * (size_t)n);
+  if (!c->host_only) TC_CUDA(c, cudaStreamSynchronize(c->stream));
+  bool bad_pos = false, bad_mass = false;
+  const float* P = c->pos.data(); const float* M = c->mass.data();
+#pragma omp parallel for schedule(static) reduction(| : bad_pos, bad_mass)
+  for (int64_t i = 0; i < n; i++) {
+    bad_pos |= !(std::isfinite(P[3 * i]) && std::isfinite(P[3 * i + 1]) && std::isfinite(P[3 * i + 2]));
+    bad_mass |= !(std::isfinite(M[i]) && M[i] >= 0.f);
+  }
+  c->n = 0;
+  if (bad_pos) return fail(c, TC_EINVAL, "tc_set_particles: non-finite position");
+  if (bad_mass) return fail(c, TC_EINVAL, "tc_set_particles: negative or non-finite mass");
+  c->n = n;
+  return TC_OK;
+}
+
+int tc_build(tc_ctx* c, int n_leaf) {
+  if (!c) return TC_EINVAL;
+  if (c->n < 1) return fail(c, TC_ESTATE, "tc_build: no particles (call tc_set_particles first)");
+  if (n_leaf < 1) return fail(c, TC_EINVAL, "tc_build: n_leaf must be >= 1");
+  c->built = false; c->forces_done = false;
+  if (!c->host_only) TC_CUDA(c, cudaStreamSynchronize(c->stream));  // the pinned buffer may still be in flight
+  const double t0 = now_ms();
+  std::string msg;
+  const int rc = tc::build_host_tree(c->pos.data(), c->mass.data(), c->n, n_leaf, c->n_group, c->tree, packed_alloc, c, msg);
+  if (rc != TC_OK) return fail(c, rc, msg);
+  const double t1 = now_ms();
+  const tc::HostTree& T = c->tree;
+  tc_stats& S = c->stats;
+  S = tc_stats{};
+  S.n = c->n; S.n_cells = T.n_cells; S.n_leaves = T.n_leaves; S.n_groups = T.n_groups; S.depth = T.depth;
+  S.n_leaf = n_leaf; S.n_group = c->n_group; S.t_host_ms = t1 - t0; S.tree_bytes = (int64_t)T.lay.bytes;
+  if (!c->host_only) {
+    if (c->d_tree_cap < T.lay.bytes) {
+      cudaFree(c->d_tree); c->d_tree = nullptr; c->d_tree_cap = 0;
+      const size_t cap = T.lay.bytes + T.lay.bytes / 8;
+      TC_CUDA(c, cudaMalloc(&c->d_tree, cap));
+      c->d_tree_cap = cap;
+    }
+    // the ONE bulk copy ("only the tree structure needs to travel")
+    TC_CUDA(c, cudaMemcpyAsync(c->d_tree, T.packed, T.lay.bytes, cudaMemcpyHostToDevice, c->stream));
+    TC_CUDA(c, cudaStreamSynchronize(c->stream));
+    S.t_copy_ms = now_ms() - t1;
+    char* b = (char*)c->d_tree;
+    tc::DeviceTree& D = c->dview;
+    D.bnd = (const float4*)(b + T.lay.off_bnd); D.xm = (const float4*)(b + T.lay.off_xm);
+    D.q0 = (const float4*)(b + T.lay.off_q0); D.q1 = (const float4*)(b + T.lay.off_q1);
+    D.part = (const float4*)(b + T.lay.off_part); D.orig = (const int32_t*)(b + T.lay.off_orig);
+    D.grp = (const int4*)(b + T.lay.off_grp);
+    D.n = c->n; D.n_cells = T.n_cells; D.n_groups = T.n_groups;
+  }
+  c->built = true;
+  return TC_OK;
+}
+
+int tc_forces(tc_ctx* c, float theta, float eps, float* acc, float* pot) {
+  if (!c) return TC_EINVAL;
+  if (c->host_only) return fail(c, TC_ESTATE, "tc_forces: host-only context has no device (there is no CPU fallback)");
+  if (!c->built) return fail(c, TC_ESTATE, "tc_forces: no tree (call tc_build first)");
+  if (!acc) return fail(c, TC_EINVAL, "tc_forces: acc is null");
+  if (!(theta >= 0.f) || !std::isfinite(theta) || !(eps >= 0.f) || !std::isfinite(eps))
+    return fail(c, TC_EINVAL, "tc_forces: theta and eps must be finite and >= 0");
+  const int64_t n = c->n;
+  const bool acc_dev = is_device_ptr(c, acc), pot_dev = pot ? is_device_ptr(c, pot) : acc_dev;
+  if (pot && acc_dev != pot_dev) return fail(c, TC_EINVAL, "tc_forces: acc and pot must both be host or both be device pointers");
+  if (c->timing_pending) { TC_CUDA(c, cudaStreamSynchronize(c->stream)); const int rc = collect(c); if (rc != TC_OK && rc != TC_EOVERFLOW) return rc; }
+  if (c->cnt_cap < n) {
+    cudaFree(c->d_npc); cudaFree(c->d_npp); c->d_npc = c->d_npp = nullptr; c->cnt_cap = 0;
+    TC_CUDA(c, cudaMalloc((void**)&c->d_npc, sizeof(int32_t) * (size_t)n));
+    TC_CUDA(c, cudaMalloc((void**)&c->d_npp, sizeof(int32_t) * (size_t)n));
+    c->cnt_cap = n;
+  }
+  if (!acc_dev && c->out_cap < n) {
+    cudaFree(c->d_acc); cudaFree(c->d_pot); c->d_acc = c->d_pot = nullptr; c->out_cap = 0;
+    TC_CUDA(c, cudaMalloc((void**)&c->d_acc, sizeof(float) * 3 * (size_t)n));
+    TC_CUDA(c, cudaMalloc((void**)&c->d_pot, sizeof(float) * (size_t)n));
+    c->out_cap = n;
+  }
+  const size_t warps = (size_t)tc::forces_total_warps(c->n_sm, c->stack_smem);
+  if (c->spill_elems < warps * (size_t)c->spill_cap) {
+    cudaFree(c->d_spill); c->d_spill = nullptr; c->spill_elems = 0;
+    TC_CUDA(c, cudaMalloc((void**)&c->d_spill, sizeof(uint32_t) * warps * (size_t)c->spill_cap));
+    c->spill_elems = warps * (size_t)c->spill_cap;
+  }
+  tc::ForceLaunch L;
+  L.theta = theta; L.eps = eps;
+  L.acc = acc_dev ? acc : c->d_acc;
+  L.pot = pot ? (acc_dev ? pot : c->d_pot) : nullptr;
+  L.n_pc = c->d_npc; L.n_pp = c->d_npp; L.counters = c->d_ctr; L.spill = c->d_spill; L.spill_cap = c->spill_cap;
+  L.stack_smem = c->stack_smem; L.n_sm = c->n_sm;
+  TC_CUDA(c, cudaMemsetAsync(c->d_ctr, 0, sizeof(tc::DeviceCounters), c->stream));
+  TC_CUDA(c, cudaEventRecord(c->ev0, c->stream));
+  const int le = tc::launch_forces(c->dview, L, c->stream);
+  if (le != 0) return cuda_fail(c, (cudaError_t)le, "forces kernel launch");
+  TC_CUDA(c, cudaEventRecord(c->ev1, c->stream));
+  c->timing_pending = true; c->forces_done = true;
+  if (!acc_dev) {
+    TC_CUDA(c, cudaMemcpyAsync(acc, c->d_acc, sizeof(float) * 3 * (size_t)n, cudaMemcpyDeviceToHost, c->stream));
+    if (pot) TC_CUDA(c, cudaMemcpyAsync(pot, c->d_pot, sizeof(float) * (size_t)n, cudaMemcpyDeviceToHost, c->stream));
+    TC_CUDA(c, cudaStreamSynchronize(c->stream));
+    return collect(c);
+  }
+  return TC_OK;
+}
+
+int tc_get_counts(tc_ctx* c, int32_t* n_pc, int32_t* n_pp) {
+  if (!c) return TC_EINVAL;
+  if (!c->forces_done) return fail(c, TC_ESTATE, "tc_get_counts: no tc_forces since the last tc_build");
+  TC_CUDA(c, cudaStreamSynchronize(c->stream));
+  if (n_pc) TC_CUDA(c, cudaMemcpy(n_pc, c->d_npc, sizeof(int32_t) * (size_t)c->n, cudaMemcpyDeviceToHost));
+  if (n_pp) TC_CUDA(c, cudaMemcpy(n_pp, c->d_npp, sizeof(int32_t) * (size_t)c->n, cudaMemcpyDeviceToHost));
+  return collect(c);
+}
+
+int tc_get_stats(tc_ctx* c, tc_stats* out) {
+  if (!c || !out) return fail(c, TC_EINVAL, "tc_get_stats: null argument");
+  int rc = TC_OK;
+  if (!c->host_only && c->timing_pending) { TC_CUDA(c, cudaStreamSynchronize(c->stream)); rc = collect(c); }
+  *out = c->stats;
+  return rc;
+}
+
+int tc_get_tree(tc_ctx* c, int32_t* perm, float* cell_bnd, float* cell_xm, float* cell_q, int32_t* cell_link,
+                int32_t* groups) {
+  if (!c) return TC_EINVAL;
+  if (!c->built) return fail(c, TC_ESTATE, "tc_get_tree: no tree (call tc_build first)");
+  const tc::HostTree& T = c->tree;
+  const char* b = (const char*)T.packed;
+  const size_t nc = (size_t)T.n_cells;
+  if (perm) std::memcpy(perm, b + T.lay.off_orig, sizeof(int32_t) * (size_t)T.n);
+  if (cell_bnd) {
+    std::memcpy(cell_bnd, b + T.lay.off_bnd, sizeof(float) * 4 * nc);
+    for (size_t i = 0; i < nc; i++) cell_bnd[4 * i + 3] = std::fabs(cell_bnd[4 * i + 3]);  // drop the leaf flag
+  }
+  if (cell_xm) std::memcpy(cell_xm, b + T.lay.off_xm, sizeof(float) * 4 * nc);
+  if (cell_q) std::memcpy(cell_q, T.q6.data(), sizeof(float) * 6 * nc);
+  if (cell_link) std::memcpy(cell_link, T.link.data(), sizeof(int32_t) * 4 * nc);
+  if (groups) {
+    const int4* g = (const int4*)(b + T.lay.off_grp);
+    for (int64_t i = 0; i < T.n_groups; i++) groups[i] = g[i].x;
+  }
+  return TC_OK;
+}
+
+}  // extern "C"

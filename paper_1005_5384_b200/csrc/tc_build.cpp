@@ -1,0 +1,346 @@
+// Host octree builder of the B200 tree-code (step A0 of DESIGN.md).
+//
+// The paper keeps tree construction and multipole moments on the host
+// (PAPER.md:17,41); so does this library.  Unlike the paper's sequential builder
+// this one is a Morton-key radix sort followed by a level-by-level
+// (breadth-first) split of sorted key ranges, OpenMP-parallel inside each level,
+// and a bottom-up parallel-axis accumulation of the fp64 moments.  Cells come out
+// in breadth-first order with the children of a node contiguous, which is what the
+// walk kernel wants: the 8 child tests of a node are 8 adjacent float4 loads.
+//
+// Readings: O1 root cube + integer grid, O2 leaf iff count <=
+// N_leaf or level 21, children = non-empty octants in order 4bx+2by+bz, O3 tight
+// bbox -> boundary cube, mass, COM, traceless quadrupole, O4 groups.
+#include <algorithm>
+#include <cmath>
+#include <cstring>
+#include <limits>
+
+#ifdef _OPENMP
+#include <omp.h>
+#endif
+
+#include "tc_internal.h"
+
+namespace tc {
+namespace {
+
+inline uint64_t spread21(uint64_t v) {  // bit i -> bit 3i
+  v &= 0x1fffffull;
+  v = (v | (v << 32)) & 0x1f00000000ffffull;
+  v = (v | (v << 16)) & 0x1f0000ff0000ffull;
+  v = (v | (v << 8)) & 0x100f00f00f00f00full;
+  v = (v | (v << 4)) & 0x10c30c30c30c30c3ull;
+  v = (v | (v << 2)) & 0x1249249249249249ull;
+  return v;
+}
+
+struct KeyIdx {
+  uint64_t key;
+  uint32_t idx;
+};
+
+// Stable LSD radix sort of (key, idx) by key, 11-bit digits, OpenMP.
+void radix_sort(std::vector<KeyIdx>& a, std::vector<KeyIdx>& tmp, uint64_t key_or) {
+  const int64_t n = (int64_t)a.size();
+  constexpr int BITS = 11, R = 1 << BITS;
+  int nthreads = 1;
+#ifdef _OPENMP
+  nthreads = omp_get_max_threads();
+#endif
+  if (n < (1 << 16)) nthreads = 1;
+  std::vector<int64_t> hist((size_t)nthreads * R);
+  KeyIdx* src = a.data();
+  KeyIdx* dst = tmp.data();
+  for (int shift = 0; shift < 63; shift += BITS) {
+    if (((key_or >> shift) & (R - 1)) == 0) continue;  // digit is zero in every key
+    std::fill(hist.begin(), hist.end(), 0);
+#pragma omp parallel num_threads(nthreads)
+    {
+#ifdef _OPENMP
+      const int t = omp_get_thread_num();
+#else
+      const int t = 0;
+#endif
+      const int64_t lo = n * t / nthreads, hi = n * (t + 1) / nthreads;
+      int64_t* h = &hist[(size_t)t * R];
+      for (int64_t i = lo; i < hi; i++) h[(src[i].key >> shift) & (R - 1)]++;
+#pragma omp barrier
+#pragma omp single
+      {
+        int64_t run = 0;
+        for (int d = 0; d < R; d++)
+          for (int tt = 0; tt < nthreads; tt++) {
+            const int64_t c = hist[(size_t)tt * R + d];
+            hist[(size_t)tt * R + d] = run;
+            run += c;
+          }
+      }
+      for (int64_t i = lo; i < hi; i++) dst[h[(src[i].key >> shift) & (R - 1)]++] = src[i];
+    }
+    std::swap(src, dst);
+  }
+  if (src != a.data()) std::memcpy(a.data(), src, sizeof(KeyIdx) * (size_t)n);
+}
+
+struct CellProp {   // fp64 moments, fp32-exact bounding box
+  float bmin[3], bmax[3];
+  double M, X[3], Q[6];  // Q: xx,yy,zz,xy,xz,yz about X
+};
+
+inline size_t align256(size_t x) { return (x + 255) & ~(size_t)255; }
+
+}  // namespace
+
+int build_host_tree(const float* pos, const float* mass, int64_t n, int n_leaf, int n_group,
+                    HostTree& T, PackedAlloc alloc, void* alloc_user, std::string& msg) {
+  if (n < 1 || n_leaf < 1 || n_group < 1) { msg = "build: n, n_leaf, n_group must be >= 1"; return TC_EINVAL; }
+  T.n = n; T.n_leaf = n_leaf; T.n_group = n_group;
+
+  // ---- O1: root cube and integer grid ("a cube containing all particles")
+  double lo[3], hi[3];
+  for (int k = 0; k < 3; k++) { lo[k] = std::numeric_limits<double>::infinity(); hi[k] = -lo[k]; }
+  for (int64_t i = 0; i < n; i++)
+    for (int k = 0; k < 3; k++) {
+      const double v = (double)pos[3 * i + k];
+      lo[k] = std::min(lo[k], v); hi[k] = std::max(hi[k], v);
+    }
+  double ext = 0.0;
+  for (int k = 0; k < 3; k++) ext = std::max(ext, hi[k] - lo[k]);
+  double side = ext * (1.0 + std::ldexp(1.0, -20));
+  if (side == 0.0) side = 1.0;
+  double org[3];
+  for (int k = 0; k < 3; k++) org[k] = (lo[k] + hi[k]) / 2.0 - side / 2.0;
+  const double scale = std::ldexp(1.0, 21) / side;
+  const double gmax = std::ldexp(1.0, 21) - 1.0;
+
+  std::vector<KeyIdx> keys, tmp;
+  try { keys.resize((size_t)n); tmp.resize((size_t)n); } catch (...) { msg = "build: out of host memory"; return TC_ENOMEM; }
+  uint64_t key_or = 0;
+#pragma omp parallel for schedule(static) reduction(| : key_or)
+  for (int64_t i = 0; i < n; i++) {
+    uint64_t g[3];
+    for (int k = 0; k < 3; k++) {
+      double v = std::floor(((double)pos[3 * i + k] - org[k]) * scale);
+      v = std::min(std::max(v, 0.0), gmax);
+      g[k] = (uint64_t)v;
+    }
+    // octant o = 4 bx + 2 by + bz at every level  ->  x is the most significant of each triple
+    const uint64_t key = (spread21(g[0]) << 2) | (spread21(g[1]) << 1) | spread21(g[2]);
+    keys[i].key = key; keys[i].idx = (uint32_t)i;
+    key_or |= key;
+  }
+  radix_sort(keys, tmp, key_or);
+  tmp.clear(); tmp.shrink_to_fit();
+
+  // ---- O2: breadth-first split of sorted key ranges
+  // cell arrays (struct of vectors), breadth-first, children contiguous
+  std::vector<int32_t> c_begin, c_count, c_first_child, c_nchild;
+  std::vector<int64_t> level_start;  // first cell id of every level (+ end sentinel)
+  c_begin.push_back(0); c_count.push_back((int32_t)n); c_first_child.push_back(-1); c_nchild.push_back(0);
+  level_start.push_back(0);
+  int64_t lvl_b = 0, lvl_e = 1;
+  int level = 0;
+  std::vector<int32_t> nch;
+  while (true) {
+    level_start.push_back(lvl_e);
+    if (level == kMaxLevel) break;
+    const int shift = 3 * (kMaxLevel - 1 - level);
+    const int64_t nl = lvl_e - lvl_b;
+    nch.assign((size_t)nl + 1, 0);
+    // pass 1: number of non-empty octants of every node of this level
+#pragma omp parallel for schedule(dynamic, 256)
+    for (int64_t c = lvl_b; c < lvl_e; c++) {
+      if (c_count[c] <= n_leaf) continue;  // leaf (R4: <=)
+      const KeyIdx* kb = keys.data() + c_begin[c];
+      const KeyIdx* ke = kb + c_count[c];
+      int cnt = 0;
+      const KeyIdx* p = kb;
+      while (p < ke) {
+        const uint64_t o = (p->key >> shift) & 7;
+        // first key of this cell with octant > o
+        p = std::partition_point(p, ke, [&](const KeyIdx& q) { return ((q.key >> shift) & 7) <= o; });
+        cnt++;
+      }
+      nch[(size_t)(c - lvl_b)] = cnt;
+    }
+    int64_t total = 0;
+    for (int64_t i = 0; i < nl; i++) { const int32_t v = nch[i]; nch[i] = (int32_t)total; total += v; }
+    nch[nl] = (int32_t)total;
+    if (total == 0) break;
+    if (lvl_e + total > (int64_t)0x0fffffff) { msg = "build: more than 2^28 cells"; return TC_EINVAL; }
+    const int64_t new_e = lvl_e + total;
+    c_begin.resize((size_t)new_e); c_count.resize((size_t)new_e);
+    c_first_child.resize((size_t)new_e, -1); c_nchild.resize((size_t)new_e, 0);
+    // pass 2: create the children
+#pragma omp parallel for schedule(dynamic, 256)
+    for (int64_t c = lvl_b; c < lvl_e; c++) {
+      const int32_t k = nch[(size_t)(c - lvl_b) + 1] - nch[(size_t)(c - lvl_b)];
+      if (k == 0) continue;
+      const int64_t first = lvl_e + nch[(size_t)(c - lvl_b)];
+      c_first_child[c] = (int32_t)first; c_nchild[c] = k;
+      const KeyIdx* k0 = keys.data();
+      const KeyIdx* kb = k0 + c_begin[c];
+      const KeyIdx* ke = kb + c_count[c];
+      const KeyIdx* p = kb;
+      int j = 0;
+      while (p < ke) {
+        const uint64_t o = (p->key >> shift) & 7;
+        const KeyIdx* q = std::partition_point(p, ke, [&](const KeyIdx& r) { return ((r.key >> shift) & 7) <= o; });
+        c_begin[first + j] = (int32_t)(p - k0); c_count[first + j] = (int32_t)(q - p);
+        j++; p = q;
+      }
+    }
+    lvl_b = lvl_e; lvl_e = new_e; level++;
+  }
+  const int64_t nc = (int64_t)c_begin.size();
+  T.n_cells = nc;
+  T.depth = (int32_t)level_start.size() - 2;
+  const int n_levels = (int)level_start.size() - 1;
+
+  // ---- O3: cell properties, fp64, bottom-up.  Leaves: direct sums
+  // over members.  Nodes: union of the children's boxes, parallel-axis shift of the
+  // children's moments to the node's centre of mass.
+  std::vector<CellProp> prop;
+  try { prop.resize((size_t)nc); } catch (...) { msg = "build: out of host memory"; return TC_ENOMEM; }
+  int64_t n_leaves = 0;
+  for (int L = n_levels - 1; L >= 0; L--) {
+    const int64_t b = level_start[L], e = level_start[L + 1];
+#pragma omp parallel for schedule(dynamic, 128) reduction(+ : n_leaves)
+    for (int64_t c = b; c < e; c++) {
+      CellProp& P = prop[c];
+      double M = 0.0, S[3] = {0, 0, 0};
+      if (c_nchild[c] == 0) {
+        n_leaves++;
+        float mn[3] = {INFINITY, INFINITY, INFINITY}, mx[3] = {-INFINITY, -INFINITY, -INFINITY};
+        const int64_t pb = c_begin[c], pe = pb + c_count[c];
+        for (int64_t t = pb; t < pe; t++) {
+          const int64_t i = keys[t].idx;
+          const double m = (double)mass[i];
+          for (int k = 0; k < 3; k++) {
+            const float v = pos[3 * i + k];
+            mn[k] = std::min(mn[k], v); mx[k] = std::max(mx[k], v);
+            S[k] += m * (double)v;
+          }
+          M += m;
+        }
+        for (int k = 0; k < 3; k++) { P.bmin[k] = mn[k]; P.bmax[k] = mx[k]; }
+        P.M = M;
+        for (int k = 0; k < 3; k++)  // massless cell (R19): centre of the boundary cube
+          P.X[k] = (M > 0.0) ? S[k] / M : ((double)mn[k] + (double)mx[k]) / 2.0;
+        double Q[6] = {0, 0, 0, 0, 0, 0};
+        for (int64_t t = pb; t < pe; t++) {
+          const int64_t i = keys[t].idx;
+          const double m = (double)mass[i];
+          const double yx = (double)pos[3 * i] - P.X[0], yy = (double)pos[3 * i + 1] - P.X[1],
+                       yz = (double)pos[3 * i + 2] - P.X[2];
+          const double y2 = yx * yx + yy * yy + yz * yz;
+          Q[0] += m * (3.0 * yx * yx - y2); Q[1] += m * (3.0 * yy * yy - y2); Q[2] += m * (3.0 * yz * yz - y2);
+          Q[3] += m * (3.0 * yx * yy); Q[4] += m * (3.0 * yx * yz); Q[5] += m * (3.0 * yy * yz);
+        }
+        for (int k = 0; k < 6; k++) P.Q[k] = Q[k];
+      } else {
+        const int64_t f = c_first_child[c], l = f + c_nchild[c];
+        for (int k = 0; k < 3; k++) { P.bmin[k] = INFINITY; P.bmax[k] = -INFINITY; }
+        for (int64_t ch = f; ch < l; ch++) {
+          const CellProp& C = prop[ch];
+          for (int k = 0; k < 3; k++) {
+            P.bmin[k] = std::min(P.bmin[k], C.bmin[k]); P.bmax[k] = std::max(P.bmax[k], C.bmax[k]);
+            S[k] += C.M * C.X[k];
+          }
+          M += C.M;
+        }
+        P.M = M;
+        for (int k = 0; k < 3; k++)
+          P.X[k] = (M > 0.0) ? S[k] / M : ((double)P.bmin[k] + (double)P.bmax[k]) / 2.0;
+        double Q[6] = {0, 0, 0, 0, 0, 0};
+        for (int64_t ch = f; ch < l; ch++) {
+          const CellProp& C = prop[ch];
+          const double dx = C.X[0] - P.X[0], dy = C.X[1] - P.X[1], dz = C.X[2] - P.X[2];
+          const double d2 = dx * dx + dy * dy + dz * dz;
+          Q[0] += C.Q[0] + C.M * (3.0 * dx * dx - d2); Q[1] += C.Q[1] + C.M * (3.0 * dy * dy - d2);
+          Q[2] += C.Q[2] + C.M * (3.0 * dz * dz - d2);
+          Q[3] += C.Q[3] + C.M * (3.0 * dx * dy); Q[4] += C.Q[4] + C.M * (3.0 * dx * dz);
+          Q[5] += C.Q[5] + C.M * (3.0 * dy * dz);
+        }
+        for (int k = 0; k < 6; k++) P.Q[k] = Q[k];
+      }
+    }
+  }
+  T.n_leaves = n_leaves;
+
+  // ---- O4: groups = maximal cells with count <= N_group, or leaves, Morton order
+  std::vector<int32_t> groups;
+  {
+    std::vector<int32_t> st;
+    st.push_back(0);
+    while (!st.empty()) {
+      const int32_t c = st.back(); st.pop_back();
+      if (c_count[c] <= n_group || c_nchild[c] == 0) { groups.push_back(c); continue; }
+      for (int j = c_nchild[c] - 1; j >= 0; j--) st.push_back(c_first_child[c] + j);
+    }
+  }
+  T.n_groups = (int64_t)groups.size();
+
+  // ---- pack: SoA float4 arrays in one buffer (layout in tc_internal.h)
+  PackedLayout& Y = T.lay;
+  size_t off = 0;
+  Y.off_bnd = off;  off = align256(off + sizeof(float4) * (size_t)nc);
+  Y.off_xm = off;   off = align256(off + sizeof(float4) * (size_t)nc);
+  Y.off_q0 = off;   off = align256(off + sizeof(float4) * (size_t)nc);
+  Y.off_q1 = off;   off = align256(off + sizeof(float4) * (size_t)nc);
+  Y.off_part = off; off = align256(off + sizeof(float4) * (size_t)n);
+  Y.off_orig = off; off = align256(off + sizeof(int32_t) * (size_t)n);
+  Y.off_grp = off;  off = align256(off + sizeof(int4) * groups.size());
+  Y.bytes = off;
+  char* base = (char*)alloc(alloc_user, Y.bytes);
+  if (!base) { msg = "build: cannot allocate the packed tree buffer"; return TC_ENOMEM; }
+  float4* bnd = (float4*)(base + Y.off_bnd);
+  float4* xm = (float4*)(base + Y.off_xm);
+  float4* q0 = (float4*)(base + Y.off_q0);
+  float4* q1 = (float4*)(base + Y.off_q1);
+  float4* part = (float4*)(base + Y.off_part);
+  int32_t* orig = (int32_t*)(base + Y.off_orig);
+  int4* grp = (int4*)(base + Y.off_grp);
+  try { T.link.resize((size_t)nc * 4); T.q6.resize((size_t)nc * 6); } catch (...) { msg = "build: out of host memory"; return TC_ENOMEM; }
+
+#pragma omp parallel for schedule(static)
+  for (int64_t c = 0; c < nc; c++) {
+    const CellProp& P = prop[c];
+    // boundary cube (Fig. 1): same centre as the tight box, side = its largest side
+    double e = 0.0;
+    float b[3];
+    for (int k = 0; k < 3; k++) {
+      b[k] = (float)(((double)P.bmin[k] + (double)P.bmax[k]) / 2.0);
+      e = std::max(e, (double)P.bmax[k] - (double)P.bmin[k]);
+    }
+    const float h = (float)(e / 2.0);
+    const bool leaf = c_nchild[c] == 0;
+    bnd[c] = make_float4(b[0], b[1], b[2], leaf ? -h : h);  // sign bit of h <=> leaf (-0.0f if h == 0)
+    xm[c] = make_float4((float)P.X[0], (float)P.X[1], (float)P.X[2], (float)P.M);
+    q0[c] = make_float4((float)P.Q[0], (float)P.Q[1], (float)P.Q[2], (float)P.Q[3]);
+    int32_t la, lb;
+    if (leaf) { la = c_begin[c]; lb = c_count[c]; } else { la = c_first_child[c]; lb = c_nchild[c]; }
+    float fa, fb;
+    std::memcpy(&fa, &la, 4); std::memcpy(&fb, &lb, 4);
+    q1[c] = make_float4((float)P.Q[4], (float)P.Q[5], fa, fb);
+    T.link[4 * c + 0] = leaf ? -1 : c_first_child[c];
+    T.link[4 * c + 1] = c_nchild[c];
+    T.link[4 * c + 2] = c_begin[c];
+    T.link[4 * c + 3] = c_count[c];
+    for (int k = 0; k < 6; k++) T.q6[6 * c + k] = (float)P.Q[k];
+  }
+#pragma omp parallel for schedule(static)
+  for (int64_t t = 0; t < n; t++) {
+    const int64_t i = keys[t].idx;
+    part[t] = make_float4(pos[3 * i], pos[3 * i + 1], pos[3 * i + 2], mass[i]);
+    orig[t] = (int32_t)i;
+  }
+  for (size_t g = 0; g < groups.size(); g++) {
+    const int32_t c = groups[g];
+    grp[g] = make_int4(c, c_begin[c], c_count[c], 0);
+  }
+  return TC_OK;
+}
+
+}  // namespace tc

@@ -1,0 +1,95 @@
+// Internal declarations shared by the host builder (tc_build.cpp), the kernels
+// (tc_kernels.cu) and the C ABI (tc_api.cpp).  Not installed; include/tc.h is the
+// public boundary.  Shares nothing with oracle/.
+#pragma once
+#include <cstdint>
+#include <string>
+#include <vector>
+
+#include <vector_functions.h>  // float4 / int4 / make_float4 (CUDA toolkit header, host-safe)
+
+#include "../../include/tc.h"
+
+namespace tc {
+
+constexpr int kMaxLevel = 21;  // 3 x 21 = 63-bit Morton keys (R7)
+
+// Packed tree in ONE host buffer (pinned when a device exists) that tc_build moves
+// with one cudaMemcpyAsync.  All section offsets are multiples
+// of 256 bytes.  Per cell c (cells in breadth-first order, children contiguous):
+//   bnd [c] = (bx, by, bz, h)        boundary cube, Fig. 1; sign bit of h set <=> leaf
+//   xm  [c] = (X, Y, Z, M)           centre of mass, mass
+//   q0  [c] = (Qxx, Qyy, Qzz, Qxy)   traceless quadrupole about X
+//   q1  [c] = (Qxz, Qyz, a, b)       a,b int bits: node -> (first_child, n_child)
+//                                                 leaf -> (first_body,  n_body)
+//   part[i] = (x, y, z, m)           particles in tree (Morton) order
+//   orig[i] = caller's index of tree-order particle i
+//   grp [g] = (cell, first_body, n_body, 0)  groups in Morton order
+struct PackedLayout {
+  size_t off_bnd = 0, off_xm = 0, off_q0 = 0, off_q1 = 0, off_part = 0, off_orig = 0, off_grp = 0;
+  size_t bytes = 0;
+};
+
+struct HostTree {
+  int64_t n = 0;
+  int32_t n_leaf = 0, n_group = 0;
+  int64_t n_cells = 0, n_leaves = 0, n_groups = 0;
+  int32_t depth = 0;
+  // link per cell (host inspection, tc_get_tree): first_child, n_child, first_body, n_body
+  std::vector<int32_t> link;
+  std::vector<float> q6;  // unpacked quadrupole for tc_get_tree [n_cells,6]
+  PackedLayout lay;
+  void* packed = nullptr;  // lay.bytes, owned by the ctx (pinned or malloc)
+  size_t packed_cap = 0;
+  bool packed_pinned = false;
+};
+
+// Host builder (tc_build.cpp).  pos [n,3], mass [n] host fp32.  Allocates/reuses
+// T.packed through alloc(bytes) (returns nullptr on failure).  Returns TC_OK or an
+// error code with msg set.
+typedef void* (*PackedAlloc)(void* user, size_t bytes);
+int build_host_tree(const float* pos, const float* mass, int64_t n, int n_leaf, int n_group,
+                    HostTree& T, PackedAlloc alloc, void* alloc_user, std::string& msg);
+
+// Device-side view handed to the kernels (tc_kernels.cu).
+struct DeviceTree {
+  const float4* bnd = nullptr;
+  const float4* xm = nullptr;
+  const float4* q0 = nullptr;
+  const float4* q1 = nullptr;
+  const float4* part = nullptr;
+  const int32_t* orig = nullptr;
+  const int4* grp = nullptr;
+  int64_t n = 0, n_cells = 0, n_groups = 0;
+};
+
+// Device counters written by the force kernel (one struct, zeroed before launch).
+struct DeviceCounters {
+  unsigned long long n_pc_total;
+  unsigned long long n_pp_total;
+  unsigned long long n_tests_total;
+  unsigned long long n_spills;
+  unsigned int next_group;  // dynamic work counter (persistent warps)
+  unsigned int overflow;    // != 0: a spill stack overflowed -> TC_EOVERFLOW
+};
+
+struct ForceLaunch {
+  float theta = 0.f, eps = 0.f;
+  float* acc = nullptr;       // device [n,3] caller order
+  float* pot = nullptr;       // device [n] caller order or nullptr
+  int32_t* n_pc = nullptr;    // device [n] caller order
+  int32_t* n_pp = nullptr;    // device [n] caller order
+  DeviceCounters* counters = nullptr;
+  uint32_t* spill = nullptr;  // device [n_warps_total * spill_cap]
+  int spill_cap = 0;
+  int stack_smem = 1024;
+  int n_sm = 148;
+};
+
+// Launches the fused walk+evaluate kernel on `stream` (a cudaStream_t).  Returns a
+// cudaError_t as int (0 = success).  Defined in tc_kernels.cu.
+int launch_forces(const DeviceTree& T, const ForceLaunch& L, void* stream);
+// Number of warps the persistent grid runs (for sizing the spill buffer).
+int forces_total_warps(int n_sm, int stack_smem);
+
+}  // namespace tc

@@ -1,0 +1,375 @@
+// Fused tree walk + interaction-list evaluation for sm_100a (steps A1-A6 of
+// DESIGN.md; Sec. 2.2-2.3 of arXiv 1005.5384).
+//
+// The paper walks every group twice with one THREAD per group (count, host scan,
+// write), stores the lists in global memory and evaluates them
+// with two more kernels (Lists 3-4).  Here one WARP owns a group from start to end:
+//   * the walk is lane-parallel: 4 nodes are popped from a shared-memory stack per
+//     iteration and their <= 8 contiguous children are tested by 32 lanes at once
+//     (`test_cell`/`open_node`, List 2 PAPER.md:73-91), 4 coalesced float4 loads per
+//     lane (boundary + multipole, issued together so an iteration costs one memory
+//     latency);
+//   * ballot/popc compaction sorts the children into: stack (opened nodes), a queue
+//     of opened leaves, and a shared-memory chunk of un-opened cells' multipoles;
+//   * a chunk is evaluated as soon as it fills (FP32 FMA + one rsqrt.approx per
+//     interaction), so no interaction list ever reaches global memory and there is
+//     no count pass, no host scan, no second walk;
+//   * lanes map to (particle, list slice): a group of P <= 32 particles uses
+//     floor(32/P) slices of the chunk at once and reduces them with shuffles at the
+//     end — the fix for the paper's 30 % thread utilisation.
+// No tensor cores: this is not a dense contraction.
+#include <cuda_runtime.h>
+
+#include <cstdint>
+
+#include "tc_internal.h"
+
+namespace tc {
+namespace {
+
+constexpr int kWarpsPerCta = 8;
+constexpr int kCellCap = 96;    // un-opened cells staged per warp before evaluation
+constexpr int kLeafQCap = 64;   // opened-leaf ranges queued per warp
+constexpr int kBodyCap = 128;   // bodies staged per warp per evaluation round
+constexpr unsigned kFull = 0xffffffffu;
+
+template <int STK>
+struct __align__(16) WarpSmem {
+  float4 cxm[kCellCap];    // (X, Y, Z, M)
+  float4 cq0[kCellCap];    // (Qxx, Qyy, Qzz, Qxy)
+  float4 body[kBodyCap];   // (x, y, z, m)
+  float2 cq1[kCellCap];    // (Qxz, Qyz)
+  int2 leafq[kLeafQCap];   // (first_body, n_body)
+  int bidx[kBodyCap];      // flattened body indices of the current round
+  uint32_t stack[STK];     // nodes to expand: first_child << 3 | (n_child - 1)
+};
+
+__device__ __forceinline__ float rsqrt_approx(float x) {
+  float y;
+  asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+  return y;
+}
+
+struct Acc {
+  float ax, ay, az, pot;
+};
+
+// particle-cell: monopole + traceless quadrupole (O6), d = X - x_i:
+//   a   += M d/s^3 - Q d/s^5 + (5/2)(d^T Q d) d/s^7
+//   phi += -M/s - (1/2)(d^T Q d)/s^5
+// 33 FP32 instructions + 1 MUFU.
+__device__ __forceinline__ void pc_interact(float xi, float yi, float zi, float eps2, const float4 xm,
+                                            const float4 q0, const float2 q1, Acc& a) {
+  const float dx = xm.x - xi, dy = xm.y - yi, dz = xm.z - zi;
+  const float s2 = fmaf(dz, dz, fmaf(dy, dy, fmaf(dx, dx, eps2)));
+  const float rinv = rsqrt_approx(s2);
+  const float rinv2 = rinv * rinv;
+  const float rinv3 = rinv * rinv2;
+  const float rinv5 = rinv3 * rinv2;
+  const float qdx = fmaf(q1.x, dz, fmaf(q0.w, dy, q0.x * dx));
+  const float qdy = fmaf(q1.y, dz, fmaf(q0.y, dy, q0.w * dx));
+  const float qdz = fmaf(q0.z, dz, fmaf(q1.y, dy, q1.x * dx));
+  const float dqd = fmaf(dz, qdz, fmaf(dy, qdy, dx * qdx));
+  const float t5 = dqd * rinv5;
+  a.pot = fmaf(-xm.w, rinv, a.pot);
+  a.pot = fmaf(-0.5f, t5, a.pot);
+  const float c = fmaf(2.5f, t5 * rinv2, xm.w * rinv3);
+  a.ax = fmaf(c, dx, a.ax); a.ay = fmaf(c, dy, a.ay); a.az = fmaf(c, dz, a.az);
+  a.ax = fmaf(-rinv5, qdx, a.ax); a.ay = fmaf(-rinv5, qdy, a.ay); a.az = fmaf(-rinv5, qdz, a.az);
+}
+
+// particle-particle, Plummer softening (O6), d = x_j - x_i:
+//   a += m_j d/s^3, phi += -m_j/s.   13 FP32 instructions + 1 MUFU.
+// kEps0: eps == 0, coincident pairs (and the particle itself) contribute nothing.
+template <bool kEps0>
+__device__ __forceinline__ void pp_interact(float xi, float yi, float zi, float eps2, const float4 b, Acc& a) {
+  const float dx = b.x - xi, dy = b.y - yi, dz = b.z - zi;
+  const float s2 = fmaf(dz, dz, fmaf(dy, dy, fmaf(dx, dx, eps2)));
+  float rinv = rsqrt_approx(s2);
+  if (kEps0) rinv = (s2 > 0.f) ? rinv : 0.f;
+  const float rinv2 = rinv * rinv;
+  const float mr = b.w * rinv;
+  const float mr3 = mr * rinv2;
+  a.pot -= mr;
+  a.ax = fmaf(mr3, dx, a.ax); a.ay = fmaf(mr3, dy, a.ay); a.az = fmaf(mr3, dz, a.az);
+}
+
+// Lane mapping of one batch of P <= 32 particles: lane = slice * P + particle.
+struct Batch {
+  int P;        // particles in the batch (0: batch unused) — warp-uniform
+  int S;        // slices = 32 / P                           — warp-uniform
+  int s;        // this lane's slice
+  bool active;  // lane < P * S
+  float x, y, z;
+  Acc a;
+};
+
+template <int STK>
+__device__ __forceinline__ void eval_cells(const WarpSmem<STK>& sm, int cnt, float eps2, Batch (&B)[2]) {
+#pragma unroll
+  for (int b = 0; b < 2; b++) {
+    if (B[b].P == 0) continue;   // warp-uniform
+    if (B[b].active) {
+      const int S = B[b].S;
+      Acc a = B[b].a;
+#pragma unroll 2
+      for (int e = B[b].s; e < cnt; e += S) pc_interact(B[b].x, B[b].y, B[b].z, eps2, sm.cxm[e], sm.cq0[e], sm.cq1[e], a);
+      B[b].a = a;
+    }
+  }
+}
+
+template <int STK, bool kEps0>
+__device__ __forceinline__ void eval_bodies(const WarpSmem<STK>& sm, int cnt, float eps2, Batch (&B)[2]) {
+#pragma unroll
+  for (int b = 0; b < 2; b++) {
+    if (B[b].P == 0) continue;
+    if (B[b].active) {
+      const int S = B[b].S;
+      Acc a = B[b].a;
+#pragma unroll 4
+      for (int e = B[b].s; e < cnt; e += S) pp_interact<kEps0>(B[b].x, B[b].y, B[b].z, eps2, sm.body[e], a);
+      B[b].a = a;
+    }
+  }
+}
+
+// Opened leaves (List 4): flatten the queued (first, n) ranges into
+// body indices, gather the bodies with one coalesced float4 load per lane, evaluate.
+template <int STK, bool kEps0>
+__device__ __forceinline__ void eval_leaves(WarpSmem<STK>& sm, int nq, const float4* __restrict__ part,
+                                            float eps2, Batch (&B)[2], int lane) {
+  for (int r0 = 0; r0 < nq; r0 += 32) {
+    int f = 0, n = 0;
+    if (r0 + lane < nq) { const int2 r = sm.leafq[r0 + lane]; f = r.x; n = r.y; }
+    int incl = n;   // inclusive scan of n
+#pragma unroll
+    for (int d = 1; d < 32; d <<= 1) { const int t = __shfl_up_sync(kFull, incl, d); if (lane >= d) incl += t; }
+    const int off = incl - n;
+    const int total = __shfl_sync(kFull, incl, 31);
+    for (int base = 0; base < total; base += kBodyCap) {
+      const int k0 = max(0, base - off), k1 = min(n, base + kBodyCap - off);
+      for (int k = k0; k < k1; k++) sm.bidx[off + k - base] = f + k;
+      __syncwarp();
+      const int cnt = min(kBodyCap, total - base);
+      for (int t = lane; t < cnt; t += 32) sm.body[t] = __ldg(part + sm.bidx[t]);
+      __syncwarp();
+      eval_bodies<STK, kEps0>(sm, cnt, eps2, B);
+      __syncwarp();
+    }
+  }
+}
+
+template <int STK, bool kEps0>
+__global__ void __launch_bounds__(kWarpsPerCta * 32)
+forces_kernel(const float4* __restrict__ bnd, const float4* __restrict__ xm, const float4* __restrict__ q0,
+              const float4* __restrict__ q1, const float4* __restrict__ part, const int32_t* __restrict__ orig,
+              const int4* __restrict__ grp, int n_groups, float theta, float eps,
+              float* __restrict__ acc, float* __restrict__ pot, int32_t* __restrict__ out_npc,
+              int32_t* __restrict__ out_npp, DeviceCounters* __restrict__ ctr, uint32_t* __restrict__ spill_all,
+              int spill_cap) {
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  WarpSmem<STK>& sm = reinterpret_cast<WarpSmem<STK>*>(smem_raw)[warp];
+  uint32_t* spill = spill_all + (size_t)(blockIdx.x * kWarpsPerCta + warp) * (size_t)spill_cap;
+  const float eps2 = eps * eps;
+  const float th2 = __fmul_rn(theta, theta);
+  const unsigned lt_mask = (1u << lane) - 1u;
+
+  // root: a leaf root is never tested (O5) — its bodies are the whole leaf list
+  const float4 root_b = __ldg(bnd);
+  const float4 root_l = __ldg(q1);
+  const bool root_leaf = __float_as_int(root_b.w) < 0;
+  const int root_a = __float_as_int(root_l.z), root_n = __float_as_int(root_l.w);
+
+  while (true) {
+    int g = 0;
+    if (lane == 0) g = (int)atomicAdd(&ctr->next_group, 1u);
+    g = __shfl_sync(kFull, g, 0);
+    if (g >= n_groups) break;
+    const int4 G = __ldg(grp + g);           // (cell, first_body, n_body, 0)
+    const float4 gb = __ldg(bnd + G.x);
+    const float gbx = gb.x, gby = gb.y, gbz = gb.z, gh = fabsf(gb.w);
+
+    // groups larger than 64 particles (level-21 leaves, or N_group > 64) repeat the walk per 64
+    for (int pb = 0; pb < G.z; pb += 64) {
+      const int m = min(64, G.z - pb);
+      Batch B[2];
+#pragma unroll
+      for (int b = 0; b < 2; b++) {
+        const int P = max(0, min(32, m - 32 * b));
+        B[b].P = P;
+        B[b].S = P ? 32 / P : 1;
+        const int p = P ? lane % P : 0;
+        B[b].s = P ? lane / P : 0;
+        B[b].active = P && lane < P * B[b].S;
+        B[b].a = Acc{0.f, 0.f, 0.f, 0.f};
+        B[b].x = B[b].y = B[b].z = 0.f;
+        if (B[b].active) {
+          const float4 me = __ldg(part + G.y + pb + 32 * b + p);
+          B[b].x = me.x; B[b].y = me.y; B[b].z = me.z;
+        }
+      }
+
+      int ssz = 0, spill_sz = 0, ccnt = 0, lq = 0;
+      long long n_pc = 0, n_pp = 0, n_tests = 0;
+      int n_spills = 0;
+      bool overflow = false;
+      if (root_leaf) {
+        if (lane == 0) sm.leafq[0] = make_int2(root_a, root_n);
+        lq = 1; n_pp = root_n;
+      } else {
+        if (lane == 0) sm.stack[0] = ((uint32_t)root_a << 3) | (uint32_t)(root_n - 1);
+        ssz = 1;
+      }
+      __syncwarp();
+
+      // ---- the walk (List 1-2): pop up to 4 nodes, test their children
+      while (true) {
+        if (ssz == 0) {
+          if (spill_sz == 0) break;
+          const int take = min(spill_sz, STK / 2);      // reload the top of the spill stack
+          for (int t = lane; t < take; t += 32) sm.stack[t] = spill[spill_sz - take + t];
+          spill_sz -= take; ssz = take;
+          __syncwarp();
+        }
+        const int npop = min(ssz, 4);
+        const int slot = lane >> 3, k = lane & 7;
+        const uint32_t packed = (slot < npop) ? sm.stack[ssz - 1 - slot] : 0u;
+        ssz -= npop;
+        const bool valid = (slot < npop) && (k <= (int)(packed & 7u));
+        const int c = (int)(packed >> 3) + k;
+        float4 cb = make_float4(0.f, 0.f, 0.f, 0.f), cx = cb, c0 = cb, c1 = cb;
+        if (valid) { cb = __ldg(bnd + c); cx = __ldg(xm + c); c0 = __ldg(q0 + c); c1 = __ldg(q1 + c); }
+        // open_node (O5/R16): one fixed sequence of correctly rounded fp32 operations
+        const float hc = fabsf(cb.w);
+        const float s = __fadd_rn(hc, gh);
+        const float tx = fmaxf(__fsub_rn(fabsf(__fsub_rn(cb.x, gbx)), s), 0.f);
+        const float ty = fmaxf(__fsub_rn(fabsf(__fsub_rn(cb.y, gby)), s), 0.f);
+        const float tz = fmaxf(__fsub_rn(fabsf(__fsub_rn(cb.z, gbz)), s), 0.f);
+        const float d2 = __fmaf_rn(tz, tz, __fmaf_rn(ty, ty, __fmul_rn(tx, tx)));
+        const float l = __fadd_rn(hc, hc);
+        const bool open = valid && (__fmul_rn(d2, th2) <= __fmul_rn(l, l));
+        const bool leaf = __float_as_int(cb.w) < 0;
+        const bool to_cell = valid && !open, to_leaf = open && leaf, to_stack = open && !leaf;
+        const int la = __float_as_int(c1.z), lb = __float_as_int(c1.w);
+
+        const unsigned m_cell = __ballot_sync(kFull, to_cell);
+        const unsigned m_leaf = __ballot_sync(kFull, to_leaf);
+        const unsigned m_stack = __ballot_sync(kFull, to_stack);
+        n_tests += __popc(__ballot_sync(kFull, valid));
+        if (to_cell) {                                   // not opened (leaf or node): multipole (R2)
+          const int p = ccnt + __popc(m_cell & lt_mask);
+          sm.cxm[p] = cx; sm.cq0[p] = c0; sm.cq1[p] = make_float2(c1.x, c1.y);
+        }
+        ccnt += __popc(m_cell); n_pc += __popc(m_cell);
+        if (m_leaf) {                                    // opened leaf: particle-particle
+          if (to_leaf) sm.leafq[lq + __popc(m_leaf & lt_mask)] = make_int2(la, lb);
+          lq += __popc(m_leaf);
+          n_pp += __reduce_add_sync(kFull, to_leaf ? lb : 0);
+        }
+        if (m_stack) {                                   // opened node: walk on
+          const int npush = __popc(m_stack);
+          __syncwarp();                                  // all pops were read before slots are reused
+          if (ssz + npush > STK) {                       // spill the bottom half to global memory
+            const int mv = STK / 2;
+            if (spill_sz + mv > spill_cap) { overflow = true; }
+            else {
+              for (int t = lane; t < mv; t += 32) spill[spill_sz + t] = sm.stack[t];
+              __syncwarp();
+              for (int t0 = mv; t0 < ssz; t0 += 32) {    // shift the rest down (ascending, chunked)
+                const int t = t0 + lane;
+                const uint32_t v = (t < ssz) ? sm.stack[t] : 0u;
+                __syncwarp();
+                if (t < ssz) sm.stack[t - mv] = v;
+                __syncwarp();
+              }
+              spill_sz += mv; ssz -= mv; n_spills++;
+            }
+          }
+          if (overflow) break;
+          if (to_stack) sm.stack[ssz + __popc(m_stack & lt_mask)] = ((uint32_t)la << 3) | (uint32_t)(lb - 1);
+          ssz += npush;
+        }
+        __syncwarp();
+        if (ccnt > kCellCap - 32) { eval_cells<STK>(sm, ccnt, eps2, B); ccnt = 0; __syncwarp(); }
+        if (lq > kLeafQCap - 32) { eval_leaves<STK, kEps0>(sm, lq, part, eps2, B, lane); lq = 0; }
+      }
+      if (ccnt) eval_cells<STK>(sm, ccnt, eps2, B);
+      __syncwarp();
+      if (lq) eval_leaves<STK, kEps0>(sm, lq, part, eps2, B, lane);
+      __syncwarp();
+
+      // ---- A6: reduce the slices of every particle, write back in the caller's order
+#pragma unroll
+      for (int b = 0; b < 2; b++) {
+        if (B[b].P == 0) continue;
+        const int P = B[b].P, S = B[b].S, s = B[b].s;
+        Acc a = B[b].a;
+        for (int w = 1; w < S; w <<= 1) {
+          const float ox = __shfl_down_sync(kFull, a.ax, w * P), oy = __shfl_down_sync(kFull, a.ay, w * P);
+          const float oz = __shfl_down_sync(kFull, a.az, w * P), op = __shfl_down_sync(kFull, a.pot, w * P);
+          if (B[b].active && (s % (2 * w)) == 0 && s + w < S) { a.ax += ox; a.ay += oy; a.az += oz; a.pot += op; }
+        }
+        if (lane < P) {
+          const int t = G.y + pb + 32 * b + lane;
+          const int i = __ldg(orig + t);
+          if (!kEps0) a.pot += __ldg(part + t).w * rsqrt_approx(eps2);  // the particle met itself once
+          acc[3 * (size_t)i + 0] = a.ax; acc[3 * (size_t)i + 1] = a.ay; acc[3 * (size_t)i + 2] = a.az;
+          if (pot) pot[i] = a.pot;
+          out_npc[i] = (int32_t)n_pc; out_npp[i] = (int32_t)(n_pp - 1);
+        }
+      }
+      if (lane == 0) {
+        atomicAdd(&ctr->n_pc_total, (unsigned long long)(n_pc * m));
+        atomicAdd(&ctr->n_pp_total, (unsigned long long)((n_pp - 1) * m));
+        atomicAdd(&ctr->n_tests_total, (unsigned long long)n_tests);
+        if (n_spills) atomicAdd(&ctr->n_spills, (unsigned long long)n_spills);
+        if (overflow) atomicExch(&ctr->overflow, 1u);
+      }
+      __syncwarp();
+    }
+  }
+}
+
+template <int STK, bool kEps0>
+int launch_t(const DeviceTree& T, const ForceLaunch& L, cudaStream_t st, int* ctas_per_sm_out) {
+  auto kern = forces_kernel<STK, kEps0>;
+  const size_t smem = sizeof(WarpSmem<STK>) * kWarpsPerCta;
+  cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+  if (e != cudaSuccess) return (int)e;
+  int per_sm = 0;
+  e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, kWarpsPerCta * 32, smem);
+  if (e != cudaSuccess) return (int)e;
+  if (per_sm < 1) per_sm = 1;
+  if (ctas_per_sm_out) { *ctas_per_sm_out = per_sm; return 0; }
+  // persistent grid: every SM full, groups handed out by an atomic counter (Morton order)
+  const int grid = L.n_sm * per_sm;
+  kern<<<grid, kWarpsPerCta * 32, smem, st>>>(T.bnd, T.xm, T.q0, T.q1, T.part, T.orig, T.grp, (int)T.n_groups,
+                                               L.theta, L.eps, L.acc, L.pot, L.n_pc, L.n_pp, L.counters, L.spill,
+                                               L.spill_cap);
+  return (int)cudaGetLastError();
+}
+
+int dispatch(const DeviceTree& T, const ForceLaunch& L, cudaStream_t st, int* per_sm) {
+  const bool eps0 = (L.eps * L.eps == 0.f);
+  if (L.stack_smem == 64) return eps0 ? launch_t<64, true>(T, L, st, per_sm) : launch_t<64, false>(T, L, st, per_sm);
+  return eps0 ? launch_t<512, true>(T, L, st, per_sm) : launch_t<512, false>(T, L, st, per_sm);
+}
+
+}  // namespace
+
+int launch_forces(const DeviceTree& T, const ForceLaunch& L, void* stream) {
+  return dispatch(T, L, (cudaStream_t)stream, nullptr);
+}
+
+int forces_total_warps(int n_sm, int stack_smem) {
+  DeviceTree T;
+  ForceLaunch L;
+  L.stack_smem = stack_smem; L.eps = 1.f;
+  int per_sm = 0;
+  if (dispatch(T, L, nullptr, &per_sm) != 0 || per_sm < 1) per_sm = 8;
+  return n_sm * per_sm * kWarpsPerCta;
+}
+
+}  // namespace tc

@@ -1,0 +1,93 @@
+"""Host logic of the library (step A0: tc_build) against the oracle's own tree.
+
+The two builders share no code: the oracle partitions recursively top-down and
+sums moments directly over members (oracle/treecode_oracle.cpp), the library
+sorts Morton keys, splits breadth-first and shifts children's moments
+(csrc/tc_build.cpp).  Same readings O1-O4 => identical cell sets, bit-identical
+fp32 boundaries, moments equal to fp32 rounding.  Runs without a GPU
+(TC_FLAG_HOST_ONLY)."""
+import numpy as np
+import pytest
+
+from oracle import Oracle
+from paper_1005_5384_b200 import binding as B
+from paper_1005_5384_b200 import build as tc_build
+from paper_1005_5384_b200 import inputs
+
+
+@pytest.fixture(scope="module", autouse=True)
+def _built():
+    tc_build.build()
+
+
+def _compare(pos, mass, n_leaf, n_group):
+    with B.TreeCode(host_only=True, n_group=n_group) as tc:
+        tc.set_particles(pos, mass)
+        tc.build(n_leaf)
+        s, tr = tc.stats(), tc.tree()
+    o = Oracle(pos, mass, n_leaf, n_group)
+    assert (s["n_cells"], s["n_leaves"], s["n_groups"], s["depth"]) == (o.n_cells, o.n_leaves, o.n_groups, o.depth)
+    n = len(mass)
+    assert np.array_equal(np.sort(tr["perm"]), np.arange(n))
+    oc = o.cells()
+    # match cells by (level, first member, count): a single-child chain shares (begin, count)
+    lvl = np.zeros(s["n_cells"], np.int64)
+    for c in range(s["n_cells"]):                        # breadth-first: parents come first
+        f, k = tr["link"][c, 0], tr["link"][c, 1]
+        if k:
+            lvl[f:f + k] = lvl[c] + 1
+    key_o = {(int(l), int(b), int(c)): i for i, (l, b, c) in enumerate(zip(oc["level"], oc["begin"], oc["count"]))}
+    idx = np.array([key_o[(int(l), int(b), int(c))] for l, (b, c) in zip(lvl, tr["link"][:, 2:4])])
+    assert len(set(idx.tolist())) == o.n_cells
+    # members of every cell are the same SET (order inside a leaf may differ)
+    operm = o.perm()
+    for c in np.random.default_rng(0).choice(o.n_cells, size=min(64, o.n_cells), replace=False):
+        b, k = tr["link"][c, 2], tr["link"][c, 3]
+        assert set(tr["perm"][b:b + k].tolist()) == set(operm[b:b + k].tolist())
+    # leaf / node flags and child structure
+    assert np.array_equal(tr["link"][:, 1], oc["n_child"][idx])
+    for c in range(min(o.n_cells, 2000)):
+        f, k = tr["link"][c, 0], tr["link"][c, 1]
+        if k:
+            want = [x for x in oc["child"][idx[c]] if x >= 0]
+            assert idx[f:f + k].tolist() == want     # octant order 4bx+2by+bz
+    # boundary cubes: bit-identical fp32 (Fig. 1)
+    assert np.array_equal(tr["bnd"][:, :3], oc["b"][idx].astype(np.float32))
+    assert np.array_equal(tr["bnd"][:, 3], oc["h"][idx].astype(np.float32))
+    # moments: fp64 parallel-axis vs fp64 direct sums, compared after fp32 rounding
+    assert np.allclose(tr["xm"][:, 3], oc["M"][idx], rtol=2e-7, atol=0)
+    ext = np.abs(pos).max()
+    assert np.abs(tr["xm"][:, :3] - oc["X"][idx]).max() <= 1.2e-7 * ext
+    qs = np.abs(oc["Q"][idx]).max(axis=1, keepdims=True) + 1e-300
+    assert (np.abs(tr["q"] - oc["Q"][idx]) / qs).max() <= 2e-7
+    # groups in the same (Morton) order
+    assert np.array_equal(idx[tr["groups"]], o.groups())
+
+
+@pytest.mark.parametrize("name,n_group", [("plummer_1k", 16), ("plummer_1k", 64), ("plummer_64k", 64), ("cube_64k", 16)])
+def test_tree_matches_oracle(name, n_group):
+    pos, mass, _, _, n_leaf = inputs.make(name)
+    _compare(pos, mass, n_leaf, n_group)
+
+
+@pytest.mark.parametrize("n_leaf", [1, 8, 32])
+def test_tree_matches_oracle_n_leaf(n_leaf):
+    pos, mass = inputs.plummer(4096, 11)
+    _compare(pos, mass, n_leaf, max(n_leaf, 24))
+
+
+def test_degenerate_inputs():
+    rng = np.random.default_rng(5)
+    one = np.array([[0.25, -1.0, 3.0]], np.float32)
+    _compare(one, np.ones(1, np.float32), 16, 16)                       # single particle: root is a leaf
+    same = np.repeat(one, 100, axis=0)
+    _compare(same, np.full(100, 0.01, np.float32), 16, 64)              # all coincident: side = 1, level-21 leaf
+    pos = rng.random((300, 3)).astype(np.float32)
+    pos[:150] = pos[0]                                                  # a coincident clump inside a cloud
+    _compare(pos, rng.random(300).astype(np.float32), 8, 32)
+    mass = rng.random(500).astype(np.float32)
+    mass[::3] = 0.0                                                     # massless particles
+    _compare(rng.standard_normal((500, 3)).astype(np.float32), mass, 4, 16)
+    line = np.zeros((64, 3), np.float32)
+    line[:, 0] = np.linspace(-1, 1, 64)                                 # collinear: two axes have zero extent
+    _compare(line, np.ones(64, np.float32), 4, 8)
