@@ -6,6 +6,7 @@
 
 #include <chrono>
 #include <cmath>
+#include <cstddef>
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
@@ -90,6 +91,9 @@ int collect(tc_ctx* c) {
   c->stats.t_gpu_ms = ms;
   c->stats.n_pc_total = (int64_t)h.n_pc_total; c->stats.n_pp_total = (int64_t)h.n_pp_total;
   c->stats.n_tests_total = (int64_t)h.n_tests_total; c->stats.n_spills = (int64_t)h.n_spills;
+  if (h.overflow) {
+    cudaMemset((char*)c->d_ctr + offsetof(tc::DeviceCounters, overflow), 0, sizeof(unsigned int));
+  }
   if (h.overflow) return fail(c, TC_EOVERFLOW, "tc_forces: a walk stack exceeded its global spill capacity");
   return TC_OK;
 }
@@ -117,6 +121,7 @@ tc_ctx* tc_create_ex(uint32_t flags) {
   if (e == cudaSuccess) e = cudaEventCreate(&c->ev0);
   if (e == cudaSuccess) e = cudaEventCreate(&c->ev1);
   if (e == cudaSuccess) e = cudaMalloc((void**)&c->d_ctr, sizeof(tc::DeviceCounters));
+  if (e == cudaSuccess) e = cudaMemset(c->d_ctr, 0, sizeof(tc::DeviceCounters));
   if (e != cudaSuccess) {
     g_create_err = std::string("tc_create: no usable CUDA device (no CPU fallback exists): ") + cudaGetErrorString(e);
     cudaGetLastError();
@@ -246,7 +251,6 @@ int tc_forces(tc_ctx* c, float theta, float eps, float* acc, float* pot) {
   const int64_t n = c->n;
   const bool acc_dev = is_device_ptr(c, acc), pot_dev = pot ? is_device_ptr(c, pot) : acc_dev;
   if (pot && acc_dev != pot_dev) return fail(c, TC_EINVAL, "tc_forces: acc and pot must both be host or both be device pointers");
-  if (c->timing_pending) { TC_CUDA(c, cudaStreamSynchronize(c->stream)); const int rc = collect(c); if (rc != TC_OK && rc != TC_EOVERFLOW) return rc; }
   if (c->cnt_cap < n) {
     cudaFree(c->d_npc); cudaFree(c->d_npp); c->d_npc = c->d_npp = nullptr; c->cnt_cap = 0;
     TC_CUDA(c, cudaMalloc((void**)&c->d_npc, sizeof(int32_t) * (size_t)n));
@@ -271,7 +275,8 @@ int tc_forces(tc_ctx* c, float theta, float eps, float* acc, float* pot) {
   L.pot = pot ? (acc_dev ? pot : c->d_pot) : nullptr;
   L.n_pc = c->d_npc; L.n_pp = c->d_npp; L.counters = c->d_ctr; L.spill = c->d_spill; L.spill_cap = c->spill_cap;
   L.stack_smem = c->stack_smem; L.n_sm = c->n_sm;
-  TC_CUDA(c, cudaMemsetAsync(c->d_ctr, 0, sizeof(tc::DeviceCounters), c->stream));
+  // stream-ordered: no host synchronisation between queued calls; the overflow flag is sticky until collect()
+  TC_CUDA(c, cudaMemsetAsync(c->d_ctr, 0, offsetof(tc::DeviceCounters, overflow), c->stream));
   TC_CUDA(c, cudaEventRecord(c->ev0, c->stream));
   const int le = tc::launch_forces(c->dview, L, c->stream);
   if (le != 0) return cuda_fail(c, (cudaError_t)le, "forces kernel launch");

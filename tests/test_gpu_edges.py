@@ -1,0 +1,146 @@
+"""Edge and degenerate cases of the CUDA path against the oracle — `-m gpu`.
+
+Empty / tiny inputs, a root that is a leaf, coincident particles (level-21
+leaves larger than N_leaf, R7), eps = 0, theta extremes, N_group > 64 (a group
+is walked once per 64 of its particles), N_group = 1, the global-memory spill
+path of the walk stack, unequal masses, call-order errors.
+"""
+import numpy as np
+import pytest
+
+from oracle import Oracle, direct
+from paper_1005_5384_b200 import binding as B
+from paper_1005_5384_b200 import build as tc_build
+from paper_1005_5384_b200 import inputs
+from test_gpu_parity import check, gpu_forces, rel_err
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module", autouse=True)
+def _built():
+    tc_build.build()
+
+
+def test_single_particle():
+    pos = np.array([[0.25, -1.0, 3.0]], np.float32)
+    mass = np.array([2.0], np.float32)
+    acc, pot, n_pc, n_pp, st = gpu_forces(pos, mass, 0.5, 0.01, 16, 64)
+    assert (acc == 0).all() and n_pc[0] == 0 and n_pp[0] == 0
+    assert abs(pot[0]) <= 1e-6 * 2.0 / 0.01          # the self term -m/eps is added and removed in fp32
+    assert st["n_cells"] == 1 and st["n_groups"] == 1
+
+
+@pytest.mark.parametrize("eps", [0.0, 0.1])
+def test_two_particles_closed_form(eps):
+    """N = 2: a = m d / (d^2 + eps^2)^(3/2) (root is a leaf, never tested)."""
+    pos = np.array([[0, 0, 0], [3, 4, 0]], np.float32)
+    mass = np.array([2.0, 5.0], np.float32)
+    acc, pot, _, n_pp, _ = gpu_forces(pos, mass, 0.5, eps, 16, 64)
+    s3 = (25.0 + eps * eps) ** 1.5
+    assert np.allclose(acc[0], 5.0 * np.array([3, 4, 0]) / s3, rtol=2e-6)
+    assert np.allclose(acc[1], -2.0 * np.array([3, 4, 0]) / s3, rtol=2e-6)
+    assert np.allclose(pot, [-5.0 / np.sqrt(25 + eps * eps), -2.0 / np.sqrt(25 + eps * eps)], rtol=1e-5)
+    assert (n_pp == 1).all()
+
+
+@pytest.mark.parametrize("eps", [0.0, 0.01])
+def test_coincident_particles_level21_leaf(eps):
+    """200 particles at one point + a Plummer cloud: the point is a level-21 leaf with count > N_leaf
+    and > 64 (R7); with eps = 0 coincident pairs contribute nothing (O6)."""
+    pos, mass = inputs.plummer(2048, 11)
+    pos[:200] = pos[0]
+    acc, pot, n_pc, n_pp, st = gpu_forces(pos, mass, 0.5, eps, 16, 64)
+    o = Oracle(pos, mass, 16, 64)
+    assert st["depth"] == 21 == o.depth
+    ref = o.forces(0.5, eps, shadow32=True)
+    check(acc, pot, n_pc, n_pp, ref)
+
+
+@pytest.mark.parametrize("n_leaf,n_group", [(1, 1), (4, 256), (16, 1000), (64, 64), (2048, 2048)])
+def test_leaf_and_group_sizes(n_leaf, n_group):
+    pos, mass = inputs.plummer(3000, 12)
+    acc, pot, n_pc, n_pp, st = gpu_forces(pos, mass, 0.6, 0.02, n_leaf, n_group)
+    o = Oracle(pos, mass, n_leaf, n_group)
+    assert st["n_groups"] == o.n_groups
+    check(acc, pot, n_pc, n_pp, o.forces(0.6, 0.02, shadow32=True))
+
+
+@pytest.mark.parametrize("theta", [0.0, 0.05, 2.0, 1e3])
+def test_theta_extremes(theta):
+    pos, mass = inputs.uniform_cube(4096, 13)
+    acc, pot, n_pc, n_pp, _ = gpu_forces(pos, mass, theta, 0.01, 8, 32)
+    ref = Oracle(pos, mass, 8, 32).forces(theta, 0.01, shadow32=True)
+    assert np.array_equal(n_pc, ref["n_pc"]) and np.array_equal(n_pp, ref["n_pp"])
+    if theta <= 2.0:       # beyond that the method itself is meaningless; counts still agree
+        check(acc, pot, n_pc, n_pp, ref)
+
+
+def test_spill_path_matches_and_is_exercised():
+    """stack_smem = 64 forces the walk stack through its global-memory spill: same result."""
+    pos, mass = inputs.plummer(32768, 14)
+    a0, p0, c0, d0, s0 = gpu_forces(pos, mass, 0.2, 0.01, 2, 16)
+    a1, p1, c1, d1, s1 = gpu_forces(pos, mass, 0.2, 0.01, 2, 16, opts={"stack_smem": 64})
+    assert s1["n_spills"] > 0 and s0["n_spills"] == 0
+    assert np.array_equal(c0, c1) and np.array_equal(d0, d1)
+    assert s0["n_tests_total"] == s1["n_tests_total"]
+    # traversal order changes => summation order changes; both are within fp32 rounding of each other
+    assert rel_err(a1.astype(np.float64), a0.astype(np.float64)).max() <= 2e-5
+    gsel = np.arange(0, 2000, 50, dtype=np.int64)
+    ref = Oracle(pos, mass, 2, 16).forces(0.2, 0.01, shadow32=True, groups=gsel)
+    check(a1, p1, c1, d1, ref, ref["n_pc"] >= 0)
+
+
+def test_unequal_masses_and_massless():
+    rng = np.random.default_rng(15)
+    pos, _ = inputs.plummer(5000, 15)
+    mass = rng.uniform(0.0, 2.0, 5000).astype(np.float32)
+    mass[::7] = 0.0
+    acc, pot, n_pc, n_pp, _ = gpu_forces(pos, mass, 0.5, 0.01, 16, 64)
+    check(acc, pot, n_pc, n_pp, Oracle(pos, mass, 16, 64).forces(0.5, 0.01, shadow32=True))
+
+
+def test_eps0_against_direct():
+    pos, mass = inputs.plummer(2000, 16)
+    acc, pot, _, _, _ = gpu_forces(pos, mass, 0.0, 0.0, 16, 64)
+    dacc, dpot = direct(pos, mass, 0.0)
+    assert rel_err(acc.astype(np.float64), dacc).max() <= 2e-5
+    assert (np.abs(pot - dpot) / np.abs(dpot)).max() <= 1e-5
+
+
+def test_repeat_calls_and_rebuild_are_deterministic_in_counts():
+    pos, mass = inputs.plummer(20000, 17)
+    with B.TreeCode(n_group=64) as tc:
+        tc.set_particles(pos, mass)
+        tc.build(16)
+        a0, p0 = tc.forces(0.5, 0.01)
+        c0 = tc.counts()
+        a1, p1 = tc.forces(0.5, 0.01)
+        c1 = tc.counts()
+        assert np.array_equal(c0[0], c1[0]) and np.array_equal(c0[1], c1[1])
+        assert rel_err(a1.astype(np.float64), a0.astype(np.float64)).max() <= 2e-5
+        # new particles invalidate the tree
+        tc.set_particles(pos[:100], mass[:100])
+        with pytest.raises(B.TcError) as e:
+            tc.forces(0.5, 0.01)
+        assert e.value.code == B.TC_ESTATE
+        tc.build(16)
+        a2, _ = tc.forces(0.5, 0.01)
+        assert a2.shape == (100, 3) and np.isfinite(a2).all()
+
+
+def test_argument_errors_on_device_context():
+    pos, mass = inputs.plummer(64, 18)
+    with B.TreeCode() as tc:
+        with pytest.raises(B.TcError) as e:
+            tc.build(16)
+        assert e.value.code == B.TC_ESTATE
+        tc.set_particles(pos, mass)
+        tc.build(16)
+        acc = np.zeros((64, 3), np.float32)
+        for theta, eps in [(-1.0, 0.01), (0.5, -0.01), (float("nan"), 0.01), (0.5, float("inf"))]:
+            with pytest.raises(B.TcError) as e:
+                B.tc_forces(tc.ctx, theta, eps, acc, None)
+            assert e.value.code == B.TC_EINVAL
+        B.tc_forces(tc.ctx, 0.5, 0.01, acc, None)       # pot = NULL is allowed
+        assert np.isfinite(acc).all() and np.abs(acc).max() > 0
