@@ -52,6 +52,7 @@ def _load():
     L.orc_get_perm.argtypes = [vp, vp]
     L.orc_get_groups.argtypes = [vp, vp]
     L.orc_get_cells.argtypes = [vp] + [vp] * 13
+    L.orc_get_bnd32.argtypes = [vp, vp, vp]
     L.orc_walk.restype = i32
     L.orc_walk.argtypes = [vp, i64, f64, i32, vp, i64, vp, i64, vp, vp, vp, vp, vp]
     L.orc_forces.restype = i64
@@ -127,6 +128,13 @@ class Oracle:
                                       ("level", "parent", "child", "n_child", "begin", "count",
                                        "bmin", "bmax", "b", "h", "M", "X", "Q")])
         return d
+
+    def bnd32(self):
+        """fp32 boundary cubes of the shadow test (R20): (b32 [n_cells,3], h32 [n_cells])."""
+        b = np.zeros((self.n_cells, 3), np.float32)
+        h = np.zeros(self.n_cells, np.float32)
+        _lib.orc_get_bnd32(self._h, _p(b), _p(h))
+        return b, h
 
     # ---- walk / forces ---------------------------------------------------
     def walk(self, group: int, theta: float, shadow32: bool = False):

@@ -135,8 +135,19 @@ void cell_properties(Oracle& T, OCell& c) {
     Q[5] += T.m[i] * (3.0 * yy * yz);
   }
   for (int k = 0; k < 6; k++) c.Q[k] = Q[k];
+  // R20: the FP32 representation of the boundary must still CONTAIN the tight
+  // box, otherwise rounding of b or h can push a particle on a face of its own group's box
+  // outside the group's cube and R14 (the own leaf opens, d = 0) is lost in FP32.
+  // b32 = fp32(b); h32 = the largest distance from b32 to a face of the tight box, rounded UP.
   for (int k = 0; k < 3; k++) c.b32[k] = (float)c.b[k];
-  c.h32 = (float)c.h;
+  double far = 0.0;
+  for (int k = 0; k < 3; k++) {
+    far = std::max(far, c.bmax[k] - (double)c.b32[k]);
+    far = std::max(far, (double)c.b32[k] - c.bmin[k]);
+  }
+  float hf = (float)far;
+  if ((double)hf < far) hf = std::nextafterf(hf, std::numeric_limits<float>::infinity());
+  c.h32 = hf;
 }
 
 // ---- O2: recursive cubic subdivision (R4, R6, R7)
@@ -372,6 +383,15 @@ void orc_get_cells(void* h, int32_t* level, int32_t* parent, int32_t* child8, in
     if (hh) hh[c] = C.h;
     if (M) M[c] = C.M;
     if (Q) for (int k = 0; k < 6; k++) Q[6 * c + k] = C.Q[k];
+  }
+}
+
+// fp32 boundaries used by the shadow test (R20): b32 [n_cells,3], h32 [n_cells]
+void orc_get_bnd32(void* h, float* b32, float* h32) {
+  Oracle* T = (Oracle*)h;
+  for (size_t c = 0; c < T->cells.size(); c++) {
+    for (int k = 0; k < 3; k++) b32[3 * c + k] = T->cells[c].b32[k];
+    h32[c] = T->cells[c].h32;
   }
 }
 

@@ -307,14 +307,19 @@ int build_host_tree(const float* pos, const float* mass, int64_t n, int n_leaf, 
 #pragma omp parallel for schedule(static)
   for (int64_t c = 0; c < nc; c++) {
     const CellProp& P = prop[c];
-    // boundary cube (Fig. 1): same centre as the tight box, side = its largest side
-    double e = 0.0;
+    // boundary cube (Fig. 1): same centre as the tight box, side = its largest side.
+    // FP32 form (R20): centre rounded to nearest, half side = reach of the tight box
+    // from that rounded centre, rounded towards +inf, so the fp32 cube contains the box and the
+    // opening test gives d = 0 exactly for every cell inside the group (R14).
     float b[3];
+    double reach = 0.0;
     for (int k = 0; k < 3; k++) {
-      b[k] = (float)(((double)P.bmin[k] + (double)P.bmax[k]) / 2.0);
-      e = std::max(e, (double)P.bmax[k] - (double)P.bmin[k]);
+      const double lo = (double)P.bmin[k], hi = (double)P.bmax[k];
+      b[k] = (float)(0.5 * (lo + hi));
+      reach = std::fmax(reach, std::fmax(hi - (double)b[k], (double)b[k] - lo));
     }
-    const float h = (float)(e / 2.0);
+    float h = (float)reach;
+    if ((double)h < reach) h = std::nextafter(h, HUGE_VALF);
     const bool leaf = c_nchild[c] == 0;
     bnd[c] = make_float4(b[0], b[1], b[2], leaf ? -h : h);  // sign bit of h <=> leaf (-0.0f if h == 0)
     xm[c] = make_float4((float)P.X[0], (float)P.X[1], (float)P.X[2], (float)P.M);

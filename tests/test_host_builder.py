@@ -51,9 +51,12 @@ def _compare(pos, mass, n_leaf, n_group):
         if k:
             want = [x for x in oc["child"][idx[c]] if x >= 0]
             assert idx[f:f + k].tolist() == want     # octant order 4bx+2by+bz
-    # boundary cubes: bit-identical fp32 (Fig. 1)
-    assert np.array_equal(tr["bnd"][:, :3], oc["b"][idx].astype(np.float32))
-    assert np.array_equal(tr["bnd"][:, 3], oc["h"][idx].astype(np.float32))
+    # boundary cubes: bit-identical fp32 (Fig. 1; fp32 form = reading R20)
+    b32, h32 = o.bnd32()
+    assert np.array_equal(tr["bnd"][:, :3], b32[idx])
+    assert np.array_equal(tr["bnd"][:, 3], h32[idx])
+    assert np.array_equal(b32, oc["b"].astype(np.float32))
+    assert (h32 >= oc["h"]).all() and (h32 <= oc["h"] * (1 + 3e-7) + 1.2e-7 * np.abs(oc["b"]).max(1)).all()
     # moments: fp64 parallel-axis vs fp64 direct sums, compared after fp32 rounding
     assert np.allclose(tr["xm"][:, 3], oc["M"][idx], rtol=2e-7, atol=0)
     ext = np.abs(pos).max()

@@ -144,3 +144,33 @@ def test_fp32_shadow_flips_are_borderline():
         assert r64["n_pc"][i] == r32["n_pc"][i] and r64["n_pp"][i] == r32["n_pp"][i]
     # total flips counted the same way in both modes
     assert np.array_equal(r64["flips"], r32["flips"])
+
+
+# ---- R20: the fp32 form of the boundary contains the tight box, so R14 survives in FP32 ----
+@pytest.mark.parametrize("n_leaf,n_group", [(4, 64), (1, 8), (16, 64)])
+def test_fp32_boundary_contains_box_and_own_cells_always_open(n_leaf, n_group):
+    """Regression pin (found on the GPU): with b32 = fp32(b), h32 = fp32(h) a particle on a face of
+    its group's tight box can fall outside the fp32 cube; alone in a leaf (h = 0) it is then NOT
+    opened and meets its own monopole.  Under R20 every cell inside a group opens in fp32 too."""
+    pos, mass = inputs.plummer(3000, 12)
+    o = oracle.Oracle(pos, mass, n_leaf, n_group)
+    c = o.cells()
+    b32, h32 = o.bnd32()
+    perm = o.perm()
+    x = pos.astype(np.float32)
+    # containment as the FP32 test evaluates it: fl32(|x - b32|) <= h32 for every member of every cell
+    for i in range(o.n_cells):
+        mem = perm[c["begin"][i]:c["begin"][i] + c["count"][i]]
+        reach = np.abs(x[mem] - b32[i]).astype(np.float32).max()
+        assert reach <= h32[i]
+    assert (h32 >= c["h"]).all()
+    ulp = 1.2e-7 * (np.abs(c["b"]).max(1) + c["h"])
+    assert (h32 - c["h"] <= 2 * ulp).all()          # ... and by no more than rounding
+    # consequence: in the fp32 shadow no cell overlapping a group's own particles is left unopened,
+    # and the shadow lists still cover every particle exactly once
+    groups = o.groups()
+    for g in range(0, o.n_groups, 3):
+        gb, ge = c["begin"][groups[g]], c["begin"][groups[g]] + c["count"][groups[g]]
+        cl, ll, _, _, _ = o.walk(g, 0.6, shadow32=True)
+        assert not ((c["begin"][cl] < ge) & (c["begin"][cl] + c["count"][cl] > gb)).any()
+        assert c["count"][cl].sum() + c["count"][ll].sum() == o.n
