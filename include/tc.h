@@ -105,7 +105,7 @@ int tc_forces(tc_ctx* ctx, float theta, float eps, float* acc, float* pot);
 /* Options (double-valued).  Keys:
  *   "n_group"     N_group >= 1; takes effect at the next tc_build
  *   "stack_smem"  walk-stack entries kept in shared memory per warp before
- *                 spilling to global memory: 512 (default) or 64 (test of the
+ *                 spilling to global memory: 256 (default) or 64 (test of the
  *                 spill path)
  * Unknown key or bad value -> TC_EINVAL.                                        */
 int tc_set_option(tc_ctx* ctx, const char* key, double value);

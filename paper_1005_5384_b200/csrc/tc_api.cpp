@@ -24,7 +24,7 @@ struct tc_ctx {
   std::string err;
   // options
   int n_group = 64;
-  int stack_smem = 512;
+  int stack_smem = 256;
   // particles (host copy, caller order)
   std::vector<float> pos, mass;
   int64_t n = 0;
@@ -156,7 +156,7 @@ int tc_set_option(tc_ctx* c, const char* key, double v) {
     c->n_group = (int)v; return TC_OK;
   }
   if (!std::strcmp(key, "stack_smem")) {
-    if (v != 512.0 && v != 64.0) return fail(c, TC_EINVAL, "tc_set_option: stack_smem must be 512 or 64");
+    if (v != 256.0 && v != 64.0) return fail(c, TC_EINVAL, "tc_set_option: stack_smem must be 256 or 64");
     c->stack_smem = (int)v; return TC_OK;
   }
   return fail(c, TC_EINVAL, std::string("tc_set_option: unknown key '") + key + "'");

@@ -341,9 +341,33 @@ int build_host_tree(const float* pos, const float* mass, int64_t n, int n_leaf, 
     part[t] = make_float4(pos[3 * i], pos[3 * i + 1], pos[3 * i + 2], mass[i]);
     orig[t] = (int32_t)i;
   }
-  for (size_t g = 0; g < groups.size(); g++) {
-    const int32_t c = groups[g];
-    grp[g] = make_int4(c, c_begin[c], c_count[c], 0);
+  // Schedule (grp[i].w = i-th group to run): the persistent kernel hands groups out through an
+  // atomic counter, so costly groups go first and the tail of the launch is made of cheap ones.
+  // Cost model = issue slots per list entry of the kernel's lane mapping (tc_kernels.cu): a pass
+  // over m <= 64 particles costs min_S ceil(m / floor(32/S)) / S.  Stable: Morton order inside a
+  // cost class keeps neighbouring groups together.
+  {
+    double pass_cost[65];
+    for (int m = 0; m <= 64; m++) {
+      double best = 1e30;
+      for (int sl = 1; sl <= 32; sl++) {
+        const int q = 32 / sl, k = (m + q - 1) / q;
+        if (k >= 1 && k <= 4) best = std::min(best, (double)k / sl);
+      }
+      pass_cost[m] = (m == 0) ? 0.0 : best;
+    }
+    std::vector<std::pair<float, int32_t>> order(groups.size());
+    for (size_t g = 0; g < groups.size(); g++) {
+      const int64_t cnt = c_count[groups[g]];
+      const double cost = (double)(cnt / 64) * pass_cost[64] + pass_cost[cnt % 64];
+      order[g] = std::make_pair((float)-cost, (int32_t)g);
+    }
+    std::stable_sort(order.begin(), order.end(),
+                     [](const std::pair<float, int32_t>& a, const std::pair<float, int32_t>& b) { return a.first < b.first; });
+    for (size_t g = 0; g < groups.size(); g++) {
+      const int32_t c = groups[g];
+      grp[g] = make_int4(c, c_begin[c], c_count[c], order[g].second);
+    }
   }
   return TC_OK;
 }

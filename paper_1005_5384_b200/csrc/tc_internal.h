@@ -24,7 +24,8 @@ constexpr int kMaxLevel = 21;  // 3 x 21 = 63-bit Morton keys (R7)
 //                                                 leaf -> (first_body,  n_body)
 //   part[i] = (x, y, z, m)           particles in tree (Morton) order
 //   orig[i] = caller's index of tree-order particle i
-//   grp [g] = (cell, first_body, n_body, 0)  groups in Morton order
+//   grp [g] = (cell, first_body, n_body, sched)  groups in Morton order; sched = index of the
+//             g-th group to RUN (costly groups first, tc_build.cpp)
 struct PackedLayout {
   size_t off_bnd = 0, off_xm = 0, off_q0 = 0, off_q1 = 0, off_part = 0, off_orig = 0, off_grp = 0;
   size_t bytes = 0;
@@ -82,7 +83,7 @@ struct ForceLaunch {
   DeviceCounters* counters = nullptr;
   uint32_t* spill = nullptr;  // device [n_warps_total * spill_cap]
   int spill_cap = 0;
-  int stack_smem = 1024;
+  int stack_smem = 256;
   int n_sm = 148;
 };
 

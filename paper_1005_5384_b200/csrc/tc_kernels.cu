@@ -10,13 +10,17 @@
 //     lane (boundary + multipole, issued together so an iteration costs one memory
 //     latency);
 //   * ballot/popc compaction sorts the children into: stack (opened nodes), a queue
-//     of opened leaves, and a shared-memory chunk of un-opened cells' multipoles;
+//     of opened leaves, and a shared-memory chunk of un-opened cells' multipoles
+//     (48-byte records);
 //   * a chunk is evaluated as soon as it fills (FP32 FMA + one rsqrt.approx per
 //     interaction), so no interaction list ever reaches global memory and there is
 //     no count pass, no host scan, no second walk;
-//   * lanes map to (particle, list slice): a group of P <= 32 particles uses
-//     floor(32/P) slices of the chunk at once and reduces them with shuffles at the
-//     end — the fix for the paper's 30 % thread utilisation.
+//   * lanes map to (list slice s, particle p): a pass over m <= 64 particles picks
+//     S slices and k = ceil(m / floor(32/S)) <= 4 particles per lane so that k/S is
+//     minimal; every list record is loaded from shared memory once per lane and
+//     applied to the lane's k particles (register blocking), slices are reduced with
+//     shuffles at the end — the fix for the paper's 30 % thread utilisation
+//     (PAPER.md:175).
 // No tensor cores: this is not a dense contraction.
 #include <cuda_runtime.h>
 
@@ -28,21 +32,53 @@ namespace tc {
 namespace {
 
 constexpr int kWarpsPerCta = 8;
-constexpr int kCellCap = 96;    // un-opened cells staged per warp before evaluation
-constexpr int kLeafQCap = 64;   // opened-leaf ranges queued per warp
-constexpr int kBodyCap = 128;   // bodies staged per warp per evaluation round
+constexpr int kCellCap = 96;     // un-opened cells staged per warp before evaluation
+constexpr int kLeafQCap = 128;   // opened-leaf ranges queued per warp
+constexpr int kBodyCap = 128;    // bodies staged per warp per evaluation round
+constexpr int kMaxK = 4;         // particles per lane
+constexpr int kPass = 64;        // particles of a group handled per walk
 constexpr unsigned kFull = 0xffffffffu;
+
+struct __align__(16) CellRec {   // one un-opened cell: 48 bytes
+  float4 xm;                     // (X, Y, Z, M)
+  float4 q0;                     // (Qxx, Qyy, Qzz, Qxy)
+  float2 q1;                     // (Qxz, Qyz)
+  float2 pad;
+};
+
+struct BodyStage {
+  float4 body[kBodyCap];         // (x, y, z, m)
+  int bidx[kBodyCap];            // flattened body indices of the current round
+};
 
 template <int STK>
 struct __align__(16) WarpSmem {
-  float4 cxm[kCellCap];    // (X, Y, Z, M)
-  float4 cq0[kCellCap];    // (Qxx, Qyy, Qzz, Qxy)
-  float4 body[kBodyCap];   // (x, y, z, m)
-  float2 cq1[kCellCap];    // (Qxz, Qyz)
-  int2 leafq[kLeafQCap];   // (first_body, n_body)
-  int bidx[kBodyCap];      // flattened body indices of the current round
-  uint32_t stack[STK];     // nodes to expand: first_child << 3 | (n_child - 1)
+  union {                        // cells are flushed before bodies are staged
+    CellRec cell[kCellCap];
+    BodyStage bs;
+  } u;
+  int2 leafq[kLeafQCap];         // (first_body, n_body)
+  uint32_t stack[STK];           // nodes to expand: first_child << 3 | (n_child - 1)
 };
+
+// Lane mapping table: for m particles in a pass the slice count S that minimises
+// k / S with k = ceil(m / floor(32 / S)) <= kMaxK (ties: fewer particles per lane).
+struct SliceTable {
+  unsigned char S[kPass + 1];
+  constexpr SliceTable() : S{} {
+    for (int m = 0; m <= kPass; m++) {
+      int bestS = 1, bestK = 64;
+      for (int s = 1; s <= 32; s++) {
+        const int q = 32 / s;
+        const int k = (m + q - 1) / q;
+        if (k < 1 || k > kMaxK) continue;
+        if (k * bestS < bestK * s) { bestS = s; bestK = k; }   // k/s < bestK/bestS
+      }
+      S[m] = (unsigned char)bestS;
+    }
+  }
+};
+__constant__ SliceTable c_slices = SliceTable();
 
 __device__ __forceinline__ float rsqrt_approx(float x) {
   float y;
@@ -53,14 +89,17 @@ __device__ __forceinline__ float rsqrt_approx(float x) {
 struct Acc {
   float ax, ay, az, pot;
 };
+struct Pos {
+  float x, y, z;
+};
 
 // particle-cell: monopole + traceless quadrupole (O6), d = X - x_i:
 //   a   += M d/s^3 - Q d/s^5 + (5/2)(d^T Q d) d/s^7
 //   phi += -M/s - (1/2)(d^T Q d)/s^5
 // 33 FP32 instructions + 1 MUFU.
-__device__ __forceinline__ void pc_interact(float xi, float yi, float zi, float eps2, const float4 xm,
-                                            const float4 q0, const float2 q1, Acc& a) {
-  const float dx = xm.x - xi, dy = xm.y - yi, dz = xm.z - zi;
+__device__ __forceinline__ void pc_interact(const Pos& p, float eps2, const float4 xm, const float4 q0,
+                                            const float2 q1, Acc& a) {
+  const float dx = xm.x - p.x, dy = xm.y - p.y, dz = xm.z - p.z;
   const float s2 = fmaf(dz, dz, fmaf(dy, dy, fmaf(dx, dx, eps2)));
   const float rinv = rsqrt_approx(s2);
   const float rinv2 = rinv * rinv;
@@ -82,8 +121,8 @@ __device__ __forceinline__ void pc_interact(float xi, float yi, float zi, float 
 //   a += m_j d/s^3, phi += -m_j/s.   13 FP32 instructions + 1 MUFU.
 // kEps0: eps == 0, coincident pairs (and the particle itself) contribute nothing.
 template <bool kEps0>
-__device__ __forceinline__ void pp_interact(float xi, float yi, float zi, float eps2, const float4 b, Acc& a) {
-  const float dx = b.x - xi, dy = b.y - yi, dz = b.z - zi;
+__device__ __forceinline__ void pp_interact(const Pos& p, float eps2, const float4 b, Acc& a) {
+  const float dx = b.x - p.x, dy = b.y - p.y, dz = b.z - p.z;
   const float s2 = fmaf(dz, dz, fmaf(dy, dy, fmaf(dx, dx, eps2)));
   float rinv = rsqrt_approx(s2);
   if (kEps0) rinv = (s2 > 0.f) ? rinv : 0.f;
@@ -94,54 +133,91 @@ __device__ __forceinline__ void pp_interact(float xi, float yi, float zi, float 
   a.ax = fmaf(mr3, dx, a.ax); a.ay = fmaf(mr3, dy, a.ay); a.az = fmaf(mr3, dz, a.az);
 }
 
-// Lane mapping of one batch of P <= 32 particles: lane = slice * P + particle.
-struct Batch {
-  int P;        // particles in the batch (0: batch unused) — warp-uniform
-  int S;        // slices = 32 / P                           — warp-uniform
-  int s;        // this lane's slice
-  bool active;  // lane < P * S
-  float x, y, z;
-  Acc a;
+// Lane mapping of one pass over m <= 64 particles of a group (see file header):
+// lane = s * q + p, q = floor(32 / S); the lane's j-th particle is j * q + p.
+struct Lanes {
+  int S, q, k;   // warp-uniform
+  int s, p;      // this lane's slice and particle column
+  bool active;   // lane < S * q
 };
 
-template <int STK>
-__device__ __forceinline__ void eval_cells(const WarpSmem<STK>& sm, int cnt, float eps2, Batch (&B)[2]) {
+// Un-opened cells (List 3): slice s takes records s, s+S, s+2S, ...
+// Each record is loaded once and applied to the lane's K particles.
+template <int K>
+__device__ __forceinline__ void eval_cells_k(const CellRec* __restrict__ rec, int cnt, float eps2, const Lanes& L,
+                                             const Pos (&P)[kMaxK], Acc (&A)[kMaxK]) {
+  if (!L.active) return;
+  const int st = L.S;
+  int e = L.s;
+  for (; e + st < cnt; e += 2 * st) {            // two records in flight
+    const CellRec* r0 = rec + e;
+    const CellRec* r1 = r0 + st;
+    const float4 a0 = r0->xm, b0 = r0->q0; const float2 c0 = r0->q1;
+    const float4 a1 = r1->xm, b1 = r1->q0; const float2 c1 = r1->q1;
 #pragma unroll
-  for (int b = 0; b < 2; b++) {
-    if (B[b].P == 0) continue;   // warp-uniform
-    if (B[b].active) {
-      const int S = B[b].S;
-      Acc a = B[b].a;
-#pragma unroll 2
-      for (int e = B[b].s; e < cnt; e += S) pc_interact(B[b].x, B[b].y, B[b].z, eps2, sm.cxm[e], sm.cq0[e], sm.cq1[e], a);
-      B[b].a = a;
-    }
+    for (int j = 0; j < K; j++) pc_interact(P[j], eps2, a0, b0, c0, A[j]);
+#pragma unroll
+    for (int j = 0; j < K; j++) pc_interact(P[j], eps2, a1, b1, c1, A[j]);
+  }
+  if (e < cnt) {
+    const CellRec* r0 = rec + e;
+    const float4 a0 = r0->xm, b0 = r0->q0; const float2 c0 = r0->q1;
+#pragma unroll
+    for (int j = 0; j < K; j++) pc_interact(P[j], eps2, a0, b0, c0, A[j]);
   }
 }
 
-template <int STK, bool kEps0>
-__device__ __forceinline__ void eval_bodies(const WarpSmem<STK>& sm, int cnt, float eps2, Batch (&B)[2]) {
+__device__ __forceinline__ void eval_cells(const CellRec* rec, int cnt, float eps2, const Lanes& L,
+                                           const Pos (&P)[kMaxK], Acc (&A)[kMaxK]) {
+  switch (L.k) {                                  // warp-uniform
+    case 1: eval_cells_k<1>(rec, cnt, eps2, L, P, A); break;
+    case 2: eval_cells_k<2>(rec, cnt, eps2, L, P, A); break;
+    case 3: eval_cells_k<3>(rec, cnt, eps2, L, P, A); break;
+    default: eval_cells_k<4>(rec, cnt, eps2, L, P, A); break;
+  }
+}
+
+template <int K, bool kEps0>
+__device__ __forceinline__ void eval_bodies_k(const float4* __restrict__ body, int cnt, float eps2, const Lanes& L,
+                                              const Pos (&P)[kMaxK], Acc (&A)[kMaxK]) {
+  if (!L.active) return;
+  const int st = L.S;
+  int e = L.s;
+  for (; e + 3 * st < cnt; e += 4 * st) {        // four bodies in flight
+    const float4 b0 = body[e], b1 = body[e + st], b2 = body[e + 2 * st], b3 = body[e + 3 * st];
 #pragma unroll
-  for (int b = 0; b < 2; b++) {
-    if (B[b].P == 0) continue;
-    if (B[b].active) {
-      const int S = B[b].S;
-      Acc a = B[b].a;
-#pragma unroll 4
-      for (int e = B[b].s; e < cnt; e += S) pp_interact<kEps0>(B[b].x, B[b].y, B[b].z, eps2, sm.body[e], a);
-      B[b].a = a;
+    for (int j = 0; j < K; j++) {
+      pp_interact<kEps0>(P[j], eps2, b0, A[j]); pp_interact<kEps0>(P[j], eps2, b1, A[j]);
+      pp_interact<kEps0>(P[j], eps2, b2, A[j]); pp_interact<kEps0>(P[j], eps2, b3, A[j]);
     }
+  }
+  for (; e < cnt; e += st) {
+    const float4 b0 = body[e];
+#pragma unroll
+    for (int j = 0; j < K; j++) pp_interact<kEps0>(P[j], eps2, b0, A[j]);
+  }
+}
+
+template <bool kEps0>
+__device__ __forceinline__ void eval_bodies(const float4* body, int cnt, float eps2, const Lanes& L,
+                                            const Pos (&P)[kMaxK], Acc (&A)[kMaxK]) {
+  switch (L.k) {
+    case 1: eval_bodies_k<1, kEps0>(body, cnt, eps2, L, P, A); break;
+    case 2: eval_bodies_k<2, kEps0>(body, cnt, eps2, L, P, A); break;
+    case 3: eval_bodies_k<3, kEps0>(body, cnt, eps2, L, P, A); break;
+    default: eval_bodies_k<4, kEps0>(body, cnt, eps2, L, P, A); break;
   }
 }
 
 // Opened leaves (List 4): flatten the queued (first, n) ranges into
 // body indices, gather the bodies with one coalesced float4 load per lane, evaluate.
-template <int STK, bool kEps0>
-__device__ __forceinline__ void eval_leaves(WarpSmem<STK>& sm, int nq, const float4* __restrict__ part,
-                                            float eps2, Batch (&B)[2], int lane) {
+template <bool kEps0>
+__device__ __forceinline__ void eval_leaves(BodyStage& bs, const int2* leafq, int nq, const float4* __restrict__ part,
+                                            float eps2, const Lanes& L, const Pos (&P)[kMaxK], Acc (&A)[kMaxK],
+                                            int lane) {
   for (int r0 = 0; r0 < nq; r0 += 32) {
     int f = 0, n = 0;
-    if (r0 + lane < nq) { const int2 r = sm.leafq[r0 + lane]; f = r.x; n = r.y; }
+    if (r0 + lane < nq) { const int2 r = leafq[r0 + lane]; f = r.x; n = r.y; }
     int incl = n;   // inclusive scan of n
 #pragma unroll
     for (int d = 1; d < 32; d <<= 1) { const int t = __shfl_up_sync(kFull, incl, d); if (lane >= d) incl += t; }
@@ -149,19 +225,19 @@ __device__ __forceinline__ void eval_leaves(WarpSmem<STK>& sm, int nq, const flo
     const int total = __shfl_sync(kFull, incl, 31);
     for (int base = 0; base < total; base += kBodyCap) {
       const int k0 = max(0, base - off), k1 = min(n, base + kBodyCap - off);
-      for (int k = k0; k < k1; k++) sm.bidx[off + k - base] = f + k;
+      for (int k = k0; k < k1; k++) bs.bidx[off + k - base] = f + k;
       __syncwarp();
       const int cnt = min(kBodyCap, total - base);
-      for (int t = lane; t < cnt; t += 32) sm.body[t] = __ldg(part + sm.bidx[t]);
+      for (int t = lane; t < cnt; t += 32) bs.body[t] = __ldg(part + bs.bidx[t]);
       __syncwarp();
-      eval_bodies<STK, kEps0>(sm, cnt, eps2, B);
+      eval_bodies<kEps0>(bs.body, cnt, eps2, L, P, A);
       __syncwarp();
     }
   }
 }
 
 template <int STK, bool kEps0>
-__global__ void __launch_bounds__(kWarpsPerCta * 32)
+__global__ void __launch_bounds__(kWarpsPerCta * 32, 3)
 forces_kernel(const float4* __restrict__ bnd, const float4* __restrict__ xm, const float4* __restrict__ q0,
               const float4* __restrict__ q1, const float4* __restrict__ part, const int32_t* __restrict__ orig,
               const int4* __restrict__ grp, int n_groups, float theta, float eps,
@@ -187,28 +263,30 @@ forces_kernel(const float4* __restrict__ bnd, const float4* __restrict__ xm, con
     if (lane == 0) g = (int)atomicAdd(&ctr->next_group, 1u);
     g = __shfl_sync(kFull, g, 0);
     if (g >= n_groups) break;
-    const int4 G = __ldg(grp + g);           // (cell, first_body, n_body, 0)
+    g = __ldg(&grp[g].w);                    // schedule: costly groups first (tc_build)
+    const int4 G = __ldg(grp + g);           // (cell, first_body, n_body, -)
     const float4 gb = __ldg(bnd + G.x);
     const float gbx = gb.x, gby = gb.y, gbz = gb.z, gh = fabsf(gb.w);
 
     // groups larger than 64 particles (level-21 leaves, or N_group > 64) repeat the walk per 64
-    for (int pb = 0; pb < G.z; pb += 64) {
-      const int m = min(64, G.z - pb);
-      Batch B[2];
+    for (int pb = 0; pb < G.z; pb += kPass) {
+      const int m = min(kPass, G.z - pb);
+      Lanes L;
+      L.S = c_slices.S[m];
+      L.q = 32 / L.S;
+      L.k = (m + L.q - 1) / L.q;
+      L.s = lane / L.q;
+      L.p = lane - L.s * L.q;
+      L.active = L.s < L.S;
+      Pos P[kMaxK];
+      Acc A[kMaxK];
 #pragma unroll
-      for (int b = 0; b < 2; b++) {
-        const int P = max(0, min(32, m - 32 * b));
-        B[b].P = P;
-        B[b].S = P ? 32 / P : 1;
-        const int p = P ? lane % P : 0;
-        B[b].s = P ? lane / P : 0;
-        B[b].active = P && lane < P * B[b].S;
-        B[b].a = Acc{0.f, 0.f, 0.f, 0.f};
-        B[b].x = B[b].y = B[b].z = 0.f;
-        if (B[b].active) {
-          const float4 me = __ldg(part + G.y + pb + 32 * b + p);
-          B[b].x = me.x; B[b].y = me.y; B[b].z = me.z;
-        }
+      for (int j = 0; j < kMaxK; j++) {
+        A[j] = Acc{0.f, 0.f, 0.f, 0.f};
+        const int t = j * L.q + L.p;
+        // slots beyond m compute on a copy of the pass's first particle; never written back
+        const float4 me = __ldg(part + G.y + pb + ((L.active && t < m) ? t : 0));
+        P[j].x = me.x; P[j].y = me.y; P[j].z = me.z;
       }
 
       int ssz = 0, spill_sz = 0, ccnt = 0, lq = 0;
@@ -259,8 +337,8 @@ forces_kernel(const float4* __restrict__ bnd, const float4* __restrict__ xm, con
         const unsigned m_stack = __ballot_sync(kFull, to_stack);
         n_tests += __popc(__ballot_sync(kFull, valid));
         if (to_cell) {                                   // not opened (leaf or node): multipole (R2)
-          const int p = ccnt + __popc(m_cell & lt_mask);
-          sm.cxm[p] = cx; sm.cq0[p] = c0; sm.cq1[p] = make_float2(c1.x, c1.y);
+          CellRec& r = sm.u.cell[ccnt + __popc(m_cell & lt_mask)];
+          r.xm = cx; r.q0 = c0; r.q1 = make_float2(c1.x, c1.y);
         }
         ccnt += __popc(m_cell); n_pc += __popc(m_cell);
         if (m_leaf) {                                    // opened leaf: particle-particle
@@ -292,27 +370,30 @@ forces_kernel(const float4* __restrict__ bnd, const float4* __restrict__ xm, con
           ssz += npush;
         }
         __syncwarp();
-        if (ccnt > kCellCap - 32) { eval_cells<STK>(sm, ccnt, eps2, B); ccnt = 0; __syncwarp(); }
-        if (lq > kLeafQCap - 32) { eval_leaves<STK, kEps0>(sm, lq, part, eps2, B, lane); lq = 0; }
+        const bool flush_leaves = lq > kLeafQCap - 32;
+        if (ccnt > kCellCap - 32 || (flush_leaves && ccnt)) {
+          eval_cells(sm.u.cell, ccnt, eps2, L, P, A); ccnt = 0; __syncwarp();
+        }
+        if (flush_leaves) { eval_leaves<kEps0>(sm.u.bs, sm.leafq, lq, part, eps2, L, P, A, lane); lq = 0; }
       }
-      if (ccnt) eval_cells<STK>(sm, ccnt, eps2, B);
+      if (ccnt) eval_cells(sm.u.cell, ccnt, eps2, L, P, A);
       __syncwarp();
-      if (lq) eval_leaves<STK, kEps0>(sm, lq, part, eps2, B, lane);
+      if (lq) eval_leaves<kEps0>(sm.u.bs, sm.leafq, lq, part, eps2, L, P, A, lane);
       __syncwarp();
 
       // ---- A6: reduce the slices of every particle, write back in the caller's order
 #pragma unroll
-      for (int b = 0; b < 2; b++) {
-        if (B[b].P == 0) continue;
-        const int P = B[b].P, S = B[b].S, s = B[b].s;
-        Acc a = B[b].a;
-        for (int w = 1; w < S; w <<= 1) {
-          const float ox = __shfl_down_sync(kFull, a.ax, w * P), oy = __shfl_down_sync(kFull, a.ay, w * P);
-          const float oz = __shfl_down_sync(kFull, a.az, w * P), op = __shfl_down_sync(kFull, a.pot, w * P);
-          if (B[b].active && (s % (2 * w)) == 0 && s + w < S) { a.ax += ox; a.ay += oy; a.az += oz; a.pot += op; }
+      for (int j = 0; j < kMaxK; j++) {
+        if (j >= L.k) break;                             // warp-uniform
+        Acc a = A[j];
+        for (int w = 1; w < L.S; w <<= 1) {
+          const float ox = __shfl_down_sync(kFull, a.ax, w * L.q), oy = __shfl_down_sync(kFull, a.ay, w * L.q);
+          const float oz = __shfl_down_sync(kFull, a.az, w * L.q), op = __shfl_down_sync(kFull, a.pot, w * L.q);
+          if ((L.s % (2 * w)) == 0 && L.s + w < L.S) { a.ax += ox; a.ay += oy; a.az += oz; a.pot += op; }
         }
-        if (lane < P) {
-          const int t = G.y + pb + 32 * b + lane;
+        const int tq = j * L.q + lane;
+        if (lane < L.q && tq < m) {
+          const int t = G.y + pb + tq;
           const int i = __ldg(orig + t);
           if (!kEps0) a.pot += __ldg(part + t).w * rsqrt_approx(eps2);  // the particle met itself once
           acc[3 * (size_t)i + 0] = a.ax; acc[3 * (size_t)i + 1] = a.ay; acc[3 * (size_t)i + 2] = a.az;
@@ -343,7 +424,7 @@ int launch_t(const DeviceTree& T, const ForceLaunch& L, cudaStream_t st, int* ct
   if (e != cudaSuccess) return (int)e;
   if (per_sm < 1) per_sm = 1;
   if (ctas_per_sm_out) { *ctas_per_sm_out = per_sm; return 0; }
-  // persistent grid: every SM full, groups handed out by an atomic counter (Morton order)
+  // persistent grid: every SM full, groups handed out by an atomic counter
   const int grid = L.n_sm * per_sm;
   kern<<<grid, kWarpsPerCta * 32, smem, st>>>(T.bnd, T.xm, T.q0, T.q1, T.part, T.orig, T.grp, (int)T.n_groups,
                                                L.theta, L.eps, L.acc, L.pot, L.n_pc, L.n_pp, L.counters, L.spill,
@@ -354,7 +435,7 @@ int launch_t(const DeviceTree& T, const ForceLaunch& L, cudaStream_t st, int* ct
 int dispatch(const DeviceTree& T, const ForceLaunch& L, cudaStream_t st, int* per_sm) {
   const bool eps0 = (L.eps * L.eps == 0.f);
   if (L.stack_smem == 64) return eps0 ? launch_t<64, true>(T, L, st, per_sm) : launch_t<64, false>(T, L, st, per_sm);
-  return eps0 ? launch_t<512, true>(T, L, st, per_sm) : launch_t<512, false>(T, L, st, per_sm);
+  return eps0 ? launch_t<256, true>(T, L, st, per_sm) : launch_t<256, false>(T, L, st, per_sm);
 }
 
 }  // namespace
