@@ -17,7 +17,8 @@ import os
 import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-LIB_PATH = os.path.join(_HERE, "libtc_b200.so")
+#: the in-tree library; TC_B200_LIB points at another build of the same sources (tuning variants)
+LIB_PATH = os.environ.get("TC_B200_LIB") or os.path.join(_HERE, "libtc_b200.so")
 
 TC_OK, TC_EINVAL, TC_ESTATE, TC_ECUDA, TC_ENOMEM, TC_EOVERFLOW = 0, -1, -2, -3, -4, -5
 TC_FLAG_HOST_ONLY = 1

@@ -31,12 +31,21 @@
 namespace tc {
 namespace {
 
+#ifndef TC_MAXK
+#define TC_MAXK 4
+#endif
+#ifndef TC_MINB
+#define TC_MINB 3
+#endif
+#ifndef TC_CELLCAP
+#define TC_CELLCAP 96
+#endif
 constexpr int kWarpsPerCta = 8;
-constexpr int kCellCap = 96;     // un-opened cells staged per warp before evaluation
+constexpr int kCellCap = TC_CELLCAP;  // un-opened cells staged per warp before evaluation
 constexpr int kLeafQCap = 128;   // opened-leaf ranges queued per warp
 constexpr int kBodyCap = 128;    // bodies staged per warp per evaluation round
-constexpr int kMaxK = 4;         // particles per lane
-constexpr int kPass = 64;        // particles of a group handled per walk
+constexpr int kMaxK = TC_MAXK;   // particles per lane
+constexpr int kPass = kMaxK >= 2 ? 64 : 32;  // particles of a group handled per walk
 constexpr unsigned kFull = 0xffffffffu;
 
 struct __align__(16) CellRec {   // one un-opened cell: 48 bytes
@@ -167,13 +176,14 @@ __device__ __forceinline__ void eval_cells_k(const CellRec* __restrict__ rec, in
   }
 }
 
+template <int K = 1>
 __device__ __forceinline__ void eval_cells(const CellRec* rec, int cnt, float eps2, const Lanes& L,
                                            const Pos (&P)[kMaxK], Acc (&A)[kMaxK]) {
-  switch (L.k) {                                  // warp-uniform
-    case 1: eval_cells_k<1>(rec, cnt, eps2, L, P, A); break;
-    case 2: eval_cells_k<2>(rec, cnt, eps2, L, P, A); break;
-    case 3: eval_cells_k<3>(rec, cnt, eps2, L, P, A); break;
-    default: eval_cells_k<4>(rec, cnt, eps2, L, P, A); break;
+  if constexpr (K == kMaxK) {
+    eval_cells_k<K>(rec, cnt, eps2, L, P, A);
+  } else {
+    if (L.k == K) eval_cells_k<K>(rec, cnt, eps2, L, P, A);   // warp-uniform
+    else eval_cells<K + 1>(rec, cnt, eps2, L, P, A);
   }
 }
 
@@ -198,14 +208,14 @@ __device__ __forceinline__ void eval_bodies_k(const float4* __restrict__ body, i
   }
 }
 
-template <bool kEps0>
+template <bool kEps0, int K = 1>
 __device__ __forceinline__ void eval_bodies(const float4* body, int cnt, float eps2, const Lanes& L,
                                             const Pos (&P)[kMaxK], Acc (&A)[kMaxK]) {
-  switch (L.k) {
-    case 1: eval_bodies_k<1, kEps0>(body, cnt, eps2, L, P, A); break;
-    case 2: eval_bodies_k<2, kEps0>(body, cnt, eps2, L, P, A); break;
-    case 3: eval_bodies_k<3, kEps0>(body, cnt, eps2, L, P, A); break;
-    default: eval_bodies_k<4, kEps0>(body, cnt, eps2, L, P, A); break;
+  if constexpr (K == kMaxK) {
+    eval_bodies_k<K, kEps0>(body, cnt, eps2, L, P, A);
+  } else {
+    if (L.k == K) eval_bodies_k<K, kEps0>(body, cnt, eps2, L, P, A);
+    else eval_bodies<kEps0, K + 1>(body, cnt, eps2, L, P, A);
   }
 }
 
@@ -237,7 +247,7 @@ __device__ __forceinline__ void eval_leaves(BodyStage& bs, const int2* leafq, in
 }
 
 template <int STK, bool kEps0>
-__global__ void __launch_bounds__(kWarpsPerCta * 32, 3)
+__global__ void __launch_bounds__(kWarpsPerCta * 32, TC_MINB)
 forces_kernel(const float4* __restrict__ bnd, const float4* __restrict__ xm, const float4* __restrict__ q0,
               const float4* __restrict__ q1, const float4* __restrict__ part, const int32_t* __restrict__ orig,
               const int4* __restrict__ grp, int n_groups, float theta, float eps,
