@@ -323,12 +323,13 @@ int build_host_tree(const float* pos, const float* mass, int64_t n, int n_leaf, 
     const bool leaf = c_nchild[c] == 0;
     bnd[c] = make_float4(b[0], b[1], b[2], leaf ? -h : h);  // sign bit of h <=> leaf (-0.0f if h == 0)
     xm[c] = make_float4((float)P.X[0], (float)P.X[1], (float)P.X[2], (float)P.M);
-    q0[c] = make_float4((float)P.Q[0], (float)P.Q[1], (float)P.Q[2], (float)P.Q[3]);
+    // the device arrays carry -Q: the packed-FP32 evaluation then needs no run-time negation (tc_kernels.cu)
+    q0[c] = make_float4(-(float)P.Q[0], -(float)P.Q[1], -(float)P.Q[2], -(float)P.Q[3]);
     int32_t la, lb;
     if (leaf) { la = c_begin[c]; lb = c_count[c]; } else { la = c_first_child[c]; lb = c_nchild[c]; }
     float fa, fb;
     std::memcpy(&fa, &la, 4); std::memcpy(&fb, &lb, 4);
-    q1[c] = make_float4((float)P.Q[4], (float)P.Q[5], fa, fb);
+    q1[c] = make_float4(-(float)P.Q[4], -(float)P.Q[5], fa, fb);
     T.link[4 * c + 0] = leaf ? -1 : c_first_child[c];
     T.link[4 * c + 1] = c_nchild[c];
     T.link[4 * c + 2] = c_begin[c];
@@ -352,7 +353,7 @@ int build_host_tree(const float* pos, const float* mass, int64_t n, int n_leaf, 
       double best = 1e30;
       for (int sl = 1; sl <= 32; sl++) {
         const int q = 32 / sl, k = (m + q - 1) / q;
-        if (k >= 1 && k <= 4) best = std::min(best, (double)k / sl);
+        if (k >= 1 && k <= 4) best = std::min(best, (double)((k + 1) / 2) / sl);   // pairs of particles per lane
       }
       pass_cost[m] = (m == 0) ? 0.0 : best;
     }

@@ -19,8 +19,8 @@ constexpr int kMaxLevel = 21;  // 3 x 21 = 63-bit Morton keys (R7)
 // of 256 bytes.  Per cell c (cells in breadth-first order, children contiguous):
 //   bnd [c] = (bx, by, bz, h)        boundary cube, Fig. 1; sign bit of h set <=> leaf
 //   xm  [c] = (X, Y, Z, M)           centre of mass, mass
-//   q0  [c] = (Qxx, Qyy, Qzz, Qxy)   traceless quadrupole about X
-//   q1  [c] = (Qxz, Qyz, a, b)       a,b int bits: node -> (first_child, n_child)
+//   q0  [c] = -(Qxx, Qyy, Qzz, Qxy)  traceless quadrupole about X, NEGATED (see tc_kernels.cu)
+//   q1  [c] = (-Qxz, -Qyz, a, b)       a,b int bits: node -> (first_child, n_child)
 //                                                 leaf -> (first_body,  n_body)
 //   part[i] = (x, y, z, m)           particles in tree (Morton) order
 //   orig[i] = caller's index of tree-order particle i

@@ -31,8 +31,8 @@
 namespace tc {
 namespace {
 
-#ifndef TC_MAXK
-#define TC_MAXK 4
+#ifndef TC_MAXKP
+#define TC_MAXKP 2
 #endif
 #ifndef TC_MINB
 #define TC_MINB 3
@@ -44,8 +44,8 @@ constexpr int kWarpsPerCta = 8;
 constexpr int kCellCap = TC_CELLCAP;  // un-opened cells staged per warp before evaluation
 constexpr int kLeafQCap = 128;   // opened-leaf ranges queued per warp
 constexpr int kBodyCap = 128;    // bodies staged per warp per evaluation round
-constexpr int kMaxK = TC_MAXK;   // particles per lane
-constexpr int kPass = kMaxK >= 2 ? 64 : 32;  // particles of a group handled per walk
+constexpr int kMaxKP = TC_MAXKP; // particle PAIRS per lane (packed f32x2 arithmetic)
+constexpr int kPass = 64;        // particles of a group handled per walk
 constexpr unsigned kFull = 0xffffffffu;
 
 struct __align__(16) CellRec {   // one un-opened cell: 48 bytes
@@ -71,7 +71,7 @@ struct __align__(16) WarpSmem {
 };
 
 // Lane mapping table: for m particles in a pass the slice count S that minimises
-// k / S with k = ceil(m / floor(32 / S)) <= kMaxK (ties: fewer particles per lane).
+// kp / S with kp = ceil(m / (2 floor(32 / S))) <= kMaxKP particle pairs per lane (ties: fewer pairs).
 struct SliceTable {
   unsigned char S[kPass + 1];
   constexpr SliceTable() : S{} {
@@ -79,8 +79,8 @@ struct SliceTable {
       int bestS = 1, bestK = 64;
       for (int s = 1; s <= 32; s++) {
         const int q = 32 / s;
-        const int k = (m + q - 1) / q;
-        if (k < 1 || k > kMaxK) continue;
+        const int k = (m + 2 * q - 1) / (2 * q);
+        if (k < 1 || k > kMaxKP) continue;
         if (k * bestS < bestK * s) { bestS = s; bestK = k; }   // k/s < bestK/bestS
       }
       S[m] = (unsigned char)bestS;
@@ -95,66 +95,81 @@ __device__ __forceinline__ float rsqrt_approx(float x) {
   return y;
 }
 
-struct Acc {
-  float ax, ay, az, pot;
+// ---- packed FP32 pairs (sm_100a FFMA2 / FMUL2 / FADD2): one instruction does the arithmetic of
+// the lane's TWO particles (lo = even, hi = odd) at half the issue cost of two scalar instructions.
+// A scalar operand (a field of the list record) is broadcast by the hardware (`R.F32` operand form).
+typedef unsigned long long f2;
+__device__ __forceinline__ f2 pk(float lo, float hi) { f2 r; asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(lo), "f"(hi)); return r; }
+__device__ __forceinline__ f2 bc(float x) { return pk(x, x); }
+__device__ __forceinline__ float lo(f2 v) { float a, b; asm("mov.b64 {%0, %1}, %2;" : "=f"(a), "=f"(b) : "l"(v)); return a; }
+__device__ __forceinline__ float hi(f2 v) { float a, b; asm("mov.b64 {%0, %1}, %2;" : "=f"(a), "=f"(b) : "l"(v)); return b; }
+__device__ __forceinline__ f2 add2(f2 a, f2 b) { f2 d; asm("add.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b)); return d; }
+__device__ __forceinline__ f2 sub2(f2 a, f2 b) { f2 d; asm("sub.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b)); return d; }
+__device__ __forceinline__ f2 mul2(f2 a, f2 b) { f2 d; asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b)); return d; }
+__device__ __forceinline__ f2 fma2(f2 a, f2 b, f2 c) { f2 d; asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(d) : "l"(a), "l"(b), "l"(c)); return d; }
+
+struct Acc2 {      // accumulators of a particle pair; `npot` accumulates -phi (negated at write-back)
+  f2 ax, ay, az, npot;
 };
-struct Pos {
-  float x, y, z;
+struct Pos2 {      // positions of a particle pair
+  f2 x, y, z;
 };
 
 // particle-cell: monopole + traceless quadrupole (O6), d = X - x_i:
 //   a   += M d/s^3 - Q d/s^5 + (5/2)(d^T Q d) d/s^7
 //   phi += -M/s - (1/2)(d^T Q d)/s^5
-// 33 FP32 instructions + 1 MUFU.
-__device__ __forceinline__ void pc_interact(const Pos& p, float eps2, const float4 xm, const float4 q0,
-                                            const float2 q1, Acc& a) {
-  const float dx = xm.x - p.x, dy = xm.y - p.y, dz = xm.z - p.z;
-  const float s2 = fmaf(dz, dz, fmaf(dy, dy, fmaf(dx, dx, eps2)));
-  const float rinv = rsqrt_approx(s2);
-  const float rinv2 = rinv * rinv;
-  const float rinv3 = rinv * rinv2;
-  const float rinv5 = rinv3 * rinv2;
-  const float qdx = fmaf(q1.x, dz, fmaf(q0.w, dy, q0.x * dx));
-  const float qdy = fmaf(q1.y, dz, fmaf(q0.y, dy, q0.w * dx));
-  const float qdz = fmaf(q0.z, dz, fmaf(q1.y, dy, q1.x * dx));
-  const float dqd = fmaf(dz, qdz, fmaf(dy, qdy, dx * qdx));
-  const float t5 = dqd * rinv5;
-  a.pot = fmaf(-xm.w, rinv, a.pot);
-  a.pot = fmaf(-0.5f, t5, a.pot);
-  const float c = fmaf(2.5f, t5 * rinv2, xm.w * rinv3);
-  a.ax = fmaf(c, dx, a.ax); a.ay = fmaf(c, dy, a.ay); a.az = fmaf(c, dz, a.az);
-  a.ax = fmaf(-rinv5, qdx, a.ax); a.ay = fmaf(-rinv5, qdy, a.ay); a.az = fmaf(-rinv5, qdz, a.az);
+// The record carries -Q (nq0, nq1; negated on the host), so no operand needs a run-time negation.
+// 33 packed FP32 instructions + 2 MUFU per PAIR of interactions.
+__device__ __forceinline__ void pc_interact(const Pos2& p, float eps2, const float4 xm, const float4 nq0,
+                                            const float2 nq1, Acc2& a) {
+  const f2 dx = sub2(bc(xm.x), p.x), dy = sub2(bc(xm.y), p.y), dz = sub2(bc(xm.z), p.z);
+  const f2 s2 = fma2(dz, dz, fma2(dy, dy, fma2(dx, dx, bc(eps2))));
+  const f2 ri = pk(rsqrt_approx(lo(s2)), rsqrt_approx(hi(s2)));
+  const f2 ri2 = mul2(ri, ri);
+  const f2 ri3 = mul2(ri, ri2);
+  const f2 ri5 = mul2(ri3, ri2);
+  const f2 gx = fma2(bc(nq1.x), dz, fma2(bc(nq0.w), dy, mul2(bc(nq0.x), dx)));   // -(Q d)
+  const f2 gy = fma2(bc(nq1.y), dz, fma2(bc(nq0.y), dy, mul2(bc(nq0.w), dx)));
+  const f2 gz = fma2(bc(nq0.z), dz, fma2(bc(nq1.y), dy, mul2(bc(nq1.x), dx)));
+  const f2 g = fma2(dz, gz, fma2(dy, gy, mul2(dx, gx)));                         // -(d^T Q d)
+  const f2 t5 = mul2(g, ri5);
+  a.npot = fma2(bc(xm.w), ri, a.npot);
+  a.npot = fma2(bc(-0.5f), t5, a.npot);
+  const f2 c = fma2(bc(-2.5f), mul2(t5, ri2), mul2(bc(xm.w), ri3));
+  a.ax = fma2(c, dx, a.ax); a.ay = fma2(c, dy, a.ay); a.az = fma2(c, dz, a.az);
+  a.ax = fma2(ri5, gx, a.ax); a.ay = fma2(ri5, gy, a.ay); a.az = fma2(ri5, gz, a.az);
 }
 
 // particle-particle, Plummer softening (O6), d = x_j - x_i:
-//   a += m_j d/s^3, phi += -m_j/s.   13 FP32 instructions + 1 MUFU.
+//   a += m_j d/s^3, phi += -m_j/s.   13 packed FP32 instructions + 2 MUFU per pair of interactions.
 // kEps0: eps == 0, coincident pairs (and the particle itself) contribute nothing.
 template <bool kEps0>
-__device__ __forceinline__ void pp_interact(const Pos& p, float eps2, const float4 b, Acc& a) {
-  const float dx = b.x - p.x, dy = b.y - p.y, dz = b.z - p.z;
-  const float s2 = fmaf(dz, dz, fmaf(dy, dy, fmaf(dx, dx, eps2)));
-  float rinv = rsqrt_approx(s2);
-  if (kEps0) rinv = (s2 > 0.f) ? rinv : 0.f;
-  const float rinv2 = rinv * rinv;
-  const float mr = b.w * rinv;
-  const float mr3 = mr * rinv2;
-  a.pot -= mr;
-  a.ax = fmaf(mr3, dx, a.ax); a.ay = fmaf(mr3, dy, a.ay); a.az = fmaf(mr3, dz, a.az);
+__device__ __forceinline__ void pp_interact(const Pos2& p, float eps2, const float4 b, Acc2& a) {
+  const f2 dx = sub2(bc(b.x), p.x), dy = sub2(bc(b.y), p.y), dz = sub2(bc(b.z), p.z);
+  const f2 s2 = fma2(dz, dz, fma2(dy, dy, fma2(dx, dx, bc(eps2))));
+  float r0 = rsqrt_approx(lo(s2)), r1 = rsqrt_approx(hi(s2));
+  if (kEps0) { r0 = (lo(s2) > 0.f) ? r0 : 0.f; r1 = (hi(s2) > 0.f) ? r1 : 0.f; }
+  const f2 ri = pk(r0, r1);
+  const f2 ri2 = mul2(ri, ri);
+  const f2 mr = mul2(bc(b.w), ri);
+  const f2 mr3 = mul2(mr, ri2);
+  a.npot = add2(a.npot, mr);
+  a.ax = fma2(mr3, dx, a.ax); a.ay = fma2(mr3, dy, a.ay); a.az = fma2(mr3, dz, a.az);
 }
 
 // Lane mapping of one pass over m <= 64 particles of a group (see file header):
-// lane = s * q + p, q = floor(32 / S); the lane's j-th particle is j * q + p.
+// lane = s * q + p, q = floor(32 / S); the lane's j-th particle is j * q + p, j < 2 kp.
 struct Lanes {
-  int S, q, k;   // warp-uniform
+  int S, q, kp;  // warp-uniform; kp = particle PAIRS per lane
   int s, p;      // this lane's slice and particle column
   bool active;   // lane < S * q
 };
 
 // Un-opened cells (List 3): slice s takes records s, s+S, s+2S, ...
-// Each record is loaded once and applied to the lane's K particles.
-template <int K>
+// Each record is loaded once and applied to the lane's KP particle pairs.
+template <int KP>
 __device__ __forceinline__ void eval_cells_k(const CellRec* __restrict__ rec, int cnt, float eps2, const Lanes& L,
-                                             const Pos (&P)[kMaxK], Acc (&A)[kMaxK]) {
+                                             const Pos2 (&P)[kMaxKP], Acc2 (&A)[kMaxKP]) {
   if (!L.active) return;
   const int st = L.S;
   int e = L.s;
@@ -164,39 +179,39 @@ __device__ __forceinline__ void eval_cells_k(const CellRec* __restrict__ rec, in
     const float4 a0 = r0->xm, b0 = r0->q0; const float2 c0 = r0->q1;
     const float4 a1 = r1->xm, b1 = r1->q0; const float2 c1 = r1->q1;
 #pragma unroll
-    for (int j = 0; j < K; j++) pc_interact(P[j], eps2, a0, b0, c0, A[j]);
+    for (int j = 0; j < KP; j++) pc_interact(P[j], eps2, a0, b0, c0, A[j]);
 #pragma unroll
-    for (int j = 0; j < K; j++) pc_interact(P[j], eps2, a1, b1, c1, A[j]);
+    for (int j = 0; j < KP; j++) pc_interact(P[j], eps2, a1, b1, c1, A[j]);
   }
   if (e < cnt) {
     const CellRec* r0 = rec + e;
     const float4 a0 = r0->xm, b0 = r0->q0; const float2 c0 = r0->q1;
 #pragma unroll
-    for (int j = 0; j < K; j++) pc_interact(P[j], eps2, a0, b0, c0, A[j]);
+    for (int j = 0; j < KP; j++) pc_interact(P[j], eps2, a0, b0, c0, A[j]);
   }
 }
 
-template <int K = 1>
+template <int KP = 1>
 __device__ __forceinline__ void eval_cells(const CellRec* rec, int cnt, float eps2, const Lanes& L,
-                                           const Pos (&P)[kMaxK], Acc (&A)[kMaxK]) {
-  if constexpr (K == kMaxK) {
-    eval_cells_k<K>(rec, cnt, eps2, L, P, A);
+                                           const Pos2 (&P)[kMaxKP], Acc2 (&A)[kMaxKP]) {
+  if constexpr (KP == kMaxKP) {
+    eval_cells_k<KP>(rec, cnt, eps2, L, P, A);
   } else {
-    if (L.k == K) eval_cells_k<K>(rec, cnt, eps2, L, P, A);   // warp-uniform
-    else eval_cells<K + 1>(rec, cnt, eps2, L, P, A);
+    if (L.kp == KP) eval_cells_k<KP>(rec, cnt, eps2, L, P, A);   // warp-uniform
+    else eval_cells<KP + 1>(rec, cnt, eps2, L, P, A);
   }
 }
 
-template <int K, bool kEps0>
+template <int KP, bool kEps0>
 __device__ __forceinline__ void eval_bodies_k(const float4* __restrict__ body, int cnt, float eps2, const Lanes& L,
-                                              const Pos (&P)[kMaxK], Acc (&A)[kMaxK]) {
+                                              const Pos2 (&P)[kMaxKP], Acc2 (&A)[kMaxKP]) {
   if (!L.active) return;
   const int st = L.S;
   int e = L.s;
   for (; e + 3 * st < cnt; e += 4 * st) {        // four bodies in flight
     const float4 b0 = body[e], b1 = body[e + st], b2 = body[e + 2 * st], b3 = body[e + 3 * st];
 #pragma unroll
-    for (int j = 0; j < K; j++) {
+    for (int j = 0; j < KP; j++) {
       pp_interact<kEps0>(P[j], eps2, b0, A[j]); pp_interact<kEps0>(P[j], eps2, b1, A[j]);
       pp_interact<kEps0>(P[j], eps2, b2, A[j]); pp_interact<kEps0>(P[j], eps2, b3, A[j]);
     }
@@ -204,18 +219,18 @@ __device__ __forceinline__ void eval_bodies_k(const float4* __restrict__ body, i
   for (; e < cnt; e += st) {
     const float4 b0 = body[e];
 #pragma unroll
-    for (int j = 0; j < K; j++) pp_interact<kEps0>(P[j], eps2, b0, A[j]);
+    for (int j = 0; j < KP; j++) pp_interact<kEps0>(P[j], eps2, b0, A[j]);
   }
 }
 
-template <bool kEps0, int K = 1>
+template <bool kEps0, int KP = 1>
 __device__ __forceinline__ void eval_bodies(const float4* body, int cnt, float eps2, const Lanes& L,
-                                            const Pos (&P)[kMaxK], Acc (&A)[kMaxK]) {
-  if constexpr (K == kMaxK) {
-    eval_bodies_k<K, kEps0>(body, cnt, eps2, L, P, A);
+                                            const Pos2 (&P)[kMaxKP], Acc2 (&A)[kMaxKP]) {
+  if constexpr (KP == kMaxKP) {
+    eval_bodies_k<KP, kEps0>(body, cnt, eps2, L, P, A);
   } else {
-    if (L.k == K) eval_bodies_k<K, kEps0>(body, cnt, eps2, L, P, A);
-    else eval_bodies<kEps0, K + 1>(body, cnt, eps2, L, P, A);
+    if (L.kp == KP) eval_bodies_k<KP, kEps0>(body, cnt, eps2, L, P, A);
+    else eval_bodies<kEps0, KP + 1>(body, cnt, eps2, L, P, A);
   }
 }
 
@@ -223,7 +238,7 @@ __device__ __forceinline__ void eval_bodies(const float4* body, int cnt, float e
 // body indices, gather the bodies with one coalesced float4 load per lane, evaluate.
 template <bool kEps0>
 __device__ __forceinline__ void eval_leaves(BodyStage& bs, const int2* leafq, int nq, const float4* __restrict__ part,
-                                            float eps2, const Lanes& L, const Pos (&P)[kMaxK], Acc (&A)[kMaxK],
+                                            float eps2, const Lanes& L, const Pos2 (&P)[kMaxKP], Acc2 (&A)[kMaxKP],
                                             int lane) {
   for (int r0 = 0; r0 < nq; r0 += 32) {
     int f = 0, n = 0;
@@ -284,19 +299,20 @@ forces_kernel(const float4* __restrict__ bnd, const float4* __restrict__ xm, con
       Lanes L;
       L.S = c_slices.S[m];
       L.q = 32 / L.S;
-      L.k = (m + L.q - 1) / L.q;
+      L.kp = (m + 2 * L.q - 1) / (2 * L.q);
       L.s = lane / L.q;
       L.p = lane - L.s * L.q;
       L.active = L.s < L.S;
-      Pos P[kMaxK];
-      Acc A[kMaxK];
+      Pos2 P[kMaxKP];
+      Acc2 A[kMaxKP];
 #pragma unroll
-      for (int j = 0; j < kMaxK; j++) {
-        A[j] = Acc{0.f, 0.f, 0.f, 0.f};
-        const int t = j * L.q + L.p;
+      for (int j = 0; j < kMaxKP; j++) {
+        A[j].ax = A[j].ay = A[j].az = A[j].npot = 0ull;  // (+0.f, +0.f)
         // slots beyond m compute on a copy of the pass's first particle; never written back
-        const float4 me = __ldg(part + G.y + pb + ((L.active && t < m) ? t : 0));
-        P[j].x = me.x; P[j].y = me.y; P[j].z = me.z;
+        const int t0 = 2 * j * L.q + L.p, t1 = t0 + L.q;
+        const float4 m0 = __ldg(part + G.y + pb + ((L.active && t0 < m) ? t0 : 0));
+        const float4 m1 = __ldg(part + G.y + pb + ((L.active && t1 < m) ? t1 : 0));
+        P[j].x = pk(m0.x, m1.x); P[j].y = pk(m0.y, m1.y); P[j].z = pk(m0.z, m1.z);
       }
 
       int ssz = 0, spill_sz = 0, ccnt = 0, lq = 0;
@@ -393,21 +409,24 @@ forces_kernel(const float4* __restrict__ bnd, const float4* __restrict__ xm, con
 
       // ---- A6: reduce the slices of every particle, write back in the caller's order
 #pragma unroll
-      for (int j = 0; j < kMaxK; j++) {
-        if (j >= L.k) break;                             // warp-uniform
-        Acc a = A[j];
+      for (int j = 0; j < 2 * kMaxKP; j++) {
+        if (j >= 2 * L.kp) break;                        // warp-uniform
+        const Acc2& a2 = A[j >> 1];
+        float ax, ay, az, ph;
+        if (j & 1) { ax = hi(a2.ax); ay = hi(a2.ay); az = hi(a2.az); ph = -hi(a2.npot); }
+        else { ax = lo(a2.ax); ay = lo(a2.ay); az = lo(a2.az); ph = -lo(a2.npot); }
         for (int w = 1; w < L.S; w <<= 1) {
-          const float ox = __shfl_down_sync(kFull, a.ax, w * L.q), oy = __shfl_down_sync(kFull, a.ay, w * L.q);
-          const float oz = __shfl_down_sync(kFull, a.az, w * L.q), op = __shfl_down_sync(kFull, a.pot, w * L.q);
-          if ((L.s % (2 * w)) == 0 && L.s + w < L.S) { a.ax += ox; a.ay += oy; a.az += oz; a.pot += op; }
+          const float ox = __shfl_down_sync(kFull, ax, w * L.q), oy = __shfl_down_sync(kFull, ay, w * L.q);
+          const float oz = __shfl_down_sync(kFull, az, w * L.q), op = __shfl_down_sync(kFull, ph, w * L.q);
+          if ((L.s % (2 * w)) == 0 && L.s + w < L.S) { ax += ox; ay += oy; az += oz; ph += op; }
         }
         const int tq = j * L.q + lane;
         if (lane < L.q && tq < m) {
           const int t = G.y + pb + tq;
           const int i = __ldg(orig + t);
-          if (!kEps0) a.pot += __ldg(part + t).w * rsqrt_approx(eps2);  // the particle met itself once
-          acc[3 * (size_t)i + 0] = a.ax; acc[3 * (size_t)i + 1] = a.ay; acc[3 * (size_t)i + 2] = a.az;
-          if (pot) pot[i] = a.pot;
+          if (!kEps0) ph += __ldg(part + t).w * rsqrt_approx(eps2);     // the particle met itself once
+          acc[3 * (size_t)i + 0] = ax; acc[3 * (size_t)i + 1] = ay; acc[3 * (size_t)i + 2] = az;
+          if (pot) pot[i] = ph;
           out_npc[i] = (int32_t)n_pc; out_npp[i] = (int32_t)(n_pp - 1);
         }
       }
