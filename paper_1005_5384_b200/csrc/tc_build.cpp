@@ -345,15 +345,15 @@ int build_host_tree(const float* pos, const float* mass, int64_t n, int n_leaf, 
   // Schedule (grp[i].w = i-th group to run): the persistent kernel hands groups out through an
   // atomic counter, so costly groups go first and the tail of the launch is made of cheap ones.
   // Cost model = issue slots per list entry of the kernel's lane mapping (tc_kernels.cu): a pass
-  // over m <= 64 particles costs min_S ceil(m / floor(32/S)) / S.  Stable: Morton order inside a
+  // over m <= 64 particles costs min_S ceil(m / (2 floor(32/S))) / S (particle pairs per lane / slices).  Stable: Morton order inside a
   // cost class keeps neighbouring groups together.
   {
     double pass_cost[65];
     for (int m = 0; m <= 64; m++) {
       double best = 1e30;
       for (int sl = 1; sl <= 32; sl++) {
-        const int q = 32 / sl, k = (m + q - 1) / q;
-        if (k >= 1 && k <= 4) best = std::min(best, (double)((k + 1) / 2) / sl);   // pairs of particles per lane
+        const int q = 32 / sl, kp = (m + 2 * q - 1) / (2 * q);                     // pairs of particles per lane
+        if (kp >= 1 && kp <= 3) best = std::min(best, (double)kp / sl);
       }
       pass_cost[m] = (m == 0) ? 0.0 : best;
     }

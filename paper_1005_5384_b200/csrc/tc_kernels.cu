@@ -15,12 +15,13 @@
 //   * a chunk is evaluated as soon as it fills (FP32 FMA + one rsqrt.approx per
 //     interaction), so no interaction list ever reaches global memory and there is
 //     no count pass, no host scan, no second walk;
-//   * lanes map to (list slice s, particle p): a pass over m <= 64 particles picks
-//     S slices and k = ceil(m / floor(32/S)) <= 4 particles per lane so that k/S is
-//     minimal; every list record is loaded from shared memory once per lane and
-//     applied to the lane's k particles (register blocking), slices are reduced with
-//     shuffles at the end — the fix for the paper's 30 % thread utilisation
-//     (PAPER.md:175).
+//   * lanes map to (list slice s, particle column p): a pass over m <= 64 particles
+//     picks S slices of q = floor(32/S) columns and kp = ceil(m / 2q) <= 3 particle
+//     PAIRS per lane so that kp/S is minimal; every list record is loaded from shared
+//     memory once per lane and applied to the lane's pairs with packed FP32
+//     instructions (FFMA2/FMUL2/FADD2: two particles per instruction), slices are
+//     reduced with shuffles at the end — the fix for the paper's 30 % thread
+//     utilisation.
 // No tensor cores: this is not a dense contraction.
 #include <cuda_runtime.h>
 
@@ -32,15 +33,18 @@ namespace tc {
 namespace {
 
 #ifndef TC_MAXKP
-#define TC_MAXKP 2
+#define TC_MAXKP 3
 #endif
 #ifndef TC_MINB
-#define TC_MINB 3
+#define TC_MINB 5
 #endif
 #ifndef TC_CELLCAP
 #define TC_CELLCAP 96
 #endif
-constexpr int kWarpsPerCta = 8;
+#ifndef TC_WARPS
+#define TC_WARPS 4
+#endif
+constexpr int kWarpsPerCta = TC_WARPS;
 constexpr int kCellCap = TC_CELLCAP;  // un-opened cells staged per warp before evaluation
 constexpr int kLeafQCap = 128;   // opened-leaf ranges queued per warp
 constexpr int kBodyCap = 128;    // bodies staged per warp per evaluation round
@@ -100,6 +104,8 @@ __device__ __forceinline__ float rsqrt_approx(float x) {
 // A scalar operand (a field of the list record) is broadcast by the hardware (`R.F32` operand form).
 typedef unsigned long long f2;
 __device__ __forceinline__ f2 pk(float lo, float hi) { f2 r; asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(lo), "f"(hi)); return r; }
+// same, but pinned where it is written: the pair is built once and lives in an aligned register pair
+__device__ __forceinline__ f2 pk_keep(float lo, float hi) { f2 r; asm volatile("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(lo), "f"(hi)); return r; }
 __device__ __forceinline__ f2 bc(float x) { return pk(x, x); }
 __device__ __forceinline__ float lo(f2 v) { float a, b; asm("mov.b64 {%0, %1}, %2;" : "=f"(a), "=f"(b) : "l"(v)); return a; }
 __device__ __forceinline__ float hi(f2 v) { float a, b; asm("mov.b64 {%0, %1}, %2;" : "=f"(a), "=f"(b) : "l"(v)); return b; }
@@ -312,7 +318,7 @@ forces_kernel(const float4* __restrict__ bnd, const float4* __restrict__ xm, con
         const int t0 = 2 * j * L.q + L.p, t1 = t0 + L.q;
         const float4 m0 = __ldg(part + G.y + pb + ((L.active && t0 < m) ? t0 : 0));
         const float4 m1 = __ldg(part + G.y + pb + ((L.active && t1 < m) ? t1 : 0));
-        P[j].x = pk(m0.x, m1.x); P[j].y = pk(m0.y, m1.y); P[j].z = pk(m0.z, m1.z);
+        P[j].x = pk_keep(m0.x, m1.x); P[j].y = pk_keep(m0.y, m1.y); P[j].z = pk_keep(m0.z, m1.z);
       }
 
       int ssz = 0, spill_sz = 0, ccnt = 0, lq = 0;
