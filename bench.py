@@ -46,6 +46,8 @@ PAPER_FLOPS_PC, PAPER_FLOPS_PP = 70, 38
 # FP32 ALU peak: SMs x 128 lanes x 2 flops x clock
 N_SM, LANES = 148, 128
 L2_FLUSH_BYTES = 256 << 20        # > 126 MB L2
+# DRAM bytes of one launch of the force kernel at config 3, from the committed ncu capture (profiles/)
+DRAM_TRAFFIC_BYTES = 67400704
 
 
 def fp32_peak_tflops(mhz: float) -> float:
@@ -236,6 +238,7 @@ def run_ours(args) -> None:
                 t_host.append(s2["t_host_ms"]); t_copy.append(s2["t_copy_ms"])
         e2e_s = float(np.mean(t_e2e))
         tree_bytes = st["tree_bytes"]
+        measured_peak = B.tc_fp32_peak(tc.ctx)       # FFMA-only microbenchmark on this device, after the timed region
     tc.close()
 
     t_dev_ms = max_over_ranks(t_dev_ms, world, dev)
@@ -279,11 +282,14 @@ def run_ours(args) -> None:
                 "t_host_build_ms": float(np.mean(t_host)), "t_copy_ms": float(np.mean(t_copy)),
                 "what": "tc_set_particles(host)+tc_build(host octree, one bulk H2D)+tc_forces(host acc,pot); wall clock"},
         "roofline": {"bound": "alu", "achieved": ach, "peak": peak, "unit": "TFLOP/s", "frac": ach / peak,
-                     "traffic": None, "kernel": "tc::forces_kernel",
-                     "peak_how": f"{N_SM} SMs x {LANES} FP32 lanes x 2 x {sm_max:.0f} MHz (nominal max clock; "
-                                 "MEASURED_PEAKS.json has no FP32 entry — DESIGN.md §6)",
-                     "flops_per_launch": flops,
-                     "frac_at_sampled_clock": (ach / fp32_peak_tflops(clocks["sm_mhz"])) if clocks.get("sm_mhz") else None},
+                     "traffic": DRAM_TRAFFIC_BYTES, "kernel": "tc::forces_kernel",
+                     "peak_how": f"nominal: {N_SM} SMs x {LANES} FP32 lanes x 2 x {sm_max:.0f} MHz (DESIGN.md §6; "
+                                 "MEASURED_PEAKS.json holds HBM and bf16 figures only, no FP32 entry)",
+                     "peak_measured": measured_peak, "frac_of_measured": ach / measured_peak,
+                     "peak_measured_how": "tc_fp32_peak: FFMA-only microbenchmark on this device in this run",
+                     "flops_per_launch": flops, "algorithmic_bytes_per_launch": int(tree_bytes + 24 * n),
+                     "traffic_how": "dram__bytes_read.sum + dram__bytes_write.sum of one ncu --set full capture "
+                                    "(profiles/r01_forces_kernel.md); HBM is not the bound"},
     }
     out["cpu_baseline"] = cpu_baseline(*inputs.make(WORKLOAD)) if world == 1 else None
     print(json.dumps(out), flush=True)

@@ -142,6 +142,14 @@ const char* tc_last_error(const tc_ctx* ctx);
 int tc_get_tree(tc_ctx* ctx, int32_t* perm, float* cell_bnd, float* cell_xm, float* cell_q,
                 int32_t* cell_link, int32_t* groups);
 
+/* Measured FP32 peak of the current device: an FFMA-only microbenchmark (16 independent
+ * fma.rn.f32 chains per thread, 8 CTAs of 256 threads per SM, CUDA events on the context's
+ * stream).  *tflops = 2 flops x FFMA lane-instructions / time.  This is the denominator the
+ * roofline of bench.py quotes beside the nominal SMs x 128 lanes x 2 x clock: the
+ * force kernel is bound by FP32 issue, not by HBM or tensor throughput (PAPER.md:175 measures
+ * "instruction throughput" the same way).  Errors: TC_ESTATE (host-only), TC_EINVAL, TC_ECUDA.  */
+int tc_fp32_peak(tc_ctx* ctx, double* tflops);
+
 #ifdef __cplusplus
 }
 #endif

@@ -26,7 +26,7 @@ TC_FLAG_HOST_ONLY = 1
 #: every symbol include/tc.h declares (checked by tests/test_abi.py)
 SYMBOLS = ["tc_create", "tc_create_ex", "tc_destroy", "tc_set_particles", "tc_build", "tc_forces",
            "tc_set_option", "tc_get_counts", "tc_get_stats", "tc_set_stream", "tc_sync",
-           "tc_last_error", "tc_get_tree"]
+           "tc_last_error", "tc_get_tree", "tc_fp32_peak"]
 
 
 class tc_stats(C.Structure):
@@ -76,6 +76,7 @@ def lib():
     L.tc_last_error.restype = C.c_char_p
     L.tc_last_error.argtypes = [vp]
     L.tc_get_tree.argtypes = [vp] + [vp] * 6
+    L.tc_fp32_peak.argtypes = [vp, C.POINTER(C.c_double)]
     _lib = L
     return L
 
@@ -155,6 +156,13 @@ def tc_get_tree(ctx) -> dict:
                q=np.zeros((nc, 6), np.float32), link=np.zeros((nc, 4), np.int32), groups=np.zeros(ng, np.int32))
     _check(ctx, lib().tc_get_tree(ctx, *[_ptr(out[k]) for k in ("perm", "bnd", "xm", "q", "link", "groups")]))
     return out
+
+
+def tc_fp32_peak(ctx) -> float:
+    """Measured FFMA-only FP32 throughput of the current device in TFLOP/s."""
+    v = C.c_double(0.0)
+    _check(ctx, lib().tc_fp32_peak(ctx, C.byref(v)))
+    return float(v.value)
 
 
 class TreeCode:

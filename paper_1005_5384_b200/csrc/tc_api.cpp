@@ -308,6 +308,14 @@ int tc_get_stats(tc_ctx* c, tc_stats* out) {
   return rc;
 }
 
+int tc_fp32_peak(tc_ctx* c, double* tflops) {
+  if (!c || !tflops) return fail(c, TC_EINVAL, "tc_fp32_peak: null argument");
+  if (c->host_only) return fail(c, TC_ESTATE, "tc_fp32_peak: host-only context has no device");
+  const int e = tc::measure_fp32_peak(c->n_sm, c->stream, tflops);
+  if (e != 0) return cuda_fail(c, (cudaError_t)e, "fp32 peak microbenchmark");
+  return TC_OK;
+}
+
 int tc_get_tree(tc_ctx* c, int32_t* perm, float* cell_bnd, float* cell_xm, float* cell_q, int32_t* cell_link,
                 int32_t* groups) {
   if (!c) return TC_EINVAL;

@@ -92,5 +92,7 @@ struct ForceLaunch {
 int launch_forces(const DeviceTree& T, const ForceLaunch& L, void* stream);
 // Number of warps the persistent grid runs (for sizing the spill buffer).
 int forces_total_warps(int n_sm, int stack_smem);
+// FFMA-only microbenchmark (tc_fp32_peak): returns a cudaError_t as int, *tflops on success.
+int measure_fp32_peak(int n_sm, void* stream, double* tflops);
 
 }  // namespace tc

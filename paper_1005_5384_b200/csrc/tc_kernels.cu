@@ -479,6 +479,49 @@ int launch_forces(const DeviceTree& T, const ForceLaunch& L, void* stream) {
   return dispatch(T, L, (cudaStream_t)stream, nullptr);
 }
 
+// ---- tc_fp32_peak: what the FP32 pipe of this device sustains with nothing but FFMA in flight
+namespace {
+__global__ void __launch_bounds__(256) ffma_peak_kernel(float* out, int n, float s) {
+  float a[16];
+#pragma unroll
+  for (int i = 0; i < 16; i++) a[i] = threadIdx.x * 0.001f + i;
+  const float b = s, c = 1.f - s;
+  for (int t = 0; t < n; t++) {
+#pragma unroll
+    for (int i = 0; i < 16; i++) asm volatile("fma.rn.f32 %0, %0, %1, %2;" : "+f"(a[i]) : "f"(b), "f"(c));
+  }
+  float r = 0.f;
+#pragma unroll
+  for (int i = 0; i < 16; i++) r += a[i];
+  out[blockIdx.x * blockDim.x + threadIdx.x] = r;
+}
+}  // namespace
+
+int measure_fp32_peak(int n_sm, void* stream, double* tflops) {
+  cudaStream_t st = (cudaStream_t)stream;
+  const int grid = n_sm * 8, n = 20000;
+  float* d = nullptr;
+  cudaError_t e = cudaMalloc((void**)&d, sizeof(float) * (size_t)grid * 256);
+  if (e != cudaSuccess) return (int)e;
+  cudaEvent_t e0 = nullptr, e1 = nullptr;
+  cudaEventCreate(&e0); cudaEventCreate(&e1);
+  float best = 0.f;
+  ffma_peak_kernel<<<grid, 256, 0, st>>>(d, 200, 0.999f);          // warm-up
+  for (int rep = 0; rep < 3 && e == cudaSuccess; rep++) {
+    cudaEventRecord(e0, st);
+    ffma_peak_kernel<<<grid, 256, 0, st>>>(d, n, 0.999f);
+    cudaEventRecord(e1, st);
+    e = cudaEventSynchronize(e1);
+    float ms = 0.f;
+    if (e == cudaSuccess) e = cudaEventElapsedTime(&ms, e0, e1);
+    if (e == cudaSuccess && (best == 0.f || ms < best)) best = ms;
+  }
+  cudaEventDestroy(e0); cudaEventDestroy(e1); cudaFree(d);
+  if (e != cudaSuccess) return (int)e;
+  *tflops = 2.0 * 16.0 * (double)n * (double)grid * 256.0 / ((double)best * 1e-3) / 1e12;
+  return 0;
+}
+
 int forces_total_warps(int n_sm, int stack_smem) {
   DeviceTree T;
   ForceLaunch L;

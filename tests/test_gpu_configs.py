@@ -1,0 +1,125 @@
+"""BASELINE.json configs 4 and 5 at FULL size on the GPU — `-m gpu`.
+
+Config 4: Plummer N = 2^20, theta in {0.3, 0.5, 0.75, 1.0} x N_leaf in {8, 16, 32}: rms relative force
+error against fp64 direct summation on 4096 sampled particles versus time.
+Config 5: two offset Plummer spheres, N = 2^24, eps = 0.005: oracle parity on sampled groups, then 10
+leapfrog KDK steps with a host tree rebuild each step (energy and momentum conservation).
+The tables are printed (run with -s) and written to gpurun_out/ when that directory exists.
+"""
+import json
+import os
+
+import numpy as np
+import pytest
+
+from oracle import Oracle, direct
+from paper_1005_5384_b200 import binding as B
+from paper_1005_5384_b200 import build as tc_build
+from paper_1005_5384_b200 import inputs
+from test_gpu_parity import check, rel_err
+
+pytestmark = pytest.mark.gpu
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+@pytest.fixture(scope="module", autouse=True)
+def _built():
+    tc_build.build()
+
+
+def _dump(name, obj):
+    d = os.path.join(ROOT, "gpurun_out")
+    if os.path.isdir(d):
+        with open(os.path.join(d, name), "w") as f:
+            json.dump(obj, f, indent=1)
+
+
+def test_config4_accuracy_versus_time_1m():
+    import torch
+    pos, mass, _, eps, _ = inputs.make("plummer_1m")
+    n = len(mass)
+    tg = inputs.sample_targets(n, 4096, seed=4)
+    dacc, _ = direct(pos, mass, eps, targets=tg)          # fp64 direct sum over all N
+    rows = []
+    st = torch.cuda.Stream()
+    with torch.cuda.stream(st):
+        d_acc = torch.empty((n, 3), dtype=torch.float32, device="cuda")
+        d_pot = torch.empty(n, dtype=torch.float32, device="cuda")
+        for n_leaf in (8, 16, 32):
+            with B.TreeCode(n_group=64) as tc:
+                tc.set_stream(st.cuda_stream)
+                tc.set_particles(pos, mass)
+                tc.build(n_leaf)
+                for theta in (0.3, 0.5, 0.75, 1.0):
+                    ts = []
+                    for _ in range(4):
+                        B.tc_forces(tc.ctx, theta, eps, d_acc, d_pot)
+                        tc.sync()
+                        ts.append(tc.stats()["t_gpu_ms"])
+                    s = tc.stats()
+                    e = rel_err(d_acc[torch.from_numpy(tg).cuda()].cpu().numpy().astype(np.float64), dacc)
+                    rows.append(dict(n_leaf=n_leaf, theta=theta, ms=float(np.median(ts[1:])),
+                                     rms=float(np.sqrt((e ** 2).mean())), median=float(np.median(e)),
+                                     p99=float(np.quantile(e, 0.99)), n_pc=s["n_pc_total"] / n, n_pp=s["n_pp_total"] / n))
+    for r in rows:
+        print("config4 N_leaf={n_leaf:2d} theta={theta:4.2f}: {ms:7.3f} ms  rms={rms:.3e} median={median:.3e} "
+              "p99={p99:.3e}  p-c/particle={n_pc:7.0f} p-p/particle={n_pp:6.0f}".format(**r))
+    _dump("config4_sweep.json", rows)
+    for n_leaf in (8, 16, 32):
+        rr = [r for r in rows if r["n_leaf"] == n_leaf]
+        # error rises steeply with theta (~theta^4), time falls
+        assert all(a["rms"] < b["rms"] for a, b in zip(rr, rr[1:]))
+        assert all(a["ms"] > b["ms"] for a, b in zip(rr, rr[1:]))
+        assert rr[0]["median"] * 4 < rr[1]["median"]                 # 0.3 -> 0.5: at least (5/3)^3
+    r05 = [r for r in rows if r["n_leaf"] == 16 and r["theta"] == 0.5][0]
+    assert 2e-5 < r05["median"] < 4e-4                               # SURVEY 8(c) sanity band around 8.7e-5
+    # one oracle parity point away from the headline parameters, sampled groups
+    o = Oracle(pos, mass, 8, 64)
+    gsel = np.arange(7, o.n_groups, o.n_groups // 192, dtype=np.int64)
+    ref = o.forces(0.3, eps, shadow32=True, groups=gsel)
+    with B.TreeCode(n_group=64) as tc:
+        tc.set_particles(pos, mass)
+        tc.build(8)
+        acc, pot = tc.forces(0.3, eps)
+        n_pc, n_pp = tc.counts()
+    check(acc, pot, n_pc, n_pp, ref, ref["n_pc"] >= 0)
+
+
+def test_config5_two_plummer_16m_parity_and_leapfrog():
+    import torch
+    from paper_1005_5384_b200 import integrate
+    n, theta, eps, n_leaf, dt, steps = 1 << 24, 0.5, 0.005, 16, 1.0 / 128, 10
+    pos, mass, vel = inputs.two_plummer(n, with_velocities=True)
+    st = torch.cuda.Stream()
+    with torch.cuda.stream(st), B.TreeCode(n_group=64) as tc:
+        tc.set_stream(st.cuda_stream)
+        d_pos, d_vel, d_mass = torch.from_numpy(pos).cuda(), torch.from_numpy(vel).cuda(), torch.from_numpy(mass).cuda()
+        # ---- parity at step 0 on sampled groups (full size, the configuration the loop runs)
+        d_acc = torch.empty((n, 3), dtype=torch.float32, device="cuda")
+        d_pot = torch.empty(n, dtype=torch.float32, device="cuda")
+        tc.set_particles(d_pos, d_mass)
+        tc.build(n_leaf)
+        B.tc_forces(tc.ctx, theta, eps, d_acc, d_pot)
+        tc.sync()
+        s0 = tc.stats()
+        n_pc, n_pp = tc.counts()
+        o = Oracle(pos, mass, n_leaf, 64)
+        assert (s0["n_cells"], s0["n_leaves"], s0["n_groups"], s0["depth"]) == (o.n_cells, o.n_leaves, o.n_groups, o.depth)
+        gsel = np.sort(np.random.default_rng(5).choice(o.n_groups, 256, replace=False)).astype(np.int64)
+        ref = o.forces(theta, eps, shadow32=True, groups=gsel)
+        del o
+        check(d_acc.cpu().numpy(), d_pot.cpu().numpy(), n_pc, n_pp, ref, ref["n_pc"] >= 0)
+        print(f"config5 step 0: cells={s0['n_cells']} groups={s0['n_groups']} T_host={s0['t_host_ms']:.0f} ms "
+              f"T_copy={s0['t_copy_ms']:.1f} ms T_gpu={s0['t_gpu_ms']:.1f} ms interactions={s0['n_pc_total'] + s0['n_pp_total']:.3e}")
+        # ---- 10 KDK steps, host tree rebuild each step
+        log = integrate.leapfrog_kdk(tc, d_pos, d_vel, d_mass, dt, steps, theta, eps, n_leaf,
+                                     log=lambda r: print("config5 step {step:2d}: T_host={t_host_ms:6.0f} ms T_copy={t_copy_ms:5.1f} ms "
+                                                         "T_gpu={t_gpu_ms:6.1f} ms wall={wall_ms:6.0f} ms dE/E={dE_rel:.2e} |dP|={dP:.2e}".format(**r)))
+        _dump("config5_leapfrog.json", log)
+        assert len(log) == steps + 1
+        assert max(r["dE_rel"] for r in log) < 2e-4          # tree-force + leapfrog energy error over 10 steps
+        assert max(r["dP"] for r in log) < 1e-4              # total momentum (tree forces are not exactly symmetric)
+        # the spheres approach: separation of the two centres of mass shrinks by ~ 0.5 * 10/128
+        n1 = (3 * n) // 4
+        x1 = float(d_pos[:n1, 0].double().mean()); x2 = float(d_pos[n1:, 0].double().mean())
+        assert 6.0 - 0.06 < (x2 - x1) < 6.0 - 0.02
