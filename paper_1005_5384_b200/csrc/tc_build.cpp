@@ -13,6 +13,7 @@
 // bbox -> boundary cube, mass, COM, traceless quadrupole, O4 groups.
 #include <algorithm>
 #include <cmath>
+#include <cstdlib>
 #include <cstring>
 #include <limits>
 

@@ -104,8 +104,6 @@ __device__ __forceinline__ float rsqrt_approx(float x) {
 // A scalar operand (a field of the list record) is broadcast by the hardware (`R.F32` operand form).
 typedef unsigned long long f2;
 __device__ __forceinline__ f2 pk(float lo, float hi) { f2 r; asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(lo), "f"(hi)); return r; }
-// same, but pinned where it is written: the pair is built once and lives in an aligned register pair
-__device__ __forceinline__ f2 pk_keep(float lo, float hi) { f2 r; asm volatile("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(lo), "f"(hi)); return r; }
 __device__ __forceinline__ f2 bc(float x) { return pk(x, x); }
 __device__ __forceinline__ float lo(f2 v) { float a, b; asm("mov.b64 {%0, %1}, %2;" : "=f"(a), "=f"(b) : "l"(v)); return a; }
 __device__ __forceinline__ float hi(f2 v) { float a, b; asm("mov.b64 {%0, %1}, %2;" : "=f"(a), "=f"(b) : "l"(v)); return b; }
@@ -318,7 +316,10 @@ forces_kernel(const float4* __restrict__ bnd, const float4* __restrict__ xm, con
         const int t0 = 2 * j * L.q + L.p, t1 = t0 + L.q;
         const float4 m0 = __ldg(part + G.y + pb + ((L.active && t0 < m) ? t0 : 0));
         const float4 m1 = __ldg(part + G.y + pb + ((L.active && t1 < m) ? t1 : 0));
-        P[j].x = pk_keep(m0.x, m1.x); P[j].y = pk_keep(m0.y, m1.y); P[j].z = pk_keep(m0.z, m1.z);
+        // (+ 0 through FADD2: the pair is then the result of a real instruction and stays in one aligned
+        // register pair; a bare mov.b64 is re-materialised with two MOVs in front of every use)
+        P[j].x = add2(pk(m0.x, m1.x), bc(0.f)); P[j].y = add2(pk(m0.y, m1.y), bc(0.f));
+        P[j].z = add2(pk(m0.z, m1.z), bc(0.f));
       }
 
       int ssz = 0, spill_sz = 0, ccnt = 0, lq = 0;
