@@ -349,19 +349,20 @@ int build_host_tree(const float* pos, const float* mass, int64_t n, int n_leaf, 
   // over m <= 64 particles costs min_S ceil(m / (2 floor(32/S))) / S (particle pairs per lane / slices).  Stable: Morton order inside a
   // cost class keeps neighbouring groups together.
   {
-    double pass_cost[65];
-    for (int m = 0; m <= 64; m++) {
+    constexpr int kPass = 64, kMaxKP = 3;        // mirror of tc_kernels.cu
+    double pass_cost[kPass + 1];
+    for (int m = 0; m <= kPass; m++) {
       double best = 1e30;
       for (int sl = 1; sl <= 32; sl++) {
         const int q = 32 / sl, kp = (m + 2 * q - 1) / (2 * q);                     // pairs of particles per lane
-        if (kp >= 1 && kp <= 3) best = std::min(best, (double)kp / sl);
+        if (kp >= 1 && kp <= kMaxKP) best = std::min(best, (double)kp / sl);
       }
       pass_cost[m] = (m == 0) ? 0.0 : best;
     }
     std::vector<std::pair<float, int32_t>> order(groups.size());
     for (size_t g = 0; g < groups.size(); g++) {
       const int64_t cnt = c_count[groups[g]];
-      const double cost = (double)(cnt / 64) * pass_cost[64] + pass_cost[cnt % 64];
+      const double cost = (double)(cnt / kPass) * pass_cost[kPass] + pass_cost[cnt % kPass];
       order[g] = std::make_pair((float)-cost, (int32_t)g);
     }
     std::stable_sort(order.begin(), order.end(),

@@ -49,7 +49,10 @@ constexpr int kCellCap = TC_CELLCAP;  // un-opened cells staged per warp before 
 constexpr int kLeafQCap = 128;   // opened-leaf ranges queued per warp
 constexpr int kBodyCap = 128;    // bodies staged per warp per evaluation round
 constexpr int kMaxKP = TC_MAXKP; // particle PAIRS per lane (packed f32x2 arithmetic)
-constexpr int kPass = 64;        // particles of a group handled per walk
+// Particles of a group handled per walk.  64 * kMaxKP would fit, but splitting a larger group into
+// passes of 64 keeps the lanes fuller (96 = 64 + 32 costs 1 + 1/2 pair-slots, one pass of 96 costs 2)
+// and measured faster although the tree is walked once per pass.
+constexpr int kPass = 64;
 constexpr unsigned kFull = 0xffffffffu;
 
 struct __align__(16) CellRec {   // one un-opened cell: 48 bytes
@@ -161,7 +164,7 @@ __device__ __forceinline__ void pp_interact(const Pos2& p, float eps2, const flo
   a.ax = fma2(mr3, dx, a.ax); a.ay = fma2(mr3, dy, a.ay); a.az = fma2(mr3, dz, a.az);
 }
 
-// Lane mapping of one pass over m <= 64 particles of a group (see file header):
+// Lane mapping of one pass over m <= kPass particles of a group (see file header):
 // lane = s * q + p, q = floor(32 / S); the lane's j-th particle is j * q + p, j < 2 kp.
 struct Lanes {
   int S, q, kp;  // warp-uniform; kp = particle PAIRS per lane
@@ -297,7 +300,7 @@ forces_kernel(const float4* __restrict__ bnd, const float4* __restrict__ xm, con
     const float4 gb = __ldg(bnd + G.x);
     const float gbx = gb.x, gby = gb.y, gbz = gb.z, gh = fabsf(gb.w);
 
-    // groups larger than 64 particles (level-21 leaves, or N_group > 64) repeat the walk per 64
+    // groups larger than kPass particles (level-21 leaves, or a large N_group) repeat the walk per kPass
     for (int pb = 0; pb < G.z; pb += kPass) {
       const int m = min(kPass, G.z - pb);
       Lanes L;
