@@ -86,7 +86,7 @@ int tc_set_particles(tc_ctx* ctx, const float* pos, const float* mass, int64_t n
 
 /* Host octree: root cube, recursive 8-way split until a cell
  * holds <= n_leaf particles (or level 21), tight bounding boxes, boundary cubes,
- * fp64 moments rounded to fp32, groups (N_group from tc_set_option, default 64),
+ * fp64 moments rounded to fp32, groups (N_group from tc_set_option, default 96),
  * SoA float4 packing, one bulk host->device copy.
  * Errors: TC_ESTATE (no particles), TC_EINVAL (n_leaf < 1), TC_ENOMEM, TC_ECUDA. */
 int tc_build(tc_ctx* ctx, int n_leaf);

@@ -23,7 +23,7 @@ struct tc_ctx {
   cudaEvent_t ev0 = nullptr, ev1 = nullptr;
   std::string err;
   // options
-  int n_group = 64;
+  int n_group = 96;
   int stack_smem = 256;
   // particles (host copy, caller order)
   std::vector<float> pos, mass;

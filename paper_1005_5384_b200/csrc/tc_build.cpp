@@ -13,9 +13,12 @@
 // bbox -> boundary cube, mass, COM, traceless quadrupole, O4 groups.
 #include <algorithm>
 #include <cmath>
+#include <cstdio>
 #include <cstdlib>
 #include <cstring>
 #include <limits>
+#include <memory>
+#include <new>
 
 #ifdef _OPENMP
 #include <omp.h>
@@ -41,19 +44,26 @@ struct KeyIdx {
   uint32_t idx;
 };
 
-// Stable LSD radix sort of (key, idx) by key, 11-bit digits, OpenMP.
-void radix_sort(std::vector<KeyIdx>& a, std::vector<KeyIdx>& tmp, uint64_t key_or) {
-  const int64_t n = (int64_t)a.size();
-  constexpr int BITS = 11, R = 1 << BITS;
+// Sort of (key, idx) by key, stable (equal keys keep ascending idx).  Three LSD radix passes of 13
+// bits order the keys by their top 39 bits (13 tree levels); a run of equal 39-bit prefixes only needs
+// its low 24 bits ordered when it is longer than `n_leaf` (it is then split below level 13), which is
+// rare — those runs are finished with std::stable_sort.  Shorter runs end up inside one leaf, where the
+// order of the members is immaterial (it stays the caller's order).
+void radix_sort(KeyIdx* a, KeyIdx* tmp, int64_t n, uint64_t key_or, int n_leaf) {
+  constexpr int BITS = 13, R = 1 << BITS, LOW = 63 - 3 * BITS;
+  if (n < 8192) {   // small inputs: the histograms would cost more than the sort
+    std::stable_sort(a, a + n, [](const KeyIdx& x, const KeyIdx& y) { return x.key < y.key; });
+    return;
+  }
   int nthreads = 1;
 #ifdef _OPENMP
   nthreads = omp_get_max_threads();
 #endif
   if (n < (1 << 16)) nthreads = 1;
   std::vector<int64_t> hist((size_t)nthreads * R);
-  KeyIdx* src = a.data();
-  KeyIdx* dst = tmp.data();
-  for (int shift = 0; shift < 63; shift += BITS) {
+  KeyIdx* src = a;
+  KeyIdx* dst = tmp;
+  for (int shift = LOW; shift < 63; shift += BITS) {
     if (((key_or >> shift) & (R - 1)) == 0) continue;  // digit is zero in every key
     std::fill(hist.begin(), hist.end(), 0);
 #pragma omp parallel num_threads(nthreads)
@@ -81,7 +91,18 @@ void radix_sort(std::vector<KeyIdx>& a, std::vector<KeyIdx>& tmp, uint64_t key_o
     }
     std::swap(src, dst);
   }
-  if (src != a.data()) std::memcpy(a.data(), src, sizeof(KeyIdx) * (size_t)n);
+  if (src != a) std::memcpy(a, src, sizeof(KeyIdx) * (size_t)n);
+  // finish the long runs (parallel over run starts; runs are disjoint)
+#pragma omp parallel for schedule(dynamic, 65536)
+  for (int64_t i = 0; i < n; i++) {
+    const uint64_t pre = a[i].key >> LOW;
+    if (i > 0 && (a[i - 1].key >> LOW) == pre) continue;      // not a run start
+    int64_t j = i + 1;
+    while (j < n && j - i <= n_leaf && (a[j].key >> LOW) == pre) j++;
+    if (j - i <= n_leaf) continue;
+    while (j < n && (a[j].key >> LOW) == pre) j++;
+    std::stable_sort(a + i, a + j, [](const KeyIdx& x, const KeyIdx& y) { return x.key < y.key; });
+  }
 }
 
 struct CellProp {   // fp64 moments, fp32-exact bounding box
@@ -97,15 +118,24 @@ int build_host_tree(const float* pos, const float* mass, int64_t n, int n_leaf, 
                     HostTree& T, PackedAlloc alloc, void* alloc_user, std::string& msg) {
   if (n < 1 || n_leaf < 1 || n_group < 1) { msg = "build: n, n_leaf, n_group must be >= 1"; return TC_EINVAL; }
   T.n = n; T.n_leaf = n_leaf; T.n_group = n_group;
+  const bool timing = std::getenv("TC_BUILD_TIMING") != nullptr;
+  double t_prev = omp_get_wtime();
+  auto lap = [&](const char* what) { if (timing) { const double t = omp_get_wtime(); std::fprintf(stderr, "[tc_build] %-10s %8.3f ms\n", what, (t - t_prev) * 1e3); t_prev = t; } };
 
   // ---- O1: root cube and integer grid ("a cube containing all particles")
   double lo[3], hi[3];
   for (int k = 0; k < 3; k++) { lo[k] = std::numeric_limits<double>::infinity(); hi[k] = -lo[k]; }
-  for (int64_t i = 0; i < n; i++)
-    for (int k = 0; k < 3; k++) {
-      const double v = (double)pos[3 * i + k];
-      lo[k] = std::min(lo[k], v); hi[k] = std::max(hi[k], v);
+  {
+    double l0 = lo[0], l1 = lo[1], l2 = lo[2], h0 = hi[0], h1 = hi[1], h2 = hi[2];
+#pragma omp parallel for schedule(static) reduction(min : l0, l1, l2) reduction(max : h0, h1, h2)
+    for (int64_t i = 0; i < n; i++) {
+      const double x = (double)pos[3 * i], y = (double)pos[3 * i + 1], z = (double)pos[3 * i + 2];
+      l0 = std::min(l0, x); h0 = std::max(h0, x);
+      l1 = std::min(l1, y); h1 = std::max(h1, y);
+      l2 = std::min(l2, z); h2 = std::max(h2, z);
     }
+    lo[0] = l0; lo[1] = l1; lo[2] = l2; hi[0] = h0; hi[1] = h1; hi[2] = h2;
+  }
   double ext = 0.0;
   for (int k = 0; k < 3; k++) ext = std::max(ext, hi[k] - lo[k]);
   double side = ext * (1.0 + std::ldexp(1.0, -20));
@@ -115,8 +145,10 @@ int build_host_tree(const float* pos, const float* mass, int64_t n, int n_leaf, 
   const double scale = std::ldexp(1.0, 21) / side;
   const double gmax = std::ldexp(1.0, 21) - 1.0;
 
-  std::vector<KeyIdx> keys, tmp;
-  try { keys.resize((size_t)n); tmp.resize((size_t)n); } catch (...) { msg = "build: out of host memory"; return TC_ENOMEM; }
+  // key buffers: plain arrays (no zero fill; every element is written below)
+  std::unique_ptr<KeyIdx[]> keys_buf(new (std::nothrow) KeyIdx[(size_t)n]), tmp_buf(new (std::nothrow) KeyIdx[(size_t)n]);
+  if (!keys_buf || !tmp_buf) { msg = "build: out of host memory"; return TC_ENOMEM; }
+  KeyIdx* keys = keys_buf.get();
   uint64_t key_or = 0;
 #pragma omp parallel for schedule(static) reduction(| : key_or)
   for (int64_t i = 0; i < n; i++) {
@@ -131,8 +163,10 @@ int build_host_tree(const float* pos, const float* mass, int64_t n, int n_leaf, 
     keys[i].key = key; keys[i].idx = (uint32_t)i;
     key_or |= key;
   }
-  radix_sort(keys, tmp, key_or);
-  tmp.clear(); tmp.shrink_to_fit();
+  lap("keys");
+  radix_sort(keys, tmp_buf.get(), n, key_or, n_leaf);
+  lap("sort");
+  tmp_buf.reset();
 
   // ---- O2: breadth-first split of sorted key ranges
   // cell arrays (struct of vectors), breadth-first, children contiguous
@@ -153,7 +187,7 @@ int build_host_tree(const float* pos, const float* mass, int64_t n, int n_leaf, 
 #pragma omp parallel for schedule(dynamic, 256)
     for (int64_t c = lvl_b; c < lvl_e; c++) {
       if (c_count[c] <= n_leaf) continue;  // leaf (R4: <=)
-      const KeyIdx* kb = keys.data() + c_begin[c];
+      const KeyIdx* kb = keys + c_begin[c];
       const KeyIdx* ke = kb + c_count[c];
       int cnt = 0;
       const KeyIdx* p = kb;
@@ -180,7 +214,7 @@ int build_host_tree(const float* pos, const float* mass, int64_t n, int n_leaf, 
       if (k == 0) continue;
       const int64_t first = lvl_e + nch[(size_t)(c - lvl_b)];
       c_first_child[c] = (int32_t)first; c_nchild[c] = k;
-      const KeyIdx* k0 = keys.data();
+      const KeyIdx* k0 = keys;
       const KeyIdx* kb = k0 + c_begin[c];
       const KeyIdx* ke = kb + c_count[c];
       const KeyIdx* p = kb;
@@ -199,6 +233,7 @@ int build_host_tree(const float* pos, const float* mass, int64_t n, int n_leaf, 
   T.depth = (int32_t)level_start.size() - 2;
   const int n_levels = (int)level_start.size() - 1;
 
+  lap("split");
   // ---- O3: cell properties, fp64, bottom-up.  Leaves: direct sums
   // over members.  Nodes: union of the children's boxes, parallel-axis shift of the
   // children's moments to the node's centre of mass.
@@ -270,6 +305,7 @@ int build_host_tree(const float* pos, const float* mass, int64_t n, int n_leaf, 
   }
   T.n_leaves = n_leaves;
 
+  lap("moments");
   // ---- O4: groups = maximal cells with count <= N_group, or leaves, Morton order
   std::vector<int32_t> groups;
   {
@@ -283,6 +319,7 @@ int build_host_tree(const float* pos, const float* mass, int64_t n, int n_leaf, 
   }
   T.n_groups = (int64_t)groups.size();
 
+  lap("groups");
   // ---- pack: SoA float4 arrays in one buffer (layout in tc_internal.h)
   PackedLayout& Y = T.lay;
   size_t off = 0;
@@ -343,6 +380,7 @@ int build_host_tree(const float* pos, const float* mass, int64_t n, int n_leaf, 
     part[t] = make_float4(pos[3 * i], pos[3 * i + 1], pos[3 * i + 2], mass[i]);
     orig[t] = (int32_t)i;
   }
+  lap("pack");
   // Schedule (grp[i].w = i-th group to run): the persistent kernel hands groups out through an
   // atomic counter, so costly groups go first and the tail of the launch is made of cheap ones.
   // Cost model = issue slots per list entry of the kernel's lane mapping (tc_kernels.cu): a pass
@@ -359,19 +397,28 @@ int build_host_tree(const float* pos, const float* mass, int64_t n, int n_leaf, 
       }
       pass_cost[m] = (m == 0) ? 0.0 : best;
     }
-    std::vector<std::pair<float, int32_t>> order(groups.size());
-    for (size_t g = 0; g < groups.size(); g++) {
+    // counting sort by cost class (cost in 1/960 units: every kp / S with S <= 32 is a multiple of it
+    // up to rounding), descending; stable, so Morton order survives inside a class
+    const size_t ng = groups.size();
+    std::vector<int32_t> cls(ng);
+    int32_t cmax = 0;
+    for (size_t g = 0; g < ng; g++) {
       const int64_t cnt = c_count[groups[g]];
       const double cost = (double)(cnt / kPass) * pass_cost[kPass] + pass_cost[cnt % kPass];
-      order[g] = std::make_pair((float)-cost, (int32_t)g);
+      cls[g] = (int32_t)std::min(cost * 960.0 + 0.5, 1.0e6);
+      cmax = std::max(cmax, cls[g]);
     }
-    std::stable_sort(order.begin(), order.end(),
-                     [](const std::pair<float, int32_t>& a, const std::pair<float, int32_t>& b) { return a.first < b.first; });
+    std::vector<int32_t> start((size_t)cmax + 2, 0);
+    for (size_t g = 0; g < ng; g++) start[(size_t)(cmax - cls[g]) + 1]++;
+    for (size_t k = 1; k < start.size(); k++) start[k] += start[k - 1];
+    std::vector<int32_t> order(ng);
+    for (size_t g = 0; g < ng; g++) order[(size_t)start[(size_t)(cmax - cls[g])]++] = (int32_t)g;
     for (size_t g = 0; g < groups.size(); g++) {
       const int32_t c = groups[g];
-      grp[g] = make_int4(c, c_begin[c], c_count[c], order[g].second);
+      grp[g] = make_int4(c, c_begin[c], c_count[c], order[g]);
     }
   }
+  lap("schedule");
   return TC_OK;
 }
 

@@ -123,7 +123,8 @@ def test_config2_64k(name, n_group):
 # ---- config 3 at FULL size in the launch configuration bench.py times: sampled groups ----
 def test_config3_plummer_1m_sampled():
     pos, mass, theta, eps, n_leaf = inputs.make("plummer_1m")
-    n_group = 64
+    import bench
+    n_group = bench.N_GROUP          # the launch configuration bench.py times
     acc, pot, n_pc, n_pp, st = gpu_forces(pos, mass, theta, eps, n_leaf, n_group, device=True)
     o = Oracle(pos, mass, n_leaf, n_group)
     assert (st["n_cells"], st["n_leaves"], st["n_groups"], st["depth"]) == (o.n_cells, o.n_leaves, o.n_groups, o.depth)
