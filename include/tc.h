@@ -142,6 +142,19 @@ const char* tc_last_error(const tc_ctx* ctx);
 int tc_get_tree(tc_ctx* ctx, int32_t* perm, float* cell_bnd, float* cell_xm, float* cell_q,
                 int32_t* cell_link, int32_t* groups);
 
+/* Direct summation over ALL particles of the last tc_set_particles — the paper's accuracy reference
+ * (forces "by direct summation ... with double precision emulation"):
+ *   a_i = sum_{j != i} m_j (x_j - x_i) / s^3,  phi_i = -sum_{j != i} m_j / s,  s^2 = |x_j - x_i|^2 + eps^2
+ * for the n_targets particles listed in `targets` (HOST int64 indices in the caller's order; NULL = all
+ * n particles, n_targets ignored).  Interactions are evaluated in packed FP32 with a Newton-refined
+ * rsqrt, partial sums of 256 sources are accumulated in fp64.  No tree is needed (tc_build not required).
+ *   acc : n_targets x 3 fp64, pot : n_targets fp64 or NULL — CALLER-ALLOCATED, host or device (both the
+ *   same kind); host pointers: synchronous on return; device pointers: stream-ordered.
+ * eps == 0: coincident pairs contribute nothing.
+ * Errors: TC_ESTATE (no particles / host-only), TC_EINVAL (null acc, bad eps, target out of range),
+ * TC_ENOMEM, TC_ECUDA.                                                                              */
+int tc_direct(tc_ctx* ctx, float eps, const int64_t* targets, int64_t n_targets, double* acc, double* pot);
+
 /* Measured FP32 peak of the current device: an FFMA-only microbenchmark (16 independent
  * fma.rn.f32 chains per thread, 8 CTAs of 256 threads per SM, CUDA events on the context's
  * stream).  *tflops = 2 flops x FFMA lane-instructions / time.  This is the denominator the

@@ -26,7 +26,7 @@ TC_FLAG_HOST_ONLY = 1
 #: every symbol include/tc.h declares (checked by tests/test_abi.py)
 SYMBOLS = ["tc_create", "tc_create_ex", "tc_destroy", "tc_set_particles", "tc_build", "tc_forces",
            "tc_set_option", "tc_get_counts", "tc_get_stats", "tc_set_stream", "tc_sync",
-           "tc_last_error", "tc_get_tree", "tc_fp32_peak"]
+           "tc_last_error", "tc_get_tree", "tc_fp32_peak", "tc_direct"]
 
 
 class tc_stats(C.Structure):
@@ -77,6 +77,7 @@ def lib():
     L.tc_last_error.argtypes = [vp]
     L.tc_get_tree.argtypes = [vp] + [vp] * 6
     L.tc_fp32_peak.argtypes = [vp, C.POINTER(C.c_double)]
+    L.tc_direct.argtypes = [vp, f32, vp, i64, vp, vp]
     _lib = L
     return L
 
@@ -158,6 +159,14 @@ def tc_get_tree(ctx) -> dict:
     return out
 
 
+def tc_direct(ctx, eps: float, targets, acc, pot=None):
+    """Direct summation for `targets` (host int64 array or None = all particles) into fp64 acc / pot."""
+    nt = 0 if targets is None else int(len(targets))
+    if targets is not None:
+        assert isinstance(targets, np.ndarray) and targets.dtype == np.int64, "targets must be a host int64 array"
+    _check(ctx, lib().tc_direct(ctx, float(eps), _ptr(targets), nt, _ptr(acc), _ptr(pot)))
+
+
 def tc_fp32_peak(ctx) -> float:
     """Measured FFMA-only FP32 throughput of the current device in TFLOP/s."""
     v = C.c_double(0.0)
@@ -207,6 +216,15 @@ class TreeCode:
             acc = np.empty((self.n, 3), np.float32)
             pot = np.empty(self.n, np.float32)
         tc_forces(self.ctx, theta, eps, acc, pot)
+        return acc, pot
+
+    def direct(self, eps, targets=None):
+        """Host path of tc_direct: returns (acc fp64 [n_t,3], pot fp64 [n_t])."""
+        nt = self.n if targets is None else len(targets)
+        acc = np.empty((nt, 3), np.float64)
+        pot = np.empty(nt, np.float64)
+        t = None if targets is None else np.ascontiguousarray(targets, dtype=np.int64)
+        tc_direct(self.ctx, eps, t, acc, pot)
         return acc, pot
 
     def counts(self):

@@ -40,6 +40,9 @@ struct tc_ctx {
   tc::DeviceCounters* d_ctr = nullptr;
   uint32_t* d_spill = nullptr; size_t spill_elems = 0; int spill_cap = 4096;
   bool forces_done = false, timing_pending = false;
+  // tc_direct scratch
+  float4* d_src = nullptr; int64_t src_cap = 0; bool src_valid = false;
+  long long* d_tgt = nullptr; double* d_dacc = nullptr; double* d_dpot = nullptr; int64_t tgt_cap = 0;
   tc_stats stats{};
 };
 
@@ -139,6 +142,7 @@ void tc_destroy(tc_ctx* c) {
     if (c->stream) cudaStreamSynchronize(c->stream);
     cudaFree(c->d_tree); cudaFree(c->d_acc); cudaFree(c->d_pot); cudaFree(c->d_npc); cudaFree(c->d_npp);
     cudaFree(c->d_ctr); cudaFree(c->d_spill);
+    cudaFree(c->d_src); cudaFree(c->d_tgt); cudaFree(c->d_dacc); cudaFree(c->d_dpot);
     if (c->ev0) cudaEventDestroy(c->ev0);
     if (c->ev1) cudaEventDestroy(c->ev1);
     if (c->own_stream) cudaStreamDestroy(c->own_stream);
@@ -181,7 +185,7 @@ int tc_set_particles(tc_ctx* c, const float* pos, const float* mass, int64_t n) 
   if (!c) return TC_EINVAL;
   if (!pos || !mass) return fail(c, TC_EINVAL, "tc_set_particles: null pointer");
   if (n < 1 || n > 2147483647LL) return fail(c, TC_EINVAL, "tc_set_particles: n must be in [1, 2^31-1]");
-  c->built = false; c->forces_done = false;
+  c->built = false; c->forces_done = false; c->src_valid = false;
   try { c->pos.resize((size_t)n * 3); c->mass.resize((size_t)n); } catch (...) { return fail(c, TC_ENOMEM, "tc_set_particles: out of host memory"); }
   if (is_device_ptr(c, pos)) { TC_CUDA(c, cudaMemcpyAsync(c->pos.data(), pos, sizeof(float) * 3 * (size_t)n, cudaMemcpyDeviceToHost, c->stream)); }
   else std::memcpy(c->pos.data(), pos, sizeof(float) * 3 * (size_t)n);
@@ -306,6 +310,64 @@ int tc_get_stats(tc_ctx* c, tc_stats* out) {
   if (!c->host_only && c->timing_pending) { TC_CUDA(c, cudaStreamSynchronize(c->stream)); rc = collect(c); }
   *out = c->stats;
   return rc;
+}
+
+int tc_direct(tc_ctx* c, float eps, const int64_t* targets, int64_t n_targets, double* acc, double* pot) {
+  if (!c) return TC_EINVAL;
+  if (c->host_only) return fail(c, TC_ESTATE, "tc_direct: host-only context has no device (there is no CPU fallback)");
+  if (c->n < 1) return fail(c, TC_ESTATE, "tc_direct: no particles (call tc_set_particles first)");
+  if (!acc) return fail(c, TC_EINVAL, "tc_direct: acc is null");
+  if (!(eps >= 0.f) || !std::isfinite(eps)) return fail(c, TC_EINVAL, "tc_direct: eps must be finite and >= 0");
+  const int64_t n = c->n;
+  const int64_t nt = targets ? n_targets : n;
+  if (nt < 1) return fail(c, TC_EINVAL, "tc_direct: n_targets must be >= 1");
+  if (targets)
+    for (int64_t t = 0; t < nt; t++)
+      if (targets[t] < 0 || targets[t] >= n) return fail(c, TC_EINVAL, "tc_direct: target index out of range");
+  const bool acc_dev = is_device_ptr(c, acc), pot_dev = pot ? is_device_ptr(c, pot) : acc_dev;
+  if (acc_dev != pot_dev) return fail(c, TC_EINVAL, "tc_direct: acc and pot must both be host or both be device pointers");
+  if (!c->src_valid) {                                   // (x, y, z, m) in the caller's order
+    if (c->src_cap < n) {
+      cudaFree(c->d_src); c->d_src = nullptr; c->src_cap = 0;
+      TC_CUDA(c, cudaMalloc((void**)&c->d_src, sizeof(float4) * (size_t)n));
+      c->src_cap = n;
+    }
+    std::vector<float4> h;
+    try { h.resize((size_t)n); } catch (...) { return fail(c, TC_ENOMEM, "tc_direct: out of host memory"); }
+    const float* P = c->pos.data(); const float* M = c->mass.data();
+#pragma omp parallel for schedule(static)
+    for (int64_t i = 0; i < n; i++) h[(size_t)i] = make_float4(P[3 * i], P[3 * i + 1], P[3 * i + 2], M[i]);
+    TC_CUDA(c, cudaMemcpyAsync(c->d_src, h.data(), sizeof(float4) * (size_t)n, cudaMemcpyHostToDevice, c->stream));
+    TC_CUDA(c, cudaStreamSynchronize(c->stream));
+    c->src_valid = true;
+  }
+  if (c->tgt_cap < nt) {
+    cudaFree(c->d_tgt); cudaFree(c->d_dacc); cudaFree(c->d_dpot); c->d_tgt = nullptr; c->d_dacc = c->d_dpot = nullptr; c->tgt_cap = 0;
+    TC_CUDA(c, cudaMalloc((void**)&c->d_tgt, sizeof(long long) * (size_t)nt));
+    TC_CUDA(c, cudaMalloc((void**)&c->d_dacc, sizeof(double) * 3 * (size_t)nt));
+    TC_CUDA(c, cudaMalloc((void**)&c->d_dpot, sizeof(double) * (size_t)nt));
+    c->tgt_cap = nt;
+  }
+  if (targets) {
+    static_assert(sizeof(long long) == sizeof(int64_t), "int64_t layout");
+    TC_CUDA(c, cudaMemcpyAsync(c->d_tgt, targets, sizeof(int64_t) * (size_t)nt, cudaMemcpyHostToDevice, c->stream));
+  }
+  double* o_acc = acc_dev ? acc : c->d_dacc;
+  double* o_pot = pot ? (acc_dev ? pot : c->d_dpot) : nullptr;
+  TC_CUDA(c, cudaEventRecord(c->ev0, c->stream));
+  const int le = tc::launch_direct(c->d_src, n, targets ? c->d_tgt : nullptr, nt, eps, o_acc, o_pot, c->n_sm, c->stream);
+  if (le != 0) return cuda_fail(c, (cudaError_t)le, "direct-sum kernel launch");
+  TC_CUDA(c, cudaEventRecord(c->ev1, c->stream));
+  if (!acc_dev) {
+    TC_CUDA(c, cudaMemcpyAsync(acc, c->d_dacc, sizeof(double) * 3 * (size_t)nt, cudaMemcpyDeviceToHost, c->stream));
+    if (pot) TC_CUDA(c, cudaMemcpyAsync(pot, c->d_dpot, sizeof(double) * (size_t)nt, cudaMemcpyDeviceToHost, c->stream));
+  }
+  // targets (host memory of the caller) must not be in flight on return
+  TC_CUDA(c, cudaStreamSynchronize(c->stream));
+  float ms = 0.f;
+  if (cudaEventElapsedTime(&ms, c->ev0, c->ev1) == cudaSuccess) c->stats.t_gpu_ms = ms; else cudaGetLastError();
+  c->timing_pending = false;
+  return TC_OK;
 }
 
 int tc_fp32_peak(tc_ctx* c, double* tflops) {

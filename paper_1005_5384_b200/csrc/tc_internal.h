@@ -92,6 +92,10 @@ struct ForceLaunch {
 int launch_forces(const DeviceTree& T, const ForceLaunch& L, void* stream);
 // Number of warps the persistent grid runs (for sizing the spill buffer).
 int forces_total_warps(int n_sm, int stack_smem);
+// Direct summation (tc_direct): src [n] (x,y,z,m) device, targets device int64 [n_t] or nullptr (all),
+// acc [n_t,3] / pot [n_t] device fp64 (zeroed inside).  Returns a cudaError_t as int.
+int launch_direct(const float4* src, long long n, const long long* targets, long long n_t, float eps, double* acc,
+                  double* pot, int n_sm, void* stream);
 // FFMA-only microbenchmark (tc_fp32_peak): returns a cudaError_t as int, *tflops on success.
 int measure_fp32_peak(int n_sm, void* stream, double* tflops);
 

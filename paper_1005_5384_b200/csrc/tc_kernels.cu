@@ -108,8 +108,8 @@ __device__ __forceinline__ float rsqrt_approx(float x) {
 typedef unsigned long long f2;
 __device__ __forceinline__ f2 pk(float lo, float hi) { f2 r; asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(lo), "f"(hi)); return r; }
 __device__ __forceinline__ f2 bc(float x) { return pk(x, x); }
-__device__ __forceinline__ float lo(f2 v) { float a, b; asm("mov.b64 {%0, %1}, %2;" : "=f"(a), "=f"(b) : "l"(v)); return a; }
-__device__ __forceinline__ float hi(f2 v) { float a, b; asm("mov.b64 {%0, %1}, %2;" : "=f"(a), "=f"(b) : "l"(v)); return b; }
+__device__ __forceinline__ float lo(f2 v) { float a; asm("{ .reg .b32 t; mov.b64 {%0, t}, %1; }" : "=f"(a) : "l"(v)); return a; }
+__device__ __forceinline__ float hi(f2 v) { float b; asm("{ .reg .b32 t; mov.b64 {t, %0}, %1; }" : "=f"(b) : "l"(v)); return b; }
 __device__ __forceinline__ f2 add2(f2 a, f2 b) { f2 d; asm("add.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b)); return d; }
 __device__ __forceinline__ f2 sub2(f2 a, f2 b) { f2 d; asm("sub.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b)); return d; }
 __device__ __forceinline__ f2 mul2(f2 a, f2 b) { f2 d; asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b)); return d; }
@@ -481,6 +481,120 @@ int dispatch(const DeviceTree& T, const ForceLaunch& L, cudaStream_t st, int* pe
 
 int launch_forces(const DeviceTree& T, const ForceLaunch& L, void* stream) {
   return dispatch(T, L, (cudaStream_t)stream, nullptr);
+}
+
+// ---- tc_direct: direct summation (the paper's accuracy reference) ----------------
+// a_i = sum_{j != i} m_j d / s^3, phi_i = -sum_{j != i} m_j / s, d = x_j - x_i, s^2 = |d|^2 + eps^2.
+// Packed FP32 per interaction with one Newton step on rsqrt.approx (relative error ~1e-7 per term),
+// partial sums of 256 sources in fp32, flushed into fp64 accumulators ("double precision emulation"
+// in the paper's words); 4 targets per thread, sources staged through shared memory, the source
+// range split over blockIdx.y and combined with fp64 atomics.
+namespace {
+constexpr int kDirThreads = 128, kDirTile = 256, kDirTargetsPerCta = 4 * kDirThreads;
+
+template <bool kEps0>
+__device__ __forceinline__ void direct_interact(const Pos2& p, float eps2, const float4 b, Acc2& a) {
+  const f2 dx = sub2(bc(b.x), p.x), dy = sub2(bc(b.y), p.y), dz = sub2(bc(b.z), p.z);
+  const f2 s2 = fma2(dz, dz, fma2(dy, dy, fma2(dx, dx, bc(eps2))));
+  float r0 = rsqrt_approx(lo(s2)), r1 = rsqrt_approx(hi(s2));
+  if (kEps0) { r0 = (lo(s2) > 0.f) ? r0 : 0.f; r1 = (hi(s2) > 0.f) ? r1 : 0.f; }
+  f2 ri = pk(r0, r1);
+  const f2 h = mul2(s2, bc(-0.5f));                       // Newton: y <- y (1.5 - 0.5 x y^2)
+  ri = mul2(ri, fma2(h, mul2(ri, ri), bc(1.5f)));
+  const f2 ri2 = mul2(ri, ri);
+  const f2 mr = mul2(bc(b.w), ri);
+  const f2 mr3 = mul2(mr, ri2);
+  a.npot = add2(a.npot, mr);
+  a.ax = fma2(mr3, dx, a.ax); a.ay = fma2(mr3, dy, a.ay); a.az = fma2(mr3, dz, a.az);
+}
+
+template <bool kEps0>
+__global__ void __launch_bounds__(kDirThreads)
+direct_kernel(const float4* __restrict__ src, long long n, const long long* __restrict__ targets, long long n_t,
+              float eps, double* __restrict__ acc, double* __restrict__ pot) {
+  __shared__ float4 tile[kDirTile];
+  const float eps2 = eps * eps;
+  const long long t0 = (long long)blockIdx.x * kDirTargetsPerCta + threadIdx.x;
+  long long ti[4];
+  Pos2 P[2];
+  float msf[4];
+#pragma unroll
+  for (int j = 0; j < 4; j++) {
+    const long long t = t0 + (long long)j * kDirThreads;
+    ti[j] = (t < n_t) ? (targets ? targets[t] : t) : -1;
+  }
+#pragma unroll
+  for (int j = 0; j < 2; j++) {
+    const float4 a = __ldg(src + (ti[2 * j] >= 0 ? ti[2 * j] : 0)), b = __ldg(src + (ti[2 * j + 1] >= 0 ? ti[2 * j + 1] : 0));
+    P[j].x = add2(pk(a.x, b.x), bc(0.f)); P[j].y = add2(pk(a.y, b.y), bc(0.f)); P[j].z = add2(pk(a.z, b.z), bc(0.f));
+    msf[2 * j] = a.w; msf[2 * j + 1] = b.w;
+  }
+  double d[4][4];
+#pragma unroll
+  for (int j = 0; j < 4; j++) d[j][0] = d[j][1] = d[j][2] = d[j][3] = 0.0;
+  // this CTA's share of the sources, in whole tiles
+  const long long n_tiles = (n + kDirTile - 1) / kDirTile;
+  const long long tb = n_tiles * blockIdx.y / gridDim.y, te = n_tiles * (blockIdx.y + 1) / gridDim.y;
+  for (long long tl = tb; tl < te; tl++) {
+    __syncthreads();
+#pragma unroll
+    for (int k = 0; k < kDirTile / kDirThreads; k++) {
+      const long long j = tl * kDirTile + threadIdx.x + k * kDirThreads;
+      // padding: massless sources far away contribute exactly zero
+      tile[threadIdx.x + k * kDirThreads] = (j < n) ? __ldg(src + j) : make_float4(1e18f, 1e18f, 1e18f, 0.f);
+    }
+    __syncthreads();
+    Acc2 A[2];
+#pragma unroll
+    for (int j = 0; j < 2; j++) A[j].ax = A[j].ay = A[j].az = A[j].npot = 0ull;
+#pragma unroll 4
+    for (int k = 0; k < kDirTile; k++) {
+      const float4 b = tile[k];
+      direct_interact<kEps0>(P[0], eps2, b, A[0]);
+      direct_interact<kEps0>(P[1], eps2, b, A[1]);
+    }
+#pragma unroll
+    for (int j = 0; j < 2; j++) {
+      d[2 * j][0] += (double)lo(A[j].ax); d[2 * j][1] += (double)lo(A[j].ay); d[2 * j][2] += (double)lo(A[j].az);
+      d[2 * j][3] += (double)lo(A[j].npot);
+      d[2 * j + 1][0] += (double)hi(A[j].ax); d[2 * j + 1][1] += (double)hi(A[j].ay); d[2 * j + 1][2] += (double)hi(A[j].az);
+      d[2 * j + 1][3] += (double)hi(A[j].npot);
+    }
+  }
+#pragma unroll
+  for (int j = 0; j < 4; j++) {
+    if (ti[j] < 0) continue;
+    const long long t = t0 + (long long)j * kDirThreads;
+    double ph = -d[j][3];
+    // the target met itself once (in exactly one source split): remove -m/eps again
+    if (!kEps0 && blockIdx.y == 0) {
+      float r = rsqrt_approx(eps2);
+      r = r * fmaf(-0.5f * eps2, r * r, 1.5f);
+      ph += (double)(msf[j] * r);
+    }
+    atomicAdd(acc + 3 * t + 0, d[j][0]); atomicAdd(acc + 3 * t + 1, d[j][1]); atomicAdd(acc + 3 * t + 2, d[j][2]);
+    if (pot) atomicAdd(pot + t, ph);
+  }
+}
+}  // namespace
+
+int launch_direct(const float4* src, long long n, const long long* targets, long long n_t, float eps, double* acc,
+                  double* pot, int n_sm, void* stream) {
+  cudaStream_t st = (cudaStream_t)stream;
+  cudaError_t e = cudaMemsetAsync(acc, 0, sizeof(double) * 3 * (size_t)n_t, st);
+  if (e == cudaSuccess && pot) e = cudaMemsetAsync(pot, 0, sizeof(double) * (size_t)n_t, st);
+  if (e != cudaSuccess) return (int)e;
+  const long long tiles_t = (n_t + kDirTargetsPerCta - 1) / kDirTargetsPerCta;
+  const long long tiles_s = (n + kDirTile - 1) / kDirTile;
+  long long splits = (8LL * n_sm + tiles_t - 1) / tiles_t;          // >= 8 CTAs per SM in flight
+  if (splits > tiles_s) splits = tiles_s;
+  if (splits > 65535) splits = 65535;
+  if (splits < 1) splits = 1;
+  if (tiles_t > 2147483647LL) return (int)cudaErrorInvalidValue;
+  const dim3 grid((unsigned)tiles_t, (unsigned)splits);
+  if (eps * eps == 0.f) direct_kernel<true><<<grid, kDirThreads, 0, st>>>(src, n, targets, n_t, eps, acc, pot);
+  else direct_kernel<false><<<grid, kDirThreads, 0, st>>>(src, n, targets, n_t, eps, acc, pot);
+  return (int)cudaGetLastError();
 }
 
 // ---- tc_fp32_peak: what the FP32 pipe of this device sustains with nothing but FFMA in flight
