@@ -104,6 +104,10 @@ int tc_forces(tc_ctx* ctx, float theta, float eps, float* acc, float* pot);
 
 /* Options (double-valued).  Keys:
  *   "n_group"     N_group >= 1; takes effect at the next tc_build
+ *   "device_build" 0 (default: host build, as in the paper) or 1: tc_build runs the same
+ *                 construction on the GPU (tc_build_gpu.cu) and writes the packed tree in device memory —
+ *                 no bulk H2D; t_host_ms of tc_stats is then the wall time of the device build, t_copy_ms 0.
+ *                 Cells, boundary cubes, groups and counts are identical to the host build's.
  *   "stack_smem"  walk-stack entries kept in shared memory per warp before
  *                 spilling to global memory: 256 (default) or 64 (test of the
  *                 spill path)

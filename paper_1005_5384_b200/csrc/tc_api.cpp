@@ -24,6 +24,7 @@ struct tc_ctx {
   std::string err;
   // options
   int n_group = 96;
+  bool device_build = false;          // option "device_build": tc_build_gpu.cu instead of tc_build.cpp
   int stack_smem = 256;
   // particles (host copy, caller order)
   std::vector<float> pos, mass;
@@ -40,6 +41,8 @@ struct tc_ctx {
   tc::DeviceCounters* d_ctr = nullptr;
   uint32_t* d_spill = nullptr; size_t spill_elems = 0; int spill_cap = 4096;
   bool forces_done = false, timing_pending = false;
+  tc::DeviceBuildScratch dscr;
+  bool tree_host_valid = false;       // the host copy of the packed tree (tc_get_tree) is current
   // tc_direct scratch
   float4* d_src = nullptr; int64_t src_cap = 0; bool src_valid = false;
   long long* d_tgt = nullptr; double* d_dacc = nullptr; double* d_dpot = nullptr; int64_t tgt_cap = 0;
@@ -101,6 +104,26 @@ int collect(tc_ctx* c) {
   return TC_OK;
 }
 
+// (x, y, z, m) of the caller's particles as one float4 array on the device (tc_direct, device build)
+int ensure_src(tc_ctx* c) {
+  if (c->src_valid) return TC_OK;
+  const int64_t n = c->n;
+  if (c->src_cap < n) {
+    cudaFree(c->d_src); c->d_src = nullptr; c->src_cap = 0;
+    TC_CUDA(c, cudaMalloc((void**)&c->d_src, sizeof(float4) * (size_t)n));
+    c->src_cap = n;
+  }
+  std::vector<float4> h;
+  try { h.resize((size_t)n); } catch (...) { return fail(c, TC_ENOMEM, "out of host memory"); }
+  const float* P = c->pos.data(); const float* M = c->mass.data();
+#pragma omp parallel for schedule(static)
+  for (int64_t i = 0; i < n; i++) h[(size_t)i] = make_float4(P[3 * i], P[3 * i + 1], P[3 * i + 2], M[i]);
+  TC_CUDA(c, cudaMemcpyAsync(c->d_src, h.data(), sizeof(float4) * (size_t)n, cudaMemcpyHostToDevice, c->stream));
+  TC_CUDA(c, cudaStreamSynchronize(c->stream));
+  c->src_valid = true;
+  return TC_OK;
+}
+
 }  // namespace
 
 extern "C" {
@@ -142,6 +165,7 @@ void tc_destroy(tc_ctx* c) {
     if (c->stream) cudaStreamSynchronize(c->stream);
     cudaFree(c->d_tree); cudaFree(c->d_acc); cudaFree(c->d_pot); cudaFree(c->d_npc); cudaFree(c->d_npp);
     cudaFree(c->d_ctr); cudaFree(c->d_spill);
+    c->dscr.release();
     cudaFree(c->d_src); cudaFree(c->d_tgt); cudaFree(c->d_dacc); cudaFree(c->d_dpot);
     if (c->ev0) cudaEventDestroy(c->ev0);
     if (c->ev1) cudaEventDestroy(c->ev1);
@@ -158,6 +182,11 @@ int tc_set_option(tc_ctx* c, const char* key, double v) {
   if (!std::strcmp(key, "n_group")) {
     if (!(v >= 1.0) || v > 2147483647.0 || v != std::floor(v)) return fail(c, TC_EINVAL, "tc_set_option: n_group must be an integer >= 1");
     c->n_group = (int)v; return TC_OK;
+  }
+  if (!std::strcmp(key, "device_build")) {
+    if (v != 0.0 && v != 1.0) return fail(c, TC_EINVAL, "tc_set_option: device_build must be 0 or 1");
+    if (c->host_only && v != 0.0) return fail(c, TC_ESTATE, "tc_set_option: device_build needs a device");
+    c->device_build = (v != 0.0); return TC_OK;
   }
   if (!std::strcmp(key, "stack_smem")) {
     if (v != 256.0 && v != 64.0) return fail(c, TC_EINVAL, "tc_set_option: stack_smem must be 256 or 64");
@@ -212,6 +241,22 @@ int tc_build(tc_ctx* c, int n_leaf) {
   if (n_leaf < 1) return fail(c, TC_EINVAL, "tc_build: n_leaf must be >= 1");
   c->built = false; c->forces_done = false;
   if (!c->host_only) TC_CUDA(c, cudaStreamSynchronize(c->stream));  // the pinned buffer may still be in flight
+  if (c->device_build) {
+    { const int rc = ensure_src(c); if (rc != TC_OK) return rc; }
+    const double t0 = now_ms();
+    std::string msg;
+    const int rc = tc::build_device_tree(c->d_src, c->n, n_leaf, c->n_group, c->dscr, &c->d_tree, &c->d_tree_cap, c->tree,
+                                         c->dview, c->stream, msg);
+    if (rc != TC_OK) { cudaGetLastError(); return fail(c, rc, "tc_build (device): " + msg); }
+    const tc::HostTree& T = c->tree;
+    tc_stats& S = c->stats;
+    S = tc_stats{};
+    S.n = c->n; S.n_cells = T.n_cells; S.n_leaves = T.n_leaves; S.n_groups = T.n_groups; S.depth = T.depth;
+    S.n_leaf = n_leaf; S.n_group = c->n_group; S.t_host_ms = now_ms() - t0; S.t_copy_ms = 0.0; S.tree_bytes = (int64_t)T.lay.bytes;
+    c->tree_host_valid = false;
+    c->built = true;
+    return TC_OK;
+  }
   const double t0 = now_ms();
   std::string msg;
   const int rc = tc::build_host_tree(c->pos.data(), c->mass.data(), c->n, n_leaf, c->n_group, c->tree, packed_alloc, c, msg);
@@ -241,6 +286,7 @@ int tc_build(tc_ctx* c, int n_leaf) {
     D.grp = (const int4*)(b + T.lay.off_grp);
     D.n = c->n; D.n_cells = T.n_cells; D.n_groups = T.n_groups;
   }
+  c->tree_host_valid = true;
   c->built = true;
   return TC_OK;
 }
@@ -326,21 +372,7 @@ int tc_direct(tc_ctx* c, float eps, const int64_t* targets, int64_t n_targets, d
       if (targets[t] < 0 || targets[t] >= n) return fail(c, TC_EINVAL, "tc_direct: target index out of range");
   const bool acc_dev = is_device_ptr(c, acc), pot_dev = pot ? is_device_ptr(c, pot) : acc_dev;
   if (acc_dev != pot_dev) return fail(c, TC_EINVAL, "tc_direct: acc and pot must both be host or both be device pointers");
-  if (!c->src_valid) {                                   // (x, y, z, m) in the caller's order
-    if (c->src_cap < n) {
-      cudaFree(c->d_src); c->d_src = nullptr; c->src_cap = 0;
-      TC_CUDA(c, cudaMalloc((void**)&c->d_src, sizeof(float4) * (size_t)n));
-      c->src_cap = n;
-    }
-    std::vector<float4> h;
-    try { h.resize((size_t)n); } catch (...) { return fail(c, TC_ENOMEM, "tc_direct: out of host memory"); }
-    const float* P = c->pos.data(); const float* M = c->mass.data();
-#pragma omp parallel for schedule(static)
-    for (int64_t i = 0; i < n; i++) h[(size_t)i] = make_float4(P[3 * i], P[3 * i + 1], P[3 * i + 2], M[i]);
-    TC_CUDA(c, cudaMemcpyAsync(c->d_src, h.data(), sizeof(float4) * (size_t)n, cudaMemcpyHostToDevice, c->stream));
-    TC_CUDA(c, cudaStreamSynchronize(c->stream));
-    c->src_valid = true;
-  }
+  { const int rc = ensure_src(c); if (rc != TC_OK) return rc; }
   if (c->tgt_cap < nt) {
     cudaFree(c->d_tgt); cudaFree(c->d_dacc); cudaFree(c->d_dpot); c->d_tgt = nullptr; c->d_dacc = c->d_dpot = nullptr; c->tgt_cap = 0;
     TC_CUDA(c, cudaMalloc((void**)&c->d_tgt, sizeof(long long) * (size_t)nt));
@@ -382,6 +414,16 @@ int tc_get_tree(tc_ctx* c, int32_t* perm, float* cell_bnd, float* cell_xm, float
                 int32_t* groups) {
   if (!c) return TC_EINVAL;
   if (!c->built) return fail(c, TC_ESTATE, "tc_get_tree: no tree (call tc_build first)");
+  if (!c->tree_host_valid) {                       // built on the device: bring the packed tree back
+    tc::HostTree& W = c->tree;
+    if (!packed_alloc(c, W.lay.bytes)) return fail(c, TC_ENOMEM, "tc_get_tree: out of host memory");
+    try { W.link.resize((size_t)W.n_cells * 4); W.q6.resize((size_t)W.n_cells * 6); } catch (...) { return fail(c, TC_ENOMEM, "tc_get_tree: out of host memory"); }
+    TC_CUDA(c, cudaStreamSynchronize(c->stream));
+    TC_CUDA(c, cudaMemcpy(W.packed, c->d_tree, W.lay.bytes, cudaMemcpyDeviceToHost));
+    TC_CUDA(c, cudaMemcpy(W.link.data(), c->dscr.link, sizeof(int32_t) * 4 * (size_t)W.n_cells, cudaMemcpyDeviceToHost));
+    TC_CUDA(c, cudaMemcpy(W.q6.data(), c->dscr.q6, sizeof(float) * 6 * (size_t)W.n_cells, cudaMemcpyDeviceToHost));
+    c->tree_host_valid = true;
+  }
   const tc::HostTree& T = c->tree;
   const char* b = (const char*)T.packed;
   const size_t nc = (size_t)T.n_cells;

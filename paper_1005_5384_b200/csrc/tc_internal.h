@@ -92,6 +92,33 @@ struct ForceLaunch {
 int launch_forces(const DeviceTree& T, const ForceLaunch& L, void* stream);
 // Number of warps the persistent grid runs (for sizing the spill buffer).
 int forces_total_warps(int n_sm, int stack_smem);
+// Scratch of the device-side builder (tc_build_gpu.cu); grow-only, owned by the context.
+struct DeviceBuildScratch {
+  unsigned long long *keys = nullptr, *keys_alt = nullptr;  size_t cap_keys = 0, cap_keys_alt = 0;
+  unsigned int *idx = nullptr, *idx_alt = nullptr;          size_t cap_idx = 0, cap_idx_alt = 0;
+  char* cub_tmp = nullptr;                                   size_t cap_tmp = 0;
+  int *c_begin = nullptr, *c_count = nullptr, *c_first = nullptr, *c_nchild = nullptr, *c_parent = nullptr;
+  size_t cap_cbegin = 0, cap_ccount = 0, cap_cfirst = 0, cap_cnchild = 0, cap_cparent = 0;
+  int *nch = nullptr, *off = nullptr;                        size_t cap_nch = 0, cap_off = 0;
+  char* mom = nullptr;                                       size_t cap_mom = 0;     // Moments[]
+  unsigned char* is_group = nullptr;                         size_t cap_isg = 0;
+  int *gcell = nullptr, *gcell_sorted = nullptr;             size_t cap_gcell = 0, cap_gcells = 0;
+  unsigned int *gkey = nullptr, *gkey_alt = nullptr, *gval = nullptr, *gval_alt = nullptr;
+  size_t cap_gkey = 0, cap_gkeya = 0, cap_gval = 0, cap_gvala = 0;
+  char* boxes = nullptr;                                     size_t cap_boxes = 0;
+  unsigned int* small = nullptr;                             size_t cap_small = 0;   // counters
+  int4* link = nullptr;                                      size_t cap_link = 0;    // tc_get_tree
+  float* q6 = nullptr;                                       size_t cap_q6 = 0;      // tc_get_tree
+  float* pass_cost = nullptr;                                size_t cap_pc = 0;
+  void release();
+};
+
+// Device-side builder (option "device_build"): same tree, same packed layout, written straight into
+// *d_tree (grown if needed).  src = (x,y,z,m) in the caller's order, device.  Fills T's sizes/layout
+// and D.  Returns TC_OK or an error code with msg set.
+int build_device_tree(const float4* src, int64_t n, int n_leaf, int n_group, DeviceBuildScratch& S, void** d_tree,
+                      size_t* d_tree_cap, HostTree& T, DeviceTree& D, void* stream, std::string& msg);
+
 // Direct summation (tc_direct): src [n] (x,y,z,m) device, targets device int64 [n_t] or nullptr (all),
 // acc [n_t,3] / pot [n_t] device fp64 (zeroed inside).  Returns a cudaError_t as int.
 int launch_direct(const float4* src, long long n, const long long* targets, long long n_t, float eps, double* acc,

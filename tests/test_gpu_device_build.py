@@ -1,0 +1,105 @@
+"""Device-side tree build (option "device_build") — `-m gpu`.
+
+The GPU builder must produce the SAME tree as the host builder and as the oracle: identical cells, links,
+groups (Morton order), bit-identical fp32 boundary cubes, moments equal up to the last fp32 bit (the
+particle order inside a leaf — hence the fp64 summation order — may differ), and therefore exactly the same
+interaction counts and forces within the usual tolerances."""
+import numpy as np
+import pytest
+
+from oracle import Oracle
+from paper_1005_5384_b200 import binding as B
+from paper_1005_5384_b200 import build as tc_build
+from paper_1005_5384_b200 import inputs
+from test_gpu_parity import check
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module", autouse=True)
+def _built():
+    tc_build.build()
+
+
+def _trees(pos, mass, n_leaf, n_group):
+    out = []
+    for dev in (0, 1):
+        with B.TreeCode(n_group=n_group) as tc:
+            tc.set_option("device_build", dev)
+            tc.set_particles(pos, mass)
+            tc.build(n_leaf)
+            out.append((tc.stats(), tc.tree()))
+    return out
+
+
+def _same_tree(h, d, pos):
+    (sh, th), (sd, td) = h, d
+    for k in ("n", "n_cells", "n_leaves", "n_groups", "depth", "tree_bytes"):
+        assert sh[k] == sd[k], k
+    assert np.array_equal(th["link"], td["link"])
+    assert np.array_equal(th["groups"], td["groups"])
+    assert np.array_equal(th["bnd"], td["bnd"])                      # boundary cubes: bit-identical
+    n = sh["n"]
+    assert np.array_equal(np.sort(td["perm"]), np.arange(n))
+    # same members per leaf (order inside a leaf may differ)
+    leaves = np.where(th["link"][:, 1] == 0)[0]
+    for c in leaves[:: max(1, len(leaves) // 500)]:
+        b, k = th["link"][c, 2], th["link"][c, 3]
+        assert set(th["perm"][b:b + k].tolist()) == set(td["perm"][b:b + k].tolist())
+    # moments: equal up to fp32 rounding of slightly different fp64 sums
+    ext = max(1.0, float(np.abs(pos).max()))
+    assert np.allclose(th["xm"][:, 3], td["xm"][:, 3], rtol=2e-7, atol=0)
+    assert np.abs(th["xm"][:, :3] - td["xm"][:, :3]).max() <= 2.4e-7 * ext
+    qs = np.abs(th["q"]).max(1) + 1e-30
+    assert (np.abs(th["q"] - td["q"]).max(1) <= 1e-5 * qs + 1e-12 * th["xm"][:, 3] * ext * ext).all()
+
+
+@pytest.mark.parametrize("name,n_leaf,n_group", [("plummer_1k", 16, 64), ("plummer_64k", 16, 96), ("cube_64k", 8, 32),
+                                                   ("plummer_64k", 1, 1), ("plummer_1m", 16, 96)])
+def test_device_tree_equals_host_tree(name, n_leaf, n_group):
+    pos, mass, *_ = inputs.make(name)
+    h, d = _trees(pos, mass, n_leaf, n_group)
+    _same_tree(h, d, pos)
+
+
+def test_device_tree_degenerate_inputs():
+    # one particle; two particles; coincident particles (level-21 leaf); all particles in one leaf
+    for pos, mass, n_leaf in [
+        (np.array([[0.5, 0.25, -1.0]], np.float32), np.array([1.0], np.float32), 16),
+        (np.array([[0, 0, 0], [1, 2, 3]], np.float32), np.array([1.0, 2.0], np.float32), 1),
+        (None, None, 16),
+        (inputs.plummer(12, 3)[0], inputs.plummer(12, 3)[1], 16),
+    ]:
+        if pos is None:
+            pos, mass = inputs.plummer(2048, 11)
+            pos[:200] = pos[0]
+        h, d = _trees(pos, mass, n_leaf, 64)
+        _same_tree(h, d, pos)
+
+
+@pytest.mark.parametrize("name", ["plummer_1k", "plummer_64k"])
+def test_forces_on_device_built_tree_match_oracle(name):
+    pos, mass, theta, eps, n_leaf = inputs.make(name)
+    with B.TreeCode(n_group=64) as tc:
+        tc.set_option("device_build", 1)
+        tc.set_particles(pos, mass)
+        tc.build(n_leaf)
+        acc, pot = tc.forces(theta, eps)
+        n_pc, n_pp = tc.counts()
+    check(acc, pot, n_pc, n_pp, Oracle(pos, mass, n_leaf, 64).forces(theta, eps, shadow32=True))
+
+
+def test_device_build_is_faster_than_host_build_1m():
+    pos, mass, theta, eps, n_leaf = inputs.make("plummer_1m")
+    t = {}
+    for dev in (0, 1):
+        with B.TreeCode() as tc:
+            tc.set_option("device_build", dev)
+            tc.set_particles(pos, mass)
+            ts = []
+            for _ in range(4):
+                tc.build(n_leaf)
+                ts.append(tc.stats()["t_host_ms"] + tc.stats()["t_copy_ms"])
+            t[dev] = min(ts[1:])
+    print(f"tc_build N=2^20: host {t[0]:.2f} ms (build + copy), device {t[1]:.2f} ms")
+    assert t[1] < t[0]
