@@ -43,6 +43,9 @@ struct tc_ctx {
   bool forces_done = false, timing_pending = false;
   tc::DeviceBuildScratch dscr;
   bool tree_host_valid = false;       // the host copy of the packed tree (tc_get_tree) is current
+  bool host_particles_valid = false;  // pos/mass below hold the current particles (else only d_src does)
+  float4* h_src = nullptr; int64_t h_src_cap = 0;     // pinned staging of (x,y,z,m) for the device build
+  unsigned int* d_flags = nullptr;
   // tc_direct scratch
   float4* d_src = nullptr; int64_t src_cap = 0; bool src_valid = false;
   long long* d_tgt = nullptr; double* d_dacc = nullptr; double* d_dpot = nullptr; int64_t tgt_cap = 0;
@@ -104,9 +107,28 @@ int collect(tc_ctx* c) {
   return TC_OK;
 }
 
+// the host copy of the particles (host build, first use after a device-only tc_set_particles)
+int ensure_host_particles(tc_ctx* c) {
+  if (c->host_particles_valid) return TC_OK;
+  if (!c->src_valid) return fail(c, TC_ESTATE, "no particles");
+  const int64_t n = c->n;
+  std::vector<float4> h;
+  try { h.resize((size_t)n); c->pos.resize((size_t)n * 3); c->mass.resize((size_t)n); } catch (...) { return fail(c, TC_ENOMEM, "out of host memory"); }
+  TC_CUDA(c, cudaMemcpyAsync(h.data(), c->d_src, sizeof(float4) * (size_t)n, cudaMemcpyDeviceToHost, c->stream));
+  TC_CUDA(c, cudaStreamSynchronize(c->stream));
+#pragma omp parallel for schedule(static)
+  for (int64_t i = 0; i < n; i++) {
+    c->pos[3 * (size_t)i] = h[(size_t)i].x; c->pos[3 * (size_t)i + 1] = h[(size_t)i].y; c->pos[3 * (size_t)i + 2] = h[(size_t)i].z;
+    c->mass[(size_t)i] = h[(size_t)i].w;
+  }
+  c->host_particles_valid = true;
+  return TC_OK;
+}
+
 // (x, y, z, m) of the caller's particles as one float4 array on the device (tc_direct, device build)
 int ensure_src(tc_ctx* c) {
   if (c->src_valid) return TC_OK;
+  { const int rc = ensure_host_particles(c); if (rc != TC_OK) return rc; }
   const int64_t n = c->n;
   if (c->src_cap < n) {
     cudaFree(c->d_src); c->d_src = nullptr; c->src_cap = 0;
@@ -166,6 +188,8 @@ void tc_destroy(tc_ctx* c) {
     cudaFree(c->d_tree); cudaFree(c->d_acc); cudaFree(c->d_pot); cudaFree(c->d_npc); cudaFree(c->d_npp);
     cudaFree(c->d_ctr); cudaFree(c->d_spill);
     c->dscr.release();
+    if (c->h_src) cudaFreeHost(c->h_src);
+    cudaFree(c->d_flags);
     cudaFree(c->d_src); cudaFree(c->d_tgt); cudaFree(c->d_dacc); cudaFree(c->d_dpot);
     if (c->ev0) cudaEventDestroy(c->ev0);
     if (c->ev1) cudaEventDestroy(c->ev1);
@@ -214,23 +238,62 @@ int tc_set_particles(tc_ctx* c, const float* pos, const float* mass, int64_t n) 
   if (!c) return TC_EINVAL;
   if (!pos || !mass) return fail(c, TC_EINVAL, "tc_set_particles: null pointer");
   if (n < 1 || n > 2147483647LL) return fail(c, TC_EINVAL, "tc_set_particles: n must be in [1, 2^31-1]");
-  c->built = false; c->forces_done = false; c->src_valid = false;
+  c->built = false; c->forces_done = false; c->src_valid = false; c->host_particles_valid = false;
+  c->n = 0;
+  const bool pos_dev = is_device_ptr(c, pos), mass_dev = is_device_ptr(c, mass);
+  const bool dev_mode = c->device_build && !c->host_only;
+  if (dev_mode) {
+    if (c->src_cap < n) {
+      TC_CUDA(c, cudaStreamSynchronize(c->stream));
+      cudaFree(c->d_src); c->d_src = nullptr; c->src_cap = 0;
+      TC_CUDA(c, cudaMalloc((void**)&c->d_src, sizeof(float4) * (size_t)n));
+      c->src_cap = n;
+    }
+    if (!c->d_flags) TC_CUDA(c, cudaMalloc((void**)&c->d_flags, sizeof(unsigned int)));
+  }
+  if (dev_mode && pos_dev && mass_dev) {
+    // device inputs, device build: nothing travels; interleave + validate in one kernel
+    const int le = tc::pack_src_device(pos, mass, n, c->d_src, c->d_flags, c->stream);
+    if (le != 0) return cuda_fail(c, (cudaError_t)le, "tc_set_particles: pack kernel");
+    unsigned int flags = 0;
+    TC_CUDA(c, cudaMemcpyAsync(&flags, c->d_flags, sizeof(flags), cudaMemcpyDeviceToHost, c->stream));
+    TC_CUDA(c, cudaStreamSynchronize(c->stream));
+    if (flags & 1u) return fail(c, TC_EINVAL, "tc_set_particles: non-finite position");
+    if (flags & 2u) return fail(c, TC_EINVAL, "tc_set_particles: negative or non-finite mass");
+    c->src_valid = true;
+    c->n = n;
+    return TC_OK;
+  }
   try { c->pos.resize((size_t)n * 3); c->mass.resize((size_t)n); } catch (...) { return fail(c, TC_ENOMEM, "tc_set_particles: out of host memory"); }
-  if (is_device_ptr(c, pos)) { TC_CUDA(c, cudaMemcpyAsync(c->pos.data(), pos, sizeof(float) * 3 * (size_t)n, cudaMemcpyDeviceToHost, c->stream)); }
-  else std::memcpy(c->pos.data(), pos, sizeof(float) * 3 * (size_t)n);
-  if (is_device_ptr(c, mass)) { TC_CUDA(c, cudaMemcpyAsync(c->mass.data(), mass, sizeof(float) * (size_t)n, cudaMemcpyDeviceToHost, c->stream)); }
-  else std::memcpy(c->mass.data(), mass, sizeof(float) * (size_t)n);
-  if (!c->host_only) TC_CUDA(c, cudaStreamSynchronize(c->stream));
+  const float* P = pos; const float* M = mass;      // where the validation pass reads from
+  if (pos_dev) { TC_CUDA(c, cudaMemcpyAsync(c->pos.data(), pos, sizeof(float) * 3 * (size_t)n, cudaMemcpyDeviceToHost, c->stream)); P = c->pos.data(); }
+  if (mass_dev) { TC_CUDA(c, cudaMemcpyAsync(c->mass.data(), mass, sizeof(float) * (size_t)n, cudaMemcpyDeviceToHost, c->stream)); M = c->mass.data(); }
+  if (!c->host_only) TC_CUDA(c, cudaStreamSynchronize(c->stream));   // also: h_src of the previous call is no longer in flight
+  if (dev_mode && c->h_src_cap < n) {
+    if (c->h_src) cudaFreeHost(c->h_src);
+    c->h_src = nullptr; c->h_src_cap = 0;
+    TC_CUDA(c, cudaHostAlloc((void**)&c->h_src, sizeof(float4) * (size_t)n, cudaHostAllocDefault));
+    c->h_src_cap = n;
+  }
+  // one pass: copy into the context, validate, and (device build) stage (x,y,z,m) in pinned memory
   bool bad_pos = false, bad_mass = false;
-  const float* P = c->pos.data(); const float* M = c->mass.data();
+  float* CP = c->pos.data(); float* CM = c->mass.data();
+  float4* H = dev_mode ? c->h_src : nullptr;
 #pragma omp parallel for schedule(static) reduction(| : bad_pos, bad_mass)
   for (int64_t i = 0; i < n; i++) {
-    bad_pos |= !(std::isfinite(P[3 * i]) && std::isfinite(P[3 * i + 1]) && std::isfinite(P[3 * i + 2]));
-    bad_mass |= !(std::isfinite(M[i]) && M[i] >= 0.f);
+    const float x = P[3 * i], y = P[3 * i + 1], z = P[3 * i + 2], m = M[i];
+    CP[3 * i] = x; CP[3 * i + 1] = y; CP[3 * i + 2] = z; CM[i] = m;
+    if (H) H[i] = make_float4(x, y, z, m);
+    bad_pos |= !(std::isfinite(x) && std::isfinite(y) && std::isfinite(z));
+    bad_mass |= !(std::isfinite(m) && m >= 0.f);
   }
-  c->n = 0;
   if (bad_pos) return fail(c, TC_EINVAL, "tc_set_particles: non-finite position");
   if (bad_mass) return fail(c, TC_EINVAL, "tc_set_particles: negative or non-finite mass");
+  c->host_particles_valid = true;
+  if (dev_mode) {     // stream-ordered: tc_build runs on the same stream
+    TC_CUDA(c, cudaMemcpyAsync(c->d_src, c->h_src, sizeof(float4) * (size_t)n, cudaMemcpyHostToDevice, c->stream));
+    c->src_valid = true;
+  }
   c->n = n;
   return TC_OK;
 }
@@ -257,6 +320,7 @@ int tc_build(tc_ctx* c, int n_leaf) {
     c->built = true;
     return TC_OK;
   }
+  { const int rc0 = ensure_host_particles(c); if (rc0 != TC_OK) return rc0; }
   const double t0 = now_ms();
   std::string msg;
   const int rc = tc::build_host_tree(c->pos.data(), c->mass.data(), c->n, n_leaf, c->n_group, c->tree, packed_alloc, c, msg);

@@ -294,6 +294,25 @@ inline unsigned blocks(long long n, int t = 256) { return (unsigned)((n + t - 1)
 
 }  // namespace
 
+// tc_set_particles with device inputs in device-build mode: interleave + validate on the device
+__global__ void k_pack_src(const float* __restrict__ pos, const float* __restrict__ mass, long long n, float4* __restrict__ out,
+                           unsigned int* __restrict__ flags) {
+  const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  const float x = pos[3 * i], y = pos[3 * i + 1], z = pos[3 * i + 2], m = mass[i];
+  out[i] = make_float4(x, y, z, m);
+  if (!(isfinite(x) && isfinite(y) && isfinite(z))) atomicOr(flags, 1u);
+  if (!(isfinite(m) && m >= 0.f)) atomicOr(flags, 2u);
+}
+
+int pack_src_device(const float* pos, const float* mass, int64_t n, float4* out, unsigned int* flags, void* stream) {
+  cudaStream_t st = (cudaStream_t)stream;
+  cudaError_t e = cudaMemsetAsync(flags, 0, sizeof(unsigned int), st);
+  if (e != cudaSuccess) return (int)e;
+  k_pack_src<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(pos, mass, n, out, flags);
+  return (int)cudaGetLastError();
+}
+
 // ---- scratch management -------------------------------------------------------------------------
 template <typename T>
 static int grow(T*& p, size_t& cap, size_t need, bool keep, cudaStream_t st, std::string& msg) {

@@ -119,6 +119,10 @@ struct DeviceBuildScratch {
 int build_device_tree(const float4* src, int64_t n, int n_leaf, int n_group, DeviceBuildScratch& S, void** d_tree,
                       size_t* d_tree_cap, HostTree& T, DeviceTree& D, void* stream, std::string& msg);
 
+// pos [n,3], mass [n] DEVICE -> out [n] (x,y,z,m); flags[0] bit 0: non-finite position, bit 1: bad mass.
+// Returns a cudaError_t as int.
+int pack_src_device(const float* pos, const float* mass, int64_t n, float4* out, unsigned int* flags, void* stream);
+
 // Direct summation (tc_direct): src [n] (x,y,z,m) device, targets device int64 [n_t] or nullptr (all),
 // acc [n_t,3] / pot [n_t] device fp64 (zeroed inside).  Returns a cudaError_t as int.
 int launch_direct(const float4* src, long long n, const long long* targets, long long n_t, float eps, double* acc,

@@ -103,3 +103,50 @@ def test_device_build_is_faster_than_host_build_1m():
             t[dev] = min(ts[1:])
     print(f"tc_build N=2^20: host {t[0]:.2f} ms (build + copy), device {t[1]:.2f} ms")
     assert t[1] < t[0]
+
+
+def test_device_inputs_device_build_leapfrog_matches_host_build():
+    """Device pointers + device build: nothing crosses PCIe per step; the trajectory equals the host-build one."""
+    import torch
+    from paper_1005_5384_b200 import integrate
+    pos, mass, vel = inputs.two_plummer(1 << 18, with_velocities=True)
+    logs = []
+    for dev in (0, 1):
+        st = torch.cuda.Stream()
+        with torch.cuda.stream(st), B.TreeCode() as tc:
+            tc.set_option("device_build", dev)
+            tc.set_stream(st.cuda_stream)
+            d_pos, d_vel, d_mass = torch.from_numpy(pos).cuda(), torch.from_numpy(vel).cuda(), torch.from_numpy(mass).cuda()
+            logs.append(integrate.leapfrog_kdk(tc, d_pos, d_vel, d_mass, 1.0 / 128, 3, 0.5, 0.005, 16))
+            x_end = d_pos.cpu().numpy()
+        logs[-1].append(x_end)
+    (h, d) = logs
+    assert np.abs(h[-1] - d[-1]).max() <= 1e-6                     # same positions after 3 steps
+    for a, b in zip(h[:-1], d[:-1]):
+        assert a["interactions"] == b["interactions"]              # identical trees -> identical lists
+        assert abs(a["E"] - b["E"]) <= 1e-7 * abs(a["E"])
+    print(f"leapfrog N=2^18: per-step build host {np.mean([r['t_host_ms'] + r['t_copy_ms'] for r in h[1:-1]]):.2f} ms, "
+          f"device {np.mean([r['t_host_ms'] for r in d[1:-1]]):.2f} ms")
+
+
+def test_device_build_rejects_bad_particles_and_switches_back_to_host():
+    import torch
+    pos, mass, *_ = inputs.make("plummer_1k")
+    with B.TreeCode() as tc:
+        tc.set_option("device_build", 1)
+        bad = torch.from_numpy(pos).cuda().clone()
+        bad[5, 1] = float("nan")
+        with pytest.raises(B.TcError) as e:
+            tc.set_particles(bad, torch.from_numpy(mass).cuda())
+        assert e.value.code == B.TC_EINVAL
+        badm = mass.copy(); badm[7] = -1.0
+        with pytest.raises(B.TcError) as e:
+            tc.set_particles(pos, badm)
+        assert e.value.code == B.TC_EINVAL
+        # device-only particles, then a HOST build: the host copy is fetched from the device
+        tc.set_particles(torch.from_numpy(pos).cuda(), torch.from_numpy(mass).cuda())
+        tc.set_option("device_build", 0)
+        tc.build(16)
+        acc, pot = tc.forces(0.5, 0.01)
+        n_pc, n_pp = tc.counts()
+    check(acc, pot, n_pc, n_pp, Oracle(pos, mass, 16, 96).forces(0.5, 0.01, shadow32=True))
