@@ -218,6 +218,19 @@ def run_ours(args) -> None:
         t_dev_ms = float(sum(per_step))                # device time of exactly K steps
         st = tc.stats()
 
+        # ---- the paper's second metric: data rate of the tree walk alone (A1-A3), lists dropped
+        tc.set_option("walk_only", 1)
+        walk_ms = []
+        for i in range(5):
+            flush.zero_()
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a.record(stream); step(); b.record(stream)
+            torch.cuda.synchronize()
+            walk_ms.append(a.elapsed_time(b))
+        tc.set_option("walk_only", 0)
+        tc.sync()
+        walk_ms = float(np.median(walk_ms[1:]))
+
         # ---- e2e: host buffers through the C ABI, every step: set_particles + build + forces
         h_pos = torch.from_numpy(pos).pin_memory().numpy()
         h_mass = torch.from_numpy(mass).pin_memory().numpy()
@@ -290,6 +303,9 @@ def run_ours(args) -> None:
                                    / (kernel_ms * 1e-3) / 1e9,
         "ms_per_step_min": float(min(per_step)), "ms_per_step_median": float(np.median(per_step)),
         "wall_ms_per_step_incl_flush": t_wall * 1e3 / K,
+        "walk": {"ms": walk_ms, "bytes_per_test": 64, "gb_per_s": 64.0 * st["n_tests_total"] / (walk_ms * 1e-3) / 1e9,
+                 "what": "option walk_only: walk + list building without evaluation; 4 float4 loads per opening test "
+                         "(L2-resident tree); the paper reports > 50 GB/s for its count pass on G80 (PAPER.md:177)"},
         "gpu_launches": K,
         "clocks": clocks,
         "e2e": {"value": inter_all / e2e_s, "unit": "interactions/s", "h2d_bytes_per_step": int(tree_bytes),

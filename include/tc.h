@@ -108,6 +108,10 @@ int tc_forces(tc_ctx* ctx, float theta, float eps, float* acc, float* pot);
  *                 construction on the GPU (tc_build_gpu.cu) and writes the packed tree in device memory —
  *                 no bulk H2D; t_host_ms of tc_stats is then the wall time of the device build, t_copy_ms 0.
  *                 Cells, boundary cubes, groups and counts are identical to the host build's.
+ *   "walk_only"   measurement aid, 0 (default) or 1: tc_forces walks the tree and builds every interaction
+ *                 list (A1-A3) but skips their evaluation; acc and pot are then ZERO, counts and
+ *                 n_tests_total are valid.  bench.py uses it to report the paper's second metric, the
+ *                 data rate of the tree walk.
  *   "stack_smem"  walk-stack entries kept in shared memory per warp before
  *                 spilling to global memory: 256 (default) or 64 (test of the
  *                 spill path)

@@ -26,6 +26,7 @@ struct tc_ctx {
   int n_group = 96;
   bool device_build = false;          // option "device_build": tc_build_gpu.cu instead of tc_build.cpp
   int stack_smem = 256;
+  int walk_only = 0;
   // particles (host copy, caller order)
   std::vector<float> pos, mass;
   int64_t n = 0;
@@ -212,6 +213,10 @@ int tc_set_option(tc_ctx* c, const char* key, double v) {
     if (c->host_only && v != 0.0) return fail(c, TC_ESTATE, "tc_set_option: device_build needs a device");
     c->device_build = (v != 0.0); return TC_OK;
   }
+  if (!std::strcmp(key, "walk_only")) {
+    if (v != 0.0 && v != 1.0) return fail(c, TC_EINVAL, "tc_set_option: walk_only must be 0 or 1");
+    c->walk_only = (int)v; return TC_OK;
+  }
   if (!std::strcmp(key, "stack_smem")) {
     if (v != 256.0 && v != 64.0) return fail(c, TC_EINVAL, "tc_set_option: stack_smem must be 256 or 64");
     c->stack_smem = (int)v; return TC_OK;
@@ -388,7 +393,7 @@ int tc_forces(tc_ctx* c, float theta, float eps, float* acc, float* pot) {
   L.acc = acc_dev ? acc : c->d_acc;
   L.pot = pot ? (acc_dev ? pot : c->d_pot) : nullptr;
   L.n_pc = c->d_npc; L.n_pp = c->d_npp; L.counters = c->d_ctr; L.spill = c->d_spill; L.spill_cap = c->spill_cap;
-  L.stack_smem = c->stack_smem; L.n_sm = c->n_sm;
+  L.stack_smem = c->stack_smem; L.n_sm = c->n_sm; L.walk_only = c->walk_only;
   // stream-ordered: no host synchronisation between queued calls; the overflow flag is sticky until collect()
   TC_CUDA(c, cudaMemsetAsync(c->d_ctr, 0, offsetof(tc::DeviceCounters, overflow), c->stream));
   TC_CUDA(c, cudaEventRecord(c->ev0, c->stream));

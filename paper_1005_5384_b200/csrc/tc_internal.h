@@ -84,6 +84,7 @@ struct ForceLaunch {
   uint32_t* spill = nullptr;  // device [n_warps_total * spill_cap]
   int spill_cap = 0;
   int stack_smem = 256;
+  int walk_only = 0;          // measurement aid: walk and build the lists, skip their evaluation
   int n_sm = 148;
 };
 

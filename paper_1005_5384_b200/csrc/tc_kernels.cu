@@ -275,7 +275,7 @@ forces_kernel(const float4* __restrict__ bnd, const float4* __restrict__ xm, con
               const int4* __restrict__ grp, int n_groups, float theta, float eps,
               float* __restrict__ acc, float* __restrict__ pot, int32_t* __restrict__ out_npc,
               int32_t* __restrict__ out_npp, DeviceCounters* __restrict__ ctr, uint32_t* __restrict__ spill_all,
-              int spill_cap) {
+              int spill_cap, int walk_only) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   WarpSmem<STK>& sm = reinterpret_cast<WarpSmem<STK>*>(smem_raw)[warp];
@@ -408,13 +408,14 @@ forces_kernel(const float4* __restrict__ bnd, const float4* __restrict__ xm, con
         __syncwarp();
         const bool flush_leaves = lq > kLeafQCap - 32;
         if (ccnt > kCellCap - 32 || (flush_leaves && ccnt)) {
-          eval_cells(sm.u.cell, ccnt, eps2, L, P, A); ccnt = 0; __syncwarp();
+          if (!walk_only) eval_cells(sm.u.cell, ccnt, eps2, L, P, A);
+          ccnt = 0; __syncwarp();
         }
-        if (flush_leaves) { eval_leaves<kEps0>(sm.u.bs, sm.leafq, lq, part, eps2, L, P, A, lane); lq = 0; }
+        if (flush_leaves) { if (!walk_only) eval_leaves<kEps0>(sm.u.bs, sm.leafq, lq, part, eps2, L, P, A, lane); lq = 0; }
       }
-      if (ccnt) eval_cells(sm.u.cell, ccnt, eps2, L, P, A);
+      if (ccnt && !walk_only) eval_cells(sm.u.cell, ccnt, eps2, L, P, A);
       __syncwarp();
-      if (lq) eval_leaves<kEps0>(sm.u.bs, sm.leafq, lq, part, eps2, L, P, A, lane);
+      if (lq && !walk_only) eval_leaves<kEps0>(sm.u.bs, sm.leafq, lq, part, eps2, L, P, A, lane);
       __syncwarp();
 
       // ---- A6: reduce the slices of every particle, write back in the caller's order
@@ -467,7 +468,7 @@ int launch_t(const DeviceTree& T, const ForceLaunch& L, cudaStream_t st, int* ct
   const int grid = L.n_sm * per_sm;
   kern<<<grid, kWarpsPerCta * 32, smem, st>>>(T.bnd, T.xm, T.q0, T.q1, T.part, T.orig, T.grp, (int)T.n_groups,
                                                L.theta, L.eps, L.acc, L.pot, L.n_pc, L.n_pp, L.counters, L.spill,
-                                               L.spill_cap);
+                                               L.spill_cap, L.walk_only);
   return (int)cudaGetLastError();
 }
 
