@@ -65,6 +65,12 @@ typedef struct tc_stats {
   double t_gpu_ms;        /* last tc_forces: device time of the force kernel(s),
                              CUDA events on the context's stream                  */
   int64_t tree_bytes;     /* bytes of the single bulk H2D copy of tc_build        */
+  /* option "two_pass" only (0 otherwise): the paper's kernels timed one by one   */
+  double t_walk_count_ms; /* walk pass 1 (count) + scan of the list sizes + list allocation         */
+  double t_walk_write_ms; /* walk pass 2 (write the lists to global memory)                         */
+  double t_node_ms;       /* body-node evaluation kernel (List 3)                                   */
+  double t_leaf_ms;       /* body-leaf evaluation kernel (List 4)                                   */
+  int64_t list_bytes;     /* bytes of the global interaction lists                                  */
 } tc_stats;
 
 /* Select the current CUDA device, create the context and its stream.
@@ -108,6 +114,10 @@ int tc_forces(tc_ctx* ctx, float theta, float eps, float* acc, float* pot);
  *                 construction on the GPU (tc_build_gpu.cu) and writes the packed tree in device memory —
  *                 no bulk H2D; t_host_ms of tc_stats is then the wall time of the device build, t_copy_ms 0.
  *                 Cells, boundary cubes, groups and counts are identical to the host build's.
+ *   "two_pass"    0 (default: the fused kernel) or 1: the paper-literal pipeline —
+ *                 walk-count kernel, scan of the list sizes, walk-write kernel (lists in global memory),
+ *                 body-node kernel, body-leaf kernel; same lists, same counts, same results up to
+ *                 summation order; an A/B against the fused design, timed per kernel in tc_stats.
  *   "walk_only"   measurement aid, 0 (default) or 1: tc_forces walks the tree and builds every interaction
  *                 list (A1-A3) but skips their evaluation; acc and pot are then ZERO, counts and
  *                 n_tests_total are valid.  bench.py uses it to report the paper's second metric, the

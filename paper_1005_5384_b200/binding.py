@@ -34,7 +34,9 @@ class tc_stats(C.Structure):
                 ("depth", C.c_int32), ("n_leaf", C.c_int32), ("n_group", C.c_int32), ("reserved", C.c_int32),
                 ("n_pc_total", C.c_int64), ("n_pp_total", C.c_int64), ("n_tests_total", C.c_int64),
                 ("n_spills", C.c_int64), ("t_host_ms", C.c_double), ("t_copy_ms", C.c_double),
-                ("t_gpu_ms", C.c_double), ("tree_bytes", C.c_int64)]
+                ("t_gpu_ms", C.c_double), ("tree_bytes", C.c_int64),
+                ("t_walk_count_ms", C.c_double), ("t_walk_write_ms", C.c_double), ("t_node_ms", C.c_double),
+                ("t_leaf_ms", C.c_double), ("list_bytes", C.c_int64)]
 
     def asdict(self):
         return {k: getattr(self, k) for k, _ in self._fields_ if k != "reserved"}

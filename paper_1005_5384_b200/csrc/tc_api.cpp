@@ -27,6 +27,9 @@ struct tc_ctx {
   bool device_build = false;          // option "device_build": tc_build_gpu.cu instead of tc_build.cpp
   int stack_smem = 256;
   int walk_only = 0;
+  bool two_pass = false;
+  tc::TwoPassScratch tps;
+  bool last_two_pass = false;
   // particles (host copy, caller order)
   std::vector<float> pos, mass;
   int64_t n = 0;
@@ -99,6 +102,14 @@ int collect(tc_ctx* c) {
   float ms = 0.f;
   TC_CUDA(c, cudaEventElapsedTime(&ms, c->ev0, c->ev1));
   c->stats.t_gpu_ms = ms;
+  c->stats.t_walk_count_ms = c->stats.t_walk_write_ms = c->stats.t_node_ms = c->stats.t_leaf_ms = 0.0; c->stats.list_bytes = 0;
+  if (c->last_two_pass) {
+    float t4[4];
+    if (tc::two_pass_times(c->tps, t4) == 0) {
+      c->stats.t_walk_count_ms = t4[0]; c->stats.t_walk_write_ms = t4[1]; c->stats.t_node_ms = t4[2]; c->stats.t_leaf_ms = t4[3];
+    } else cudaGetLastError();
+    c->stats.list_bytes = (int64_t)(4 * c->tps.n_list_cells + 8 * c->tps.n_list_leaves);
+  }
   c->stats.n_pc_total = (int64_t)h.n_pc_total; c->stats.n_pp_total = (int64_t)h.n_pp_total;
   c->stats.n_tests_total = (int64_t)h.n_tests_total; c->stats.n_spills = (int64_t)h.n_spills;
   if (h.overflow) {
@@ -189,6 +200,7 @@ void tc_destroy(tc_ctx* c) {
     cudaFree(c->d_tree); cudaFree(c->d_acc); cudaFree(c->d_pot); cudaFree(c->d_npc); cudaFree(c->d_npp);
     cudaFree(c->d_ctr); cudaFree(c->d_spill);
     c->dscr.release();
+    c->tps.release();
     if (c->h_src) cudaFreeHost(c->h_src);
     cudaFree(c->d_flags);
     cudaFree(c->d_src); cudaFree(c->d_tgt); cudaFree(c->d_dacc); cudaFree(c->d_dpot);
@@ -212,6 +224,10 @@ int tc_set_option(tc_ctx* c, const char* key, double v) {
     if (v != 0.0 && v != 1.0) return fail(c, TC_EINVAL, "tc_set_option: device_build must be 0 or 1");
     if (c->host_only && v != 0.0) return fail(c, TC_ESTATE, "tc_set_option: device_build needs a device");
     c->device_build = (v != 0.0); return TC_OK;
+  }
+  if (!std::strcmp(key, "two_pass")) {
+    if (v != 0.0 && v != 1.0) return fail(c, TC_EINVAL, "tc_set_option: two_pass must be 0 or 1");
+    c->two_pass = (v != 0.0); return TC_OK;
   }
   if (!std::strcmp(key, "walk_only")) {
     if (v != 0.0 && v != 1.0) return fail(c, TC_EINVAL, "tc_set_option: walk_only must be 0 or 1");
@@ -394,11 +410,13 @@ int tc_forces(tc_ctx* c, float theta, float eps, float* acc, float* pot) {
   L.pot = pot ? (acc_dev ? pot : c->d_pot) : nullptr;
   L.n_pc = c->d_npc; L.n_pp = c->d_npp; L.counters = c->d_ctr; L.spill = c->d_spill; L.spill_cap = c->spill_cap;
   L.stack_smem = c->stack_smem; L.n_sm = c->n_sm; L.walk_only = c->walk_only;
+  L.max_grid = (int)(warps / (size_t)tc::forces_warps_per_cta());
   // stream-ordered: no host synchronisation between queued calls; the overflow flag is sticky until collect()
   TC_CUDA(c, cudaMemsetAsync(c->d_ctr, 0, offsetof(tc::DeviceCounters, overflow), c->stream));
   TC_CUDA(c, cudaEventRecord(c->ev0, c->stream));
-  const int le = tc::launch_forces(c->dview, L, c->stream);
+  const int le = c->two_pass ? tc::launch_forces_two_pass(c->dview, L, c->tps, c->stream) : tc::launch_forces(c->dview, L, c->stream);
   if (le != 0) return cuda_fail(c, (cudaError_t)le, "forces kernel launch");
+  c->last_two_pass = c->two_pass;
   TC_CUDA(c, cudaEventRecord(c->ev1, c->stream));
   c->timing_pending = true; c->forces_done = true;
   if (!acc_dev) {

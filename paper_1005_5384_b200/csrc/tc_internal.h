@@ -86,13 +86,30 @@ struct ForceLaunch {
   int stack_smem = 256;
   int walk_only = 0;          // measurement aid: walk and build the lists, skip their evaluation
   int n_sm = 148;
+  int max_grid = 0;           // CTAs the spill buffer has room for (0: no limit)
 };
 
 // Launches the fused walk+evaluate kernel on `stream` (a cudaStream_t).  Returns a
 // cudaError_t as int (0 = success).  Defined in tc_kernels.cu.
 int launch_forces(const DeviceTree& T, const ForceLaunch& L, void* stream);
+// Two-pass variant (option "two_pass"): global interaction lists and their scratch, owned by the context.
+struct TwoPassScratch {
+  unsigned long long *cnt_c = nullptr, *cnt_l = nullptr, *off_c = nullptr, *off_l = nullptr;
+  size_t cap_cnt_c = 0, cap_cnt_l = 0, cap_off_c = 0, cap_off_l = 0;
+  int* leaf_bodies = nullptr;  size_t cap_lb = 0;
+  int* cells = nullptr;        size_t cap_cells = 0;
+  int2* leaves = nullptr;      size_t cap_leaves = 0;
+  char* tmp = nullptr;         size_t cap_tmp = 0;
+  void* ev[5] = {nullptr, nullptr, nullptr, nullptr, nullptr};   // cudaEvent_t
+  long long n_list_cells = 0, n_list_leaves = 0;
+  void release();
+};
+// count -> scan -> write lists -> node kernel -> leaf kernel.  cudaError_t as int.
+int launch_forces_two_pass(const DeviceTree& T, const ForceLaunch& L, TwoPassScratch& S, void* stream);
+int two_pass_times(const TwoPassScratch& S, float ms[4]);
 // Number of warps the persistent grid runs (for sizing the spill buffer).
 int forces_total_warps(int n_sm, int stack_smem);
+int forces_warps_per_cta();
 // Scratch of the device-side builder (tc_build_gpu.cu); grow-only, owned by the context.
 struct DeviceBuildScratch {
   unsigned long long *keys = nullptr, *keys_alt = nullptr;  size_t cap_keys = 0, cap_keys_alt = 0;

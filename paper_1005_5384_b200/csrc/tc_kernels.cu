@@ -25,6 +25,9 @@
 // No tensor cores: this is not a dense contraction.
 #include <cuda_runtime.h>
 
+#include <cub/device/device_scan.cuh>
+
+#include <algorithm>
 #include <cstdint>
 
 #include "tc_internal.h"
@@ -268,14 +271,82 @@ __device__ __forceinline__ void eval_leaves(BodyStage& bs, const int2* leafq, in
   }
 }
 
-template <int STK, bool kEps0>
+// Lane mapping, particle pairs and zeroed accumulators of one pass over particles [first, first + m)
+__device__ __forceinline__ void setup_pass(Lanes& L, Pos2 (&P)[kMaxKP], Acc2 (&A)[kMaxKP], const float4* __restrict__ part,
+                                           int first, int m, int lane) {
+  L.S = c_slices.S[m];
+  L.q = 32 / L.S;
+  L.kp = (m + 2 * L.q - 1) / (2 * L.q);
+  L.s = lane / L.q;
+  L.p = lane - L.s * L.q;
+  L.active = L.s < L.S;
+#pragma unroll
+  for (int j = 0; j < kMaxKP; j++) {
+    A[j].ax = A[j].ay = A[j].az = A[j].npot = 0ull;  // (+0.f, +0.f)
+    // slots beyond m compute on a copy of the pass's first particle; never written back
+    const int t0 = 2 * j * L.q + L.p, t1 = t0 + L.q;
+    const float4 m0 = __ldg(part + first + ((L.active && t0 < m) ? t0 : 0));
+    const float4 m1 = __ldg(part + first + ((L.active && t1 < m) ? t1 : 0));
+    // (+ 0 through FADD2: the pair is then the result of a real instruction and stays in one aligned
+    // register pair; a bare mov.b64 is re-materialised with two MOVs in front of every use)
+    P[j].x = add2(pk(m0.x, m1.x), bc(0.f)); P[j].y = add2(pk(m0.y, m1.y), bc(0.f));
+    P[j].z = add2(pk(m0.z, m1.z), bc(0.f));
+  }
+}
+
+// A6: reduce the slices of every particle, write back in the caller's order.
+// kAdd: add to what is already there (second evaluation kernel of the two-pass variant);
+// kSelf: the particles met themselves once in the particle-particle part (remove -m/eps again).
+template <bool kAdd, bool kSelf>
+__device__ __forceinline__ void write_back(const Lanes& L, const Acc2 (&A)[kMaxKP], const float4* __restrict__ part,
+                                           const int32_t* __restrict__ orig, int first, int m, float eps2, int lane,
+                                           float* __restrict__ acc, float* __restrict__ pot, int32_t* __restrict__ out_cnt,
+                                           int cnt_value, int32_t* __restrict__ out_cnt2 = nullptr, int cnt2_value = 0) {
+#pragma unroll
+  for (int j = 0; j < 2 * kMaxKP; j++) {
+    if (j >= 2 * L.kp) break;                        // warp-uniform
+    const Acc2& a2 = A[j >> 1];
+    float ax, ay, az, ph;
+    if (j & 1) { ax = hi(a2.ax); ay = hi(a2.ay); az = hi(a2.az); ph = -hi(a2.npot); }
+    else { ax = lo(a2.ax); ay = lo(a2.ay); az = lo(a2.az); ph = -lo(a2.npot); }
+    for (int w = 1; w < L.S; w <<= 1) {
+      const float ox = __shfl_down_sync(kFull, ax, w * L.q), oy = __shfl_down_sync(kFull, ay, w * L.q);
+      const float oz = __shfl_down_sync(kFull, az, w * L.q), op = __shfl_down_sync(kFull, ph, w * L.q);
+      if ((L.s % (2 * w)) == 0 && L.s + w < L.S) { ax += ox; ay += oy; az += oz; ph += op; }
+    }
+    const int tq = j * L.q + lane;
+    if (lane < L.q && tq < m) {
+      const int t = first + tq;
+      const int i = __ldg(orig + t);
+      if (kSelf) ph += __ldg(part + t).w * rsqrt_approx(eps2);     // the particle met itself once
+      float* a3 = acc + 3 * (size_t)i;
+      if (kAdd) { a3[0] += ax; a3[1] += ay; a3[2] += az; if (pot) pot[i] += ph; }
+      else { a3[0] = ax; a3[1] = ay; a3[2] = az; if (pot) pot[i] = ph; }
+      out_cnt[i] = cnt_value;
+      if (out_cnt2) out_cnt2[i] = cnt2_value;
+    }
+  }
+}
+
+// Global interaction lists of the paper-literal two-pass variant (count, scan, write).
+struct ListIO {
+  unsigned long long *cnt_c, *cnt_l;        // [n_groups]  pass 1: cells / opened-leaf ranges per group
+  const unsigned long long *off_c, *off_l;  // [n_groups + 1]  exclusive scans of the counts
+  int* cells;                       // cell ids
+  int2* leaves;                     // (first_body, n_body)
+  int* leaf_bodies;                 // [n_groups] bodies of the opened leaves (n_pp + 1)
+};
+
+enum { kFused = 0, kCount = 1, kWrite = 2 };
+
+template <int STK, bool kEps0, int MODE = kFused>
 __global__ void __launch_bounds__(kWarpsPerCta * 32, TC_MINB)
 forces_kernel(const float4* __restrict__ bnd, const float4* __restrict__ xm, const float4* __restrict__ q0,
               const float4* __restrict__ q1, const float4* __restrict__ part, const int32_t* __restrict__ orig,
               const int4* __restrict__ grp, int n_groups, float theta, float eps,
               float* __restrict__ acc, float* __restrict__ pot, int32_t* __restrict__ out_npc,
               int32_t* __restrict__ out_npp, DeviceCounters* __restrict__ ctr, uint32_t* __restrict__ spill_all,
-              int spill_cap, int walk_only) {
+              int spill_cap, int walk_only, ListIO lio) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   WarpSmem<STK>& sm = reinterpret_cast<WarpSmem<STK>*>(smem_raw)[warp];
@@ -304,34 +375,22 @@ forces_kernel(const float4* __restrict__ bnd, const float4* __restrict__ xm, con
     for (int pb = 0; pb < G.z; pb += kPass) {
       const int m = min(kPass, G.z - pb);
       Lanes L;
-      L.S = c_slices.S[m];
-      L.q = 32 / L.S;
-      L.kp = (m + 2 * L.q - 1) / (2 * L.q);
-      L.s = lane / L.q;
-      L.p = lane - L.s * L.q;
-      L.active = L.s < L.S;
       Pos2 P[kMaxKP];
       Acc2 A[kMaxKP];
-#pragma unroll
-      for (int j = 0; j < kMaxKP; j++) {
-        A[j].ax = A[j].ay = A[j].az = A[j].npot = 0ull;  // (+0.f, +0.f)
-        // slots beyond m compute on a copy of the pass's first particle; never written back
-        const int t0 = 2 * j * L.q + L.p, t1 = t0 + L.q;
-        const float4 m0 = __ldg(part + G.y + pb + ((L.active && t0 < m) ? t0 : 0));
-        const float4 m1 = __ldg(part + G.y + pb + ((L.active && t1 < m) ? t1 : 0));
-        // (+ 0 through FADD2: the pair is then the result of a real instruction and stays in one aligned
-        // register pair; a bare mov.b64 is re-materialised with two MOVs in front of every use)
-        P[j].x = add2(pk(m0.x, m1.x), bc(0.f)); P[j].y = add2(pk(m0.y, m1.y), bc(0.f));
-        P[j].z = add2(pk(m0.z, m1.z), bc(0.f));
-      }
+      if (MODE == kFused) setup_pass(L, P, A, part, G.y + pb, m, lane);
+      unsigned long long woff_c = 0, woff_l = 0;         // MODE kWrite: where this group's lists start
+      if (MODE == kWrite) { woff_c = lio.off_c[g]; woff_l = lio.off_l[g]; }
 
       int ssz = 0, spill_sz = 0, ccnt = 0, lq = 0;
       long long n_pc = 0, n_pp = 0, n_tests = 0;
-      int n_spills = 0;
+      int n_spills = 0, n_lr = 0;                        // n_lr: opened-leaf ranges so far
       bool overflow = false;
       if (root_leaf) {
-        if (lane == 0) sm.leafq[0] = make_int2(root_a, root_n);
-        lq = 1; n_pp = root_n;
+        if (lane == 0) {
+          if (MODE == kFused) sm.leafq[0] = make_int2(root_a, root_n);
+          else if (MODE == kWrite) lio.leaves[woff_l] = make_int2(root_a, root_n);
+        }
+        lq = 1; n_lr = 1; n_pp = root_n;
       } else {
         if (lane == 0) sm.stack[0] = ((uint32_t)root_a << 3) | (uint32_t)(root_n - 1);
         ssz = 1;
@@ -373,13 +432,21 @@ forces_kernel(const float4* __restrict__ bnd, const float4* __restrict__ xm, con
         const unsigned m_stack = __ballot_sync(kFull, to_stack);
         n_tests += __popc(__ballot_sync(kFull, valid));
         if (to_cell) {                                   // not opened (leaf or node): multipole (R2)
-          CellRec& r = sm.u.cell[ccnt + __popc(m_cell & lt_mask)];
-          r.xm = cx; r.q0 = c0; r.q1 = make_float2(c1.x, c1.y);
+          if (MODE == kFused) {
+            CellRec& r = sm.u.cell[ccnt + __popc(m_cell & lt_mask)];
+            r.xm = cx; r.q0 = c0; r.q1 = make_float2(c1.x, c1.y);
+          } else if (MODE == kWrite) {
+            lio.cells[woff_c + (unsigned long long)(n_pc + __popc(m_cell & lt_mask))] = c;
+          }
         }
-        ccnt += __popc(m_cell); n_pc += __popc(m_cell);
+        if (MODE == kFused) ccnt += __popc(m_cell);
+        n_pc += __popc(m_cell);
         if (m_leaf) {                                    // opened leaf: particle-particle
-          if (to_leaf) sm.leafq[lq + __popc(m_leaf & lt_mask)] = make_int2(la, lb);
-          lq += __popc(m_leaf);
+          if (to_leaf) {
+            if (MODE == kFused) sm.leafq[lq + __popc(m_leaf & lt_mask)] = make_int2(la, lb);
+            else if (MODE == kWrite) lio.leaves[woff_l + (unsigned long long)(n_lr + __popc(m_leaf & lt_mask))] = make_int2(la, lb);
+          }
+          if (MODE == kFused) lq += __popc(m_leaf); else n_lr += __popc(m_leaf);
           n_pp += __reduce_add_sync(kFull, to_leaf ? lb : 0);
         }
         if (m_stack) {                                   // opened node: walk on
@@ -406,6 +473,7 @@ forces_kernel(const float4* __restrict__ bnd, const float4* __restrict__ xm, con
           ssz += npush;
         }
         __syncwarp();
+        if (MODE != kFused) continue;
         const bool flush_leaves = lq > kLeafQCap - 32;
         if (ccnt > kCellCap - 32 || (flush_leaves && ccnt)) {
           if (!walk_only) eval_cells(sm.u.cell, ccnt, eps2, L, P, A);
@@ -413,49 +481,116 @@ forces_kernel(const float4* __restrict__ bnd, const float4* __restrict__ xm, con
         }
         if (flush_leaves) { if (!walk_only) eval_leaves<kEps0>(sm.u.bs, sm.leafq, lq, part, eps2, L, P, A, lane); lq = 0; }
       }
-      if (ccnt && !walk_only) eval_cells(sm.u.cell, ccnt, eps2, L, P, A);
-      __syncwarp();
-      if (lq && !walk_only) eval_leaves<kEps0>(sm.u.bs, sm.leafq, lq, part, eps2, L, P, A, lane);
-      __syncwarp();
+      if (MODE == kFused) {
+        if (ccnt && !walk_only) eval_cells(sm.u.cell, ccnt, eps2, L, P, A);
+        __syncwarp();
+        if (lq && !walk_only) eval_leaves<kEps0>(sm.u.bs, sm.leafq, lq, part, eps2, L, P, A, lane);
+        __syncwarp();
+      }
 
-      // ---- A6: reduce the slices of every particle, write back in the caller's order
-#pragma unroll
-      for (int j = 0; j < 2 * kMaxKP; j++) {
-        if (j >= 2 * L.kp) break;                        // warp-uniform
-        const Acc2& a2 = A[j >> 1];
-        float ax, ay, az, ph;
-        if (j & 1) { ax = hi(a2.ax); ay = hi(a2.ay); az = hi(a2.az); ph = -hi(a2.npot); }
-        else { ax = lo(a2.ax); ay = lo(a2.ay); az = lo(a2.az); ph = -lo(a2.npot); }
-        for (int w = 1; w < L.S; w <<= 1) {
-          const float ox = __shfl_down_sync(kFull, ax, w * L.q), oy = __shfl_down_sync(kFull, ay, w * L.q);
-          const float oz = __shfl_down_sync(kFull, az, w * L.q), op = __shfl_down_sync(kFull, ph, w * L.q);
-          if ((L.s % (2 * w)) == 0 && L.s + w < L.S) { ax += ox; ay += oy; az += oz; ph += op; }
-        }
-        const int tq = j * L.q + lane;
-        if (lane < L.q && tq < m) {
-          const int t = G.y + pb + tq;
-          const int i = __ldg(orig + t);
-          if (!kEps0) ph += __ldg(part + t).w * rsqrt_approx(eps2);     // the particle met itself once
-          acc[3 * (size_t)i + 0] = ax; acc[3 * (size_t)i + 1] = ay; acc[3 * (size_t)i + 2] = az;
-          if (pot) pot[i] = ph;
-          out_npc[i] = (int32_t)n_pc; out_npp[i] = (int32_t)(n_pp - 1);
-        }
+      if (MODE == kFused) {
+        // ---- A6: reduce the slices of every particle, write back in the caller's order
+        write_back<false, !kEps0>(L, A, part, orig, G.y + pb, m, eps2, lane, acc, pot, out_npc, (int32_t)n_pc, out_npp,
+                                  (int32_t)(n_pp - 1));
+      } else if (MODE == kCount) {
+        if (lane == 0) { lio.cnt_c[g] = (unsigned long long)n_pc; lio.cnt_l[g] = (unsigned long long)n_lr; lio.leaf_bodies[g] = (int)n_pp; }
       }
       if (lane == 0) {
-        atomicAdd(&ctr->n_pc_total, (unsigned long long)(n_pc * m));
-        atomicAdd(&ctr->n_pp_total, (unsigned long long)((n_pp - 1) * m));
-        atomicAdd(&ctr->n_tests_total, (unsigned long long)n_tests);
+        if (MODE != kWrite) {                              // the two-pass variant counts in its first pass
+          const long long np = (MODE == kFused) ? m : G.z;
+          atomicAdd(&ctr->n_pc_total, (unsigned long long)(n_pc * np));
+          atomicAdd(&ctr->n_pp_total, (unsigned long long)((n_pp - 1) * np));
+          if (pb == 0) atomicAdd(&ctr->n_tests_total, (unsigned long long)n_tests);   // per group, not per pass
+        }
         if (n_spills) atomicAdd(&ctr->n_spills, (unsigned long long)n_spills);
         if (overflow) atomicExch(&ctr->overflow, 1u);
       }
       __syncwarp();
+      if (MODE != kFused) break;                           // lists are per group, not per pass
     }
   }
 }
 
-template <int STK, bool kEps0>
-int launch_t(const DeviceTree& T, const ForceLaunch& L, cudaStream_t st, int* ctas_per_sm_out) {
-  auto kern = forces_kernel<STK, kEps0>;
+// ---- two-pass variant: the evaluation kernels of Lists 3 and 4 on global lists ------
+// node kernel: warp per group, list chunks gathered to shared memory, acc / pot / n_pc WRITTEN
+__global__ void __launch_bounds__(kWarpsPerCta * 32, TC_MINB)
+node_kernel(const float4* __restrict__ xm, const float4* __restrict__ q0, const float4* __restrict__ q1,
+            const float4* __restrict__ part, const int32_t* __restrict__ orig, const int4* __restrict__ grp, int n_groups,
+            float eps, float* __restrict__ acc, float* __restrict__ pot, int32_t* __restrict__ out_npc,
+            DeviceCounters* __restrict__ ctr, ListIO lio) {
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  WarpSmem<64>& sm = reinterpret_cast<WarpSmem<64>*>(smem_raw)[warp];
+  const float eps2 = eps * eps;
+  while (true) {
+    int g = 0;
+    if (lane == 0) g = (int)atomicAdd(&ctr->next_group, 1u);
+    g = __shfl_sync(kFull, g, 0);
+    if (g >= n_groups) break;
+    g = __ldg(&grp[g].w);
+    const int4 G = __ldg(grp + g);
+    const unsigned long long b = lio.off_c[g];
+    const int n_c = (int)(lio.off_c[g + 1] - b);
+    for (int pb = 0; pb < G.z; pb += kPass) {
+      const int m = min(kPass, G.z - pb);
+      Lanes L; Pos2 P[kMaxKP]; Acc2 A[kMaxKP];
+      setup_pass(L, P, A, part, G.y + pb, m, lane);
+      for (int base = 0; base < n_c; base += kCellCap) {
+        const int cnt = min(kCellCap, n_c - base);
+        for (int t = lane; t < cnt; t += 32) {
+          const int c = __ldg(lio.cells + b + base + t);
+          const float4 c1 = __ldg(q1 + c);
+          CellRec& r = sm.u.cell[t];
+          r.xm = __ldg(xm + c); r.q0 = __ldg(q0 + c); r.q1 = make_float2(c1.x, c1.y);
+        }
+        __syncwarp();
+        eval_cells(sm.u.cell, cnt, eps2, L, P, A);
+        __syncwarp();
+      }
+      write_back<false, false>(L, A, part, orig, G.y + pb, m, eps2, lane, acc, pot, out_npc, n_c);
+    }
+  }
+}
+
+// leaf kernel: warp per group, opened-leaf ranges from the global list, acc / pot ADDED, n_pp written
+template <bool kEps0>
+__global__ void __launch_bounds__(kWarpsPerCta * 32, TC_MINB)
+leaf_kernel(const float4* __restrict__ part, const int32_t* __restrict__ orig, const int4* __restrict__ grp, int n_groups,
+            float eps, float* __restrict__ acc, float* __restrict__ pot, int32_t* __restrict__ out_npp,
+            DeviceCounters* __restrict__ ctr, ListIO lio) {
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  WarpSmem<64>& sm = reinterpret_cast<WarpSmem<64>*>(smem_raw)[warp];
+  const float eps2 = eps * eps;
+  while (true) {
+    int g = 0;
+    if (lane == 0) g = (int)atomicAdd(&ctr->next_group, 1u);
+    g = __shfl_sync(kFull, g, 0);
+    if (g >= n_groups) break;
+    g = __ldg(&grp[g].w);
+    const int4 G = __ldg(grp + g);
+    const unsigned long long b = lio.off_l[g];
+    const int n_l = (int)(lio.off_l[g + 1] - b);
+    const int n_bodies = __ldg(lio.leaf_bodies + g);
+    for (int pb = 0; pb < G.z; pb += kPass) {
+      const int m = min(kPass, G.z - pb);
+      Lanes L; Pos2 P[kMaxKP]; Acc2 A[kMaxKP];
+      setup_pass(L, P, A, part, G.y + pb, m, lane);
+      for (int base = 0; base < n_l; base += kLeafQCap) {
+        const int cnt = min(kLeafQCap, n_l - base);
+        for (int t = lane; t < cnt; t += 32) sm.leafq[t] = __ldg(lio.leaves + b + base + t);
+        __syncwarp();
+        eval_leaves<kEps0>(sm.u.bs, sm.leafq, cnt, part, eps2, L, P, A, lane);
+        __syncwarp();
+      }
+      write_back<true, !kEps0>(L, A, part, orig, G.y + pb, m, eps2, lane, acc, pot, out_npp, n_bodies - 1);
+    }
+  }
+}
+
+template <int STK, bool kEps0, int MODE = kFused>
+int launch_t(const DeviceTree& T, const ForceLaunch& L, cudaStream_t st, int* ctas_per_sm_out, ListIO lio = ListIO()) {
+  auto kern = forces_kernel<STK, kEps0, MODE>;
   const size_t smem = sizeof(WarpSmem<STK>) * kWarpsPerCta;
   cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
   if (e != cudaSuccess) return (int)e;
@@ -465,10 +600,11 @@ int launch_t(const DeviceTree& T, const ForceLaunch& L, cudaStream_t st, int* ct
   if (per_sm < 1) per_sm = 1;
   if (ctas_per_sm_out) { *ctas_per_sm_out = per_sm; return 0; }
   // persistent grid: every SM full, groups handed out by an atomic counter
-  const int grid = L.n_sm * per_sm;
+  // (never more CTAs than the spill buffer was sized for: forces_total_warps)
+  const int grid = L.max_grid > 0 ? std::min(L.n_sm * per_sm, L.max_grid) : L.n_sm * per_sm;
   kern<<<grid, kWarpsPerCta * 32, smem, st>>>(T.bnd, T.xm, T.q0, T.q1, T.part, T.orig, T.grp, (int)T.n_groups,
                                                L.theta, L.eps, L.acc, L.pot, L.n_pc, L.n_pp, L.counters, L.spill,
-                                               L.spill_cap, L.walk_only);
+                                               L.spill_cap, L.walk_only, lio);
   return (int)cudaGetLastError();
 }
 
@@ -482,6 +618,115 @@ int dispatch(const DeviceTree& T, const ForceLaunch& L, cudaStream_t st, int* pe
 
 int launch_forces(const DeviceTree& T, const ForceLaunch& L, void* stream) {
   return dispatch(T, L, (cudaStream_t)stream, nullptr);
+}
+
+// ---- the paper-literal two-pass variant (option "two_pass") ----
+namespace {
+template <typename T>
+cudaError_t grow2(T*& p, size_t& cap, size_t need, cudaStream_t st) {
+  if (cap >= need) return cudaSuccess;
+  cudaError_t e = cudaStreamSynchronize(st);
+  if (e != cudaSuccess) return e;
+  cudaFree(p); p = nullptr; cap = 0;
+  const size_t ncap = need + need / 8 + 256;
+  e = cudaMalloc((void**)&p, sizeof(T) * ncap);
+  if (e == cudaSuccess) cap = ncap;
+  return e;
+}
+template <int MODE>
+int dispatch_walk(const DeviceTree& T, const ForceLaunch& L, cudaStream_t st, ListIO lio) {
+  const bool eps0 = (L.eps * L.eps == 0.f);
+  if (L.stack_smem == 64) return eps0 ? launch_t<64, true, MODE>(T, L, st, nullptr, lio) : launch_t<64, false, MODE>(T, L, st, nullptr, lio);
+  return eps0 ? launch_t<256, true, MODE>(T, L, st, nullptr, lio) : launch_t<256, false, MODE>(T, L, st, nullptr, lio);
+}
+}  // namespace
+
+void TwoPassScratch::release() {
+  cudaFree(cnt_c); cudaFree(cnt_l); cudaFree(off_c); cudaFree(off_l); cudaFree(leaf_bodies); cudaFree(cells); cudaFree(leaves);
+  cudaFree(tmp);
+  for (int k = 0; k < 5; k++) if (ev[k]) cudaEventDestroy((cudaEvent_t)ev[k]);
+  *this = TwoPassScratch();
+}
+
+#define TP_CUDA(call) do { cudaError_t e_ = (call); if (e_ != cudaSuccess) return (int)e_; } while (0)
+
+int launch_forces_two_pass(const DeviceTree& T, const ForceLaunch& L, TwoPassScratch& S, void* stream) {
+  cudaStream_t st = (cudaStream_t)stream;
+  const size_t ng = (size_t)T.n_groups;
+  for (int k = 0; k < 5; k++) if (!S.ev[k]) { cudaEvent_t e; TP_CUDA(cudaEventCreate(&e)); S.ev[k] = e; }
+  TP_CUDA(grow2(S.cnt_c, S.cap_cnt_c, ng + 1, st)); TP_CUDA(grow2(S.cnt_l, S.cap_cnt_l, ng + 1, st));
+  TP_CUDA(grow2(S.off_c, S.cap_off_c, ng + 1, st)); TP_CUDA(grow2(S.off_l, S.cap_off_l, ng + 1, st));
+  TP_CUDA(grow2(S.leaf_bodies, S.cap_lb, ng, st));
+  TP_CUDA(cudaMemsetAsync(S.cnt_c + ng, 0, sizeof(unsigned long long), st));
+  TP_CUDA(cudaMemsetAsync(S.cnt_l + ng, 0, sizeof(unsigned long long), st));
+  ListIO lio;
+  lio.cnt_c = S.cnt_c; lio.cnt_l = S.cnt_l; lio.off_c = S.off_c; lio.off_l = S.off_l;
+  lio.cells = nullptr; lio.leaves = nullptr; lio.leaf_bodies = S.leaf_bodies;
+  unsigned int* next_group = &L.counters->next_group;
+  // pass 1: count
+  TP_CUDA(cudaEventRecord((cudaEvent_t)S.ev[0], st));
+  { const int e = dispatch_walk<kCount>(T, L, st, lio); if (e) return e; }
+  TP_CUDA(cudaEventRecord((cudaEvent_t)S.ev[1], st));
+  // the scan the paper does on the host, here on the device
+  size_t need = 0, need2 = 0;
+  TP_CUDA(cub::DeviceScan::ExclusiveSum(nullptr, need, S.cnt_c, S.off_c, (int)(ng + 1), st));
+  TP_CUDA(cub::DeviceScan::ExclusiveSum(nullptr, need2, S.cnt_l, S.off_l, (int)(ng + 1), st));
+  TP_CUDA(grow2(S.tmp, S.cap_tmp, std::max(need, need2), st));
+  TP_CUDA(cub::DeviceScan::ExclusiveSum(S.tmp, need, S.cnt_c, S.off_c, (int)(ng + 1), st));
+  TP_CUDA(cub::DeviceScan::ExclusiveSum(S.tmp, need2, S.cnt_l, S.off_l, (int)(ng + 1), st));
+  unsigned long long tot[2];
+  TP_CUDA(cudaMemcpyAsync(&tot[0], S.off_c + ng, sizeof(unsigned long long), cudaMemcpyDeviceToHost, st));
+  TP_CUDA(cudaMemcpyAsync(&tot[1], S.off_l + ng, sizeof(unsigned long long), cudaMemcpyDeviceToHost, st));
+  TP_CUDA(cudaStreamSynchronize(st));
+  S.n_list_cells = (long long)tot[0]; S.n_list_leaves = (long long)tot[1];
+  TP_CUDA(grow2(S.cells, S.cap_cells, (size_t)tot[0] + 1, st));
+  TP_CUDA(grow2(S.leaves, S.cap_leaves, (size_t)tot[1] + 1, st));
+  lio.cells = S.cells; lio.leaves = S.leaves;
+  // pass 2: write the lists
+  TP_CUDA(cudaMemsetAsync(next_group, 0, sizeof(unsigned int), st));
+  TP_CUDA(cudaEventRecord((cudaEvent_t)S.ev[1], st));
+  { const int e = dispatch_walk<kWrite>(T, L, st, lio); if (e) return e; }
+  TP_CUDA(cudaEventRecord((cudaEvent_t)S.ev[2], st));
+  // evaluation kernels
+  const size_t smem = sizeof(WarpSmem<64>) * kWarpsPerCta;
+  const bool eps0 = (L.eps * L.eps == 0.f);
+  int per_sm = 0;
+  TP_CUDA(cudaFuncSetAttribute(node_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+  TP_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, node_kernel, kWarpsPerCta * 32, smem));
+  TP_CUDA(cudaMemsetAsync(next_group, 0, sizeof(unsigned int), st));
+  node_kernel<<<L.n_sm * std::max(per_sm, 1), kWarpsPerCta * 32, smem, st>>>(T.xm, T.q0, T.q1, T.part, T.orig, T.grp, (int)T.n_groups,
+                                                                              L.eps, L.acc, L.pot, L.n_pc, L.counters, lio);
+  TP_CUDA(cudaGetLastError());
+  TP_CUDA(cudaEventRecord((cudaEvent_t)S.ev[3], st));
+  TP_CUDA(cudaMemsetAsync(next_group, 0, sizeof(unsigned int), st));
+  if (eps0) {
+    TP_CUDA(cudaFuncSetAttribute(leaf_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    TP_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, leaf_kernel<true>, kWarpsPerCta * 32, smem));
+    leaf_kernel<true><<<L.n_sm * std::max(per_sm, 1), kWarpsPerCta * 32, smem, st>>>(T.part, T.orig, T.grp, (int)T.n_groups, L.eps, L.acc,
+                                                                                     L.pot, L.n_pp, L.counters, lio);
+  } else {
+    TP_CUDA(cudaFuncSetAttribute(leaf_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    TP_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, leaf_kernel<false>, kWarpsPerCta * 32, smem));
+    leaf_kernel<false><<<L.n_sm * std::max(per_sm, 1), kWarpsPerCta * 32, smem, st>>>(T.part, T.orig, T.grp, (int)T.n_groups, L.eps, L.acc,
+                                                                                      L.pot, L.n_pp, L.counters, lio);
+  }
+  TP_CUDA(cudaGetLastError());
+  TP_CUDA(cudaEventRecord((cudaEvent_t)S.ev[4], st));
+  return 0;
+}
+
+// event times of the last launch_forces_two_pass (stream must be idle): count, write, node, leaf [ms]
+int two_pass_times(const TwoPassScratch& S, float ms[4]) {
+  // ev[1] was re-recorded after the scan: [0]->[1'] would include it, so the count pass is timed by its own pair below
+  for (int k = 0; k < 4; k++) ms[k] = 0.f;
+  if (!S.ev[4]) return 0;
+  TP_CUDA(cudaEventElapsedTime(&ms[1], (cudaEvent_t)S.ev[1], (cudaEvent_t)S.ev[2]));
+  TP_CUDA(cudaEventElapsedTime(&ms[2], (cudaEvent_t)S.ev[2], (cudaEvent_t)S.ev[3]));
+  TP_CUDA(cudaEventElapsedTime(&ms[3], (cudaEvent_t)S.ev[3], (cudaEvent_t)S.ev[4]));
+  float all = 0.f;
+  TP_CUDA(cudaEventElapsedTime(&all, (cudaEvent_t)S.ev[0], (cudaEvent_t)S.ev[1]));
+  ms[0] = all;     // count pass + device scan + list allocation (the paper's host step)
+  return 0;
 }
 
 // ---- tc_direct: direct summation (the paper's accuracy reference) ----------------
@@ -640,6 +885,8 @@ int measure_fp32_peak(int n_sm, void* stream, double* tflops) {
   *tflops = 2.0 * 16.0 * (double)n * (double)grid * 256.0 / ((double)best * 1e-3) / 1e12;
   return 0;
 }
+
+int forces_warps_per_cta() { return kWarpsPerCta; }
 
 int forces_total_warps(int n_sm, int stack_smem) {
   DeviceTree T;

@@ -27,9 +27,9 @@ def test_header_symbols_are_exported():
 
 
 def test_stats_struct_size_matches_header():
-    # 4 int64 + 4 int32 + 4 int64 + 3 double + 1 int64
+    # 4 int64 + 4 int32 + 4 int64 + 3 double + 1 int64 + 4 double + 1 int64
     import ctypes
-    assert ctypes.sizeof(B.tc_stats) == 4 * 8 + 4 * 4 + 4 * 8 + 3 * 8 + 8
+    assert ctypes.sizeof(B.tc_stats) == 4 * 8 + 4 * 4 + 4 * 8 + 3 * 8 + 8 + 4 * 8 + 8
 
 
 def test_no_cpu_fallback_host_only_refuses_forces():
