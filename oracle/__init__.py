@@ -42,6 +42,7 @@ def _load():
     L.orc_create.restype = vp
     L.orc_create.argtypes = [i64, vp, vp, i32, i32]
     L.orc_destroy.argtypes = [vp]
+    L.orc_set_variant.argtypes = [vp, i32, i32]
     for f in ("orc_n_cells", "orc_n_leaves", "orc_n_groups"):
         getattr(L, f).restype = i64
         getattr(L, f).argtypes = [vp]
@@ -74,7 +75,8 @@ def num_threads() -> int:
 class Oracle:
     """fp64 CPU tree-code: own tree (O1-O4), own walk (O5), own evaluation (O6)."""
 
-    def __init__(self, pos, mass, n_leaf: int = 16, n_group: int | None = None):
+    def __init__(self, pos, mass, n_leaf: int = 16, n_group: int | None = None, open_rule: int = 0,
+                 quadrupole: bool = True):
         L = _load()
         self.pos = np.ascontiguousarray(pos, dtype=np.float32)
         self.mass = np.ascontiguousarray(mass, dtype=np.float32)
@@ -85,6 +87,9 @@ class Oracle:
         self._h = L.orc_create(self.n, _p(self.pos), _p(self.mass), self.n_leaf, self.n_group)
         if not self._h:
             raise ValueError("orc_create failed (n, n_leaf, n_group must be >= 1)")
+        # variants: open_rule 1 = group cube to cell COM (R21); quadrupole False = monopole only (R22)
+        L.orc_set_variant(self._h, int(open_rule), int(bool(quadrupole)))
+        self.open_rule, self.quadrupole = int(open_rule), bool(quadrupole)
         self.n_cells = int(L.orc_n_cells(self._h))
         self.n_leaves = int(L.orc_n_leaves(self._h))
         self.n_groups = int(L.orc_n_groups(self._h))

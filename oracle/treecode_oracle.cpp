@@ -24,6 +24,9 @@
 //    evaluation  : N = 2 closed form; theta = 0 == direct sum; theta -> 0 convergence;
 //                  momentum invariant; Plummer analytic field
 //    direct sum  : N = 2, N = 3 closed forms; sum m a = 0
+//    variants    : R21 (opening test on the cell's centre of mass) and R22 (monopole-only cells), both off
+//                  by default: lists re-derived from the recursive definition, theta = 0, own cells open
+//                  in fp32, monopole closed form, error orders (tests/test_oracle_variants.py)
 //  "parity unpinned": the opening RULE itself (R1) — the paper never prints
 //  its formula (PAPER.md:79 calls open_node, never defined) — and every value
 //  that lives only in Figs. 4-8.
@@ -58,6 +61,9 @@ struct OCell {
 struct Oracle {
   int64_t n = 0;
   int n_leaf = 0, n_group = 0;
+  // variants (R21, R22): 0 = the default readings
+  int open_rule = 0;   // 0: cube-to-cube distance (R1); 1: group cube to the cell's centre of mass (R21)
+  int quadrupole = 1;  // 1: monopole + quadrupole (R10); 0: monopole only (R22)
   std::vector<double> x, y, z, m;  // inputs widened to fp64
   std::vector<int32_t> gx, gy, gz; // O1 integer grid coordinates
   double org[3], side;
@@ -196,10 +202,12 @@ void find_groups(Oracle& T, int c) {
 
 // ---- O5: the opening test (List 2 PAPER.md:73-91 `open_node`; R1, R9, R14)
 //  fp64: d_k = max(0, |b_c,k - b_g,k| - h_c - h_g), open iff d^2 theta^2 <= (2 h_c)^2
-inline bool open64(const OCell& c, const OCell& g, double theta, double* margin) {
+//  rule 1 (R21): the cell is represented by its centre of mass: d_k = max(0, |X_c,k - b_g,k| - h_g)
+inline bool open64(const OCell& c, const OCell& g, double theta, double* margin, int rule) {
   double d2 = 0.0;
   for (int k = 0; k < 3; k++) {
-    const double d = std::max(0.0, std::fabs(c.b[k] - g.b[k]) - c.h - g.h);
+    const double d = rule ? std::max(0.0, std::fabs(c.X[k] - g.b[k]) - g.h)
+                          : std::max(0.0, std::fabs(c.b[k] - g.b[k]) - c.h - g.h);
     d2 += d * d;
   }
   const double l = 2.0 * c.h;
@@ -211,11 +219,12 @@ inline bool open64(const OCell& c, const OCell& g, double theta, double* margin)
 //     s = h_c + h_g;  t_k = max(|b_c,k - b_g,k| - s, 0)
 //     d2 = fma(t_z,t_z, fma(t_y,t_y, t_x*t_x));  l = h_c + h_c
 //     open iff d2 * (theta*theta) <= l * l
-inline bool open32(const OCell& c, const OCell& g, float theta) {
-  const float s = c.h32 + g.h32;
+//  rule 1: the same sequence with the fp32 centre of mass in place of b_c and 0 in place of h_c
+inline bool open32(const OCell& c, const OCell& g, float theta, int rule) {
+  const float s = (rule ? 0.0f : c.h32) + g.h32;
   float t[3];
   for (int k = 0; k < 3; k++) {
-    const float u = c.b32[k] - g.b32[k];
+    const float u = (rule ? (float)c.X[k] : c.b32[k]) - g.b32[k];
     const float v = std::fabs(u) - s;
     t[k] = std::fmax(v, 0.0f);
   }
@@ -252,8 +261,8 @@ void walk_group(const Oracle& T, int gcell, double theta, int mode, WalkOut& W) 
       if (ch < 0) continue;
       const OCell& C = T.cells[ch];
       double margin;
-      const bool o64 = open64(C, G, theta, &margin);
-      const bool o32 = open32(C, G, (float)theta);
+      const bool o64 = open64(C, G, theta, &margin, T.open_rule);
+      const bool o32 = open32(C, G, (float)theta, T.open_rule);
       W.n_tests++;
       W.min_margin = std::min(W.min_margin, margin);
       if (o64 != o32) W.n_flips++;
@@ -284,6 +293,11 @@ void eval_group(const Oracle& T, int gcell, const WalkOut& W, double eps,
       const double s2 = rx * rx + ry * ry + rz * rz + eps2;
       const double s = std::sqrt(s2);
       const double s3 = s2 * s, s5 = s3 * s2, s7 = s5 * s2;
+      if (!T.quadrupole) {             // R22: monopole only
+        ax += -C.M * rx / s3; ay += -C.M * ry / s3; az += -C.M * rz / s3;
+        ph += -C.M / s;
+        continue;
+      }
       const double Qrx = C.Q[0] * rx + C.Q[3] * ry + C.Q[4] * rz;
       const double Qry = C.Q[3] * rx + C.Q[1] * ry + C.Q[5] * rz;
       const double Qrz = C.Q[4] * rx + C.Q[5] * ry + C.Q[2] * rz;
@@ -338,6 +352,12 @@ void* orc_create(int64_t n, const float* pos, const float* mass, int n_leaf, int
 }
 
 void orc_destroy(void* h) { delete (Oracle*)h; }
+
+// variants (R21, R22); 0 / 1 = the default readings
+void orc_set_variant(void* h, int open_rule, int quadrupole) {
+  Oracle* T = (Oracle*)h;
+  T->open_rule = open_rule ? 1 : 0; T->quadrupole = quadrupole ? 1 : 0;
+}
 
 int64_t orc_n_cells(void* h) { return (int64_t)((Oracle*)h)->cells.size(); }
 int64_t orc_n_leaves(void* h) { return ((Oracle*)h)->n_leaves; }
