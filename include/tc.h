@@ -114,6 +114,11 @@ int tc_forces(tc_ctx* ctx, float theta, float eps, float* acc, float* pot);
  *                 construction on the GPU (tc_build_gpu.cu) and writes the packed tree in device memory —
  *                 no bulk H2D; t_host_ms of tc_stats is then the wall time of the device build, t_copy_ms 0.
  *                 Cells, boundary cubes, groups and counts are identical to the host build's.
+ *   "open_rule"   0 (default: minimum distance between the group's and the cell's boundary cubes, R1)
+ *                 or 1: distance from the group's cube to the cell's centre of mass (variant R21): about 45 %
+ *                 fewer interactions and about twice the error at equal theta.
+ *   "quadrupole"  1 (default: monopole + quadrupole) or 0: monopole-only cells (variant R22, the expansion of
+ *                 the Hamada et al. code the paper compares with).
  *   "two_pass"    0 (default: the fused kernel) or 1: the paper-literal pipeline —
  *                 walk-count kernel, scan of the list sizes, walk-write kernel (lists in global memory),
  *                 body-node kernel, body-leaf kernel; same lists, same counts, same results up to

@@ -26,7 +26,7 @@ struct tc_ctx {
   int n_group = 96;
   bool device_build = false;          // option "device_build": tc_build_gpu.cu instead of tc_build.cpp
   int stack_smem = 256;
-  int walk_only = 0;
+  int walk_only = 0, open_rule = 0, quadrupole = 1;
   bool two_pass = false;
   tc::TwoPassScratch tps;
   bool last_two_pass = false;
@@ -225,6 +225,14 @@ int tc_set_option(tc_ctx* c, const char* key, double v) {
     if (c->host_only && v != 0.0) return fail(c, TC_ESTATE, "tc_set_option: device_build needs a device");
     c->device_build = (v != 0.0); return TC_OK;
   }
+  if (!std::strcmp(key, "open_rule")) {
+    if (v != 0.0 && v != 1.0) return fail(c, TC_EINVAL, "tc_set_option: open_rule must be 0 or 1");
+    c->open_rule = (int)v; return TC_OK;
+  }
+  if (!std::strcmp(key, "quadrupole")) {
+    if (v != 0.0 && v != 1.0) return fail(c, TC_EINVAL, "tc_set_option: quadrupole must be 0 or 1");
+    c->quadrupole = (int)v; return TC_OK;
+  }
   if (!std::strcmp(key, "two_pass")) {
     if (v != 0.0 && v != 1.0) return fail(c, TC_EINVAL, "tc_set_option: two_pass must be 0 or 1");
     c->two_pass = (v != 0.0); return TC_OK;
@@ -409,7 +417,7 @@ int tc_forces(tc_ctx* c, float theta, float eps, float* acc, float* pot) {
   L.acc = acc_dev ? acc : c->d_acc;
   L.pot = pot ? (acc_dev ? pot : c->d_pot) : nullptr;
   L.n_pc = c->d_npc; L.n_pp = c->d_npp; L.counters = c->d_ctr; L.spill = c->d_spill; L.spill_cap = c->spill_cap;
-  L.stack_smem = c->stack_smem; L.n_sm = c->n_sm; L.walk_only = c->walk_only;
+  L.stack_smem = c->stack_smem; L.n_sm = c->n_sm; L.flags = (c->walk_only ? 1 : 0) | (c->open_rule ? 2 : 0) | (c->quadrupole ? 0 : 4);
   L.max_grid = (int)(warps / (size_t)tc::forces_warps_per_cta());
   // stream-ordered: no host synchronisation between queued calls; the overflow flag is sticky until collect()
   TC_CUDA(c, cudaMemsetAsync(c->d_ctr, 0, offsetof(tc::DeviceCounters, overflow), c->stream));

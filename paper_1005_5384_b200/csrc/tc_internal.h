@@ -84,7 +84,7 @@ struct ForceLaunch {
   uint32_t* spill = nullptr;  // device [n_warps_total * spill_cap]
   int spill_cap = 0;
   int stack_smem = 256;
-  int walk_only = 0;          // measurement aid: walk and build the lists, skip their evaluation
+  int flags = 0;              // bit 0: walk_only (measurement aid), bit 1: COM opening rule (R21), bit 2: monopole only (R22)
   int n_sm = 148;
   int max_grid = 0;           // CTAs the spill buffer has room for (0: no limit)
 };

@@ -212,6 +212,30 @@ __device__ __forceinline__ void eval_cells(const CellRec* rec, int cnt, float ep
   }
 }
 
+// Monopole-only variant (R22, option "quadrupole" = 0): a cell is a point mass (X, M)
+template <int KP, bool kEps0>
+__device__ __forceinline__ void eval_cells_mono_k(const CellRec* __restrict__ rec, int cnt, float eps2, const Lanes& L,
+                                                  const Pos2 (&P)[kMaxKP], Acc2 (&A)[kMaxKP]) {
+  if (!L.active) return;
+  const int st = L.S;
+  for (int e = L.s; e < cnt; e += st) {
+    const float4 b0 = rec[e].xm;
+#pragma unroll
+    for (int j = 0; j < KP; j++) pp_interact<kEps0>(P[j], eps2, b0, A[j]);
+  }
+}
+
+template <bool kEps0, int KP = 1>
+__device__ __forceinline__ void eval_cells_mono(const CellRec* rec, int cnt, float eps2, const Lanes& L,
+                                                const Pos2 (&P)[kMaxKP], Acc2 (&A)[kMaxKP]) {
+  if constexpr (KP == kMaxKP) {
+    eval_cells_mono_k<KP, kEps0>(rec, cnt, eps2, L, P, A);
+  } else {
+    if (L.kp == KP) eval_cells_mono_k<KP, kEps0>(rec, cnt, eps2, L, P, A);
+    else eval_cells_mono<kEps0, KP + 1>(rec, cnt, eps2, L, P, A);
+  }
+}
+
 template <int KP, bool kEps0>
 __device__ __forceinline__ void eval_bodies_k(const float4* __restrict__ body, int cnt, float eps2, const Lanes& L,
                                               const Pos2 (&P)[kMaxKP], Acc2 (&A)[kMaxKP]) {
@@ -338,6 +362,7 @@ struct ListIO {
 };
 
 enum { kFused = 0, kCount = 1, kWrite = 2 };
+enum { kFlagWalkOnly = 1, kFlagComRule = 2, kFlagMonopole = 4 };   // run-time variants of a launch
 
 template <int STK, bool kEps0, int MODE = kFused>
 __global__ void __launch_bounds__(kWarpsPerCta * 32, TC_MINB)
@@ -346,7 +371,7 @@ forces_kernel(const float4* __restrict__ bnd, const float4* __restrict__ xm, con
               const int4* __restrict__ grp, int n_groups, float theta, float eps,
               float* __restrict__ acc, float* __restrict__ pot, int32_t* __restrict__ out_npc,
               int32_t* __restrict__ out_npp, DeviceCounters* __restrict__ ctr, uint32_t* __restrict__ spill_all,
-              int spill_cap, int walk_only, ListIO lio) {
+              int spill_cap, int flags, ListIO lio) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   WarpSmem<STK>& sm = reinterpret_cast<WarpSmem<STK>*>(smem_raw)[warp];
@@ -354,6 +379,7 @@ forces_kernel(const float4* __restrict__ bnd, const float4* __restrict__ xm, con
   const float eps2 = eps * eps;
   const float th2 = __fmul_rn(theta, theta);
   const unsigned lt_mask = (1u << lane) - 1u;
+  const bool walk_only = flags & kFlagWalkOnly, com_rule = flags & kFlagComRule, mono = flags & kFlagMonopole;
 
   // root: a leaf root is never tested (O5) — its bodies are the whole leaf list
   const float4 root_b = __ldg(bnd);
@@ -415,11 +441,13 @@ forces_kernel(const float4* __restrict__ bnd, const float4* __restrict__ xm, con
         float4 cb = make_float4(0.f, 0.f, 0.f, 0.f), cx = cb, c0 = cb, c1 = cb;
         if (valid) { cb = __ldg(bnd + c); cx = __ldg(xm + c); c0 = __ldg(q0 + c); c1 = __ldg(q1 + c); }
         // open_node (O5/R16): one fixed sequence of correctly rounded fp32 operations
+        // (variant R21, com_rule: the cell's centre of mass in place of b_c, 0 in place of h_c in the distance)
         const float hc = fabsf(cb.w);
-        const float s = __fadd_rn(hc, gh);
-        const float tx = fmaxf(__fsub_rn(fabsf(__fsub_rn(cb.x, gbx)), s), 0.f);
-        const float ty = fmaxf(__fsub_rn(fabsf(__fsub_rn(cb.y, gby)), s), 0.f);
-        const float tz = fmaxf(__fsub_rn(fabsf(__fsub_rn(cb.z, gbz)), s), 0.f);
+        const float s = __fadd_rn(com_rule ? 0.f : hc, gh);
+        const float px = com_rule ? cx.x : cb.x, py = com_rule ? cx.y : cb.y, pz = com_rule ? cx.z : cb.z;
+        const float tx = fmaxf(__fsub_rn(fabsf(__fsub_rn(px, gbx)), s), 0.f);
+        const float ty = fmaxf(__fsub_rn(fabsf(__fsub_rn(py, gby)), s), 0.f);
+        const float tz = fmaxf(__fsub_rn(fabsf(__fsub_rn(pz, gbz)), s), 0.f);
         const float d2 = __fmaf_rn(tz, tz, __fmaf_rn(ty, ty, __fmul_rn(tx, tx)));
         const float l = __fadd_rn(hc, hc);
         const bool open = valid && (__fmul_rn(d2, th2) <= __fmul_rn(l, l));
@@ -476,13 +504,13 @@ forces_kernel(const float4* __restrict__ bnd, const float4* __restrict__ xm, con
         if (MODE != kFused) continue;
         const bool flush_leaves = lq > kLeafQCap - 32;
         if (ccnt > kCellCap - 32 || (flush_leaves && ccnt)) {
-          if (!walk_only) eval_cells(sm.u.cell, ccnt, eps2, L, P, A);
+          if (!walk_only) { if (mono) eval_cells_mono<kEps0>(sm.u.cell, ccnt, eps2, L, P, A); else eval_cells(sm.u.cell, ccnt, eps2, L, P, A); }
           ccnt = 0; __syncwarp();
         }
         if (flush_leaves) { if (!walk_only) eval_leaves<kEps0>(sm.u.bs, sm.leafq, lq, part, eps2, L, P, A, lane); lq = 0; }
       }
       if (MODE == kFused) {
-        if (ccnt && !walk_only) eval_cells(sm.u.cell, ccnt, eps2, L, P, A);
+        if (ccnt && !walk_only) { if (mono) eval_cells_mono<kEps0>(sm.u.cell, ccnt, eps2, L, P, A); else eval_cells(sm.u.cell, ccnt, eps2, L, P, A); }
         __syncwarp();
         if (lq && !walk_only) eval_leaves<kEps0>(sm.u.bs, sm.leafq, lq, part, eps2, L, P, A, lane);
         __syncwarp();
@@ -517,11 +545,12 @@ __global__ void __launch_bounds__(kWarpsPerCta * 32, TC_MINB)
 node_kernel(const float4* __restrict__ xm, const float4* __restrict__ q0, const float4* __restrict__ q1,
             const float4* __restrict__ part, const int32_t* __restrict__ orig, const int4* __restrict__ grp, int n_groups,
             float eps, float* __restrict__ acc, float* __restrict__ pot, int32_t* __restrict__ out_npc,
-            DeviceCounters* __restrict__ ctr, ListIO lio) {
+            DeviceCounters* __restrict__ ctr, ListIO lio, int flags) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   WarpSmem<64>& sm = reinterpret_cast<WarpSmem<64>*>(smem_raw)[warp];
   const float eps2 = eps * eps;
+  const bool mono = flags & kFlagMonopole;
   while (true) {
     int g = 0;
     if (lane == 0) g = (int)atomicAdd(&ctr->next_group, 1u);
@@ -544,7 +573,7 @@ node_kernel(const float4* __restrict__ xm, const float4* __restrict__ q0, const 
           r.xm = __ldg(xm + c); r.q0 = __ldg(q0 + c); r.q1 = make_float2(c1.x, c1.y);
         }
         __syncwarp();
-        eval_cells(sm.u.cell, cnt, eps2, L, P, A);
+        if (mono) eval_cells_mono<false>(sm.u.cell, cnt, eps2, L, P, A); else eval_cells(sm.u.cell, cnt, eps2, L, P, A);
         __syncwarp();
       }
       write_back<false, false>(L, A, part, orig, G.y + pb, m, eps2, lane, acc, pot, out_npc, n_c);
@@ -604,7 +633,7 @@ int launch_t(const DeviceTree& T, const ForceLaunch& L, cudaStream_t st, int* ct
   const int grid = L.max_grid > 0 ? std::min(L.n_sm * per_sm, L.max_grid) : L.n_sm * per_sm;
   kern<<<grid, kWarpsPerCta * 32, smem, st>>>(T.bnd, T.xm, T.q0, T.q1, T.part, T.orig, T.grp, (int)T.n_groups,
                                                L.theta, L.eps, L.acc, L.pot, L.n_pc, L.n_pp, L.counters, L.spill,
-                                               L.spill_cap, L.walk_only, lio);
+                                               L.spill_cap, L.flags, lio);
   return (int)cudaGetLastError();
 }
 
@@ -695,7 +724,7 @@ int launch_forces_two_pass(const DeviceTree& T, const ForceLaunch& L, TwoPassScr
   TP_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, node_kernel, kWarpsPerCta * 32, smem));
   TP_CUDA(cudaMemsetAsync(next_group, 0, sizeof(unsigned int), st));
   node_kernel<<<L.n_sm * std::max(per_sm, 1), kWarpsPerCta * 32, smem, st>>>(T.xm, T.q0, T.q1, T.part, T.orig, T.grp, (int)T.n_groups,
-                                                                              L.eps, L.acc, L.pot, L.n_pc, L.counters, lio);
+                                                                              L.eps, L.acc, L.pot, L.n_pc, L.counters, lio, L.flags);
   TP_CUDA(cudaGetLastError());
   TP_CUDA(cudaEventRecord((cudaEvent_t)S.ev[3], st));
   TP_CUDA(cudaMemsetAsync(next_group, 0, sizeof(unsigned int), st));
