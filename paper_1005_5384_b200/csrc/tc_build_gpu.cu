@@ -112,44 +112,50 @@ __device__ __forceinline__ int lower_octant(const unsigned long long* __restrict
   return b;
 }
 
-// O2 pass 1: number of non-empty octants of every node of the level (0 for leaves)
+// O2 pass 1: 8 lanes per node — lane o finds where octant o starts in the node's sorted key range (one binary
+// search each, side by side), the 8 lanes count the non-empty octants (0 for leaves) and keep the bounds.
 __global__ void k_count_children(const unsigned long long* __restrict__ keys, const int* __restrict__ c_begin,
-                                 const int* __restrict__ c_count, int lb, int nl, int shift, int n_leaf, int* __restrict__ nch) {
+                                 const int* __restrict__ c_count, int lb, int nl, int shift, int n_leaf, int* __restrict__ nch,
+                                 int* __restrict__ bounds) {
   const int t = blockIdx.x * blockDim.x + threadIdx.x;
-  if (t >= nl) return;
-  const int c = lb + t;
-  int cnt = 0;
-  if (c_count[c] > n_leaf) {
-    const int b = c_begin[c], e = b + c_count[c];
-    int prev = b;
-#pragma unroll
-    for (unsigned o = 1; o <= 8; o++) {
-      const int pos = (o == 8) ? e : lower_octant(keys, prev, e, shift, o);
-      cnt += (pos > prev);
-      prev = pos;
-    }
-  }
-  nch[t] = cnt;
+  const int node = t >> 3;
+  const unsigned o = (unsigned)(t & 7);
+  const bool valid = node < nl;
+  const int c = lb + (valid ? node : 0);
+  const int b = c_begin[c], e = b + c_count[c];
+  const bool split = valid && c_count[c] > n_leaf;
+  const int p0 = (o == 0 || !split) ? b : lower_octant(keys, b, e, shift, o);
+  int p1 = __shfl_down_sync(0xffffffffu, p0, 1, 8);
+  if (o == 7) p1 = e;
+  const unsigned seg = 0xffu << ((threadIdx.x & 31) & ~7);
+  const unsigned m = __ballot_sync(0xffffffffu, split && p1 > p0) & seg;
+  if (!valid) return;
+  bounds[t] = p0;
+  if (o == 0) nch[node] = __popc(m);
 }
 
-// O2 pass 2: create the children (contiguous, octant order)
-__global__ void k_make_children(const unsigned long long* __restrict__ keys, int* __restrict__ c_begin, int* __restrict__ c_count,
-                                int* __restrict__ c_first, int* __restrict__ c_nchild, int* __restrict__ c_parent,
-                                int lb, int nl, int le, int shift, const int* __restrict__ nch, const int* __restrict__ off) {
+// O2 pass 2: create the children (contiguous, octant order) from the kept bounds
+__global__ void k_make_children(int* __restrict__ c_begin, int* __restrict__ c_count, int* __restrict__ c_first,
+                                int* __restrict__ c_nchild, int* __restrict__ c_parent, int lb, int nl, int le,
+                                const int* __restrict__ nch, const int* __restrict__ off, const int* __restrict__ bounds) {
   const int t = blockIdx.x * blockDim.x + threadIdx.x;
-  if (t >= nl) return;
-  const int c = lb + t;
-  const int k = nch[t];
-  c_nchild[c] = k;
-  c_first[c] = k ? le + off[t] : -1;
-  if (!k) return;
-  const int b = c_begin[c], e = b + c_count[c];
-  int prev = b, j = le + off[t];
-#pragma unroll
-  for (unsigned o = 1; o <= 8; o++) {
-    const int pos = (o == 8) ? e : lower_octant(keys, prev, e, shift, o);
-    if (pos > prev) { c_begin[j] = prev; c_count[j] = pos - prev; c_parent[j] = c; j++; }
-    prev = pos;
+  const int node = t >> 3;
+  const unsigned o = (unsigned)(t & 7);
+  const bool valid = node < nl;
+  const int c = lb + (valid ? node : 0);
+  const int k = valid ? nch[node] : 0;
+  const int e = c_begin[c] + c_count[c];
+  const int p0 = valid ? bounds[t] : 0;
+  int p1 = __shfl_down_sync(0xffffffffu, p0, 1, 8);
+  if (o == 7) p1 = e;
+  const bool nonempty = k > 0 && p1 > p0;
+  const unsigned seg_shift = (threadIdx.x & 31) & ~7;
+  const unsigned m = (__ballot_sync(0xffffffffu, nonempty) >> seg_shift) & 0xffu;
+  if (!valid) return;
+  if (o == 0) { c_nchild[c] = k; c_first[c] = k ? le + off[node] : -1; }
+  if (nonempty) {
+    const int j = le + off[node] + __popc(m & ((1u << o) - 1u));
+    c_begin[j] = p0; c_count[j] = p1 - p0; c_parent[j] = c;
   }
 }
 
@@ -329,7 +335,7 @@ static int grow(T*& p, size_t& cap, size_t need, bool keep, cudaStream_t st, std
 
 void DeviceBuildScratch::release() {
   void* ptrs[] = {keys, keys_alt, idx, idx_alt, cub_tmp, c_begin, c_count, c_first, c_nchild, c_parent, nch, off, mom,
-                  is_group, gcell, gcell_sorted, gkey, gkey_alt, gval, gval_alt, boxes, small, link, q6, pass_cost};
+                  is_group, gcell, gcell_sorted, gkey, gkey_alt, gval, gval_alt, boxes, small, link, q6, pass_cost, bounds};
   for (void* p : ptrs) cudaFree(p);
   *this = DeviceBuildScratch();
 }
@@ -401,8 +407,8 @@ int build_device_tree(const float4* src, int64_t n, int n_leaf, int n_group, Dev
       break;
     }
     const int shift = 3 * (kMaxLevel - 1 - level);
-    TCG_GROW(S.nch, S.cap_nch, nl, false); TCG_GROW(S.off, S.cap_off, nl, false);
-    k_count_children<<<blocks(nl), 256, 0, st>>>(S.keys, S.c_begin, S.c_count, (int)lb, (int)nl, shift, n_leaf, S.nch);
+    TCG_GROW(S.nch, S.cap_nch, nl, false); TCG_GROW(S.off, S.cap_off, nl, false); TCG_GROW(S.bounds, S.cap_bounds, 8 * nl, false);
+    k_count_children<<<blocks(8 * nl), 256, 0, st>>>(S.keys, S.c_begin, S.c_count, (int)lb, (int)nl, shift, n_leaf, S.nch, S.bounds);
     size_t need = 0;
     TCG_CUDA(cub::DeviceScan::ExclusiveSum(nullptr, need, S.nch, S.off, (int)nl, st));
     TCG_GROW(S.cub_tmp, S.cap_tmp, need, false);
@@ -419,8 +425,8 @@ int build_device_tree(const float4* src, int64_t n, int n_leaf, int n_group, Dev
       TCG_GROW(S.c_first, S.cap_cfirst, new_e, true); TCG_GROW(S.c_nchild, S.cap_cnchild, new_e, true);
       TCG_GROW(S.c_parent, S.cap_cparent, new_e, true);
     }
-    k_make_children<<<blocks(nl), 256, 0, st>>>(S.keys, S.c_begin, S.c_count, S.c_first, S.c_nchild, S.c_parent, (int)lb,
-                                                 (int)nl, (int)le, shift, S.nch, S.off);
+    k_make_children<<<blocks(8 * nl), 256, 0, st>>>(S.c_begin, S.c_count, S.c_first, S.c_nchild, S.c_parent, (int)lb, (int)nl,
+                                                     (int)le, S.nch, S.off, S.bounds);
     if (total == 0) break;
     lb = le; le = new_e; level++;
   }

@@ -118,6 +118,7 @@ struct DeviceBuildScratch {
   int *c_begin = nullptr, *c_count = nullptr, *c_first = nullptr, *c_nchild = nullptr, *c_parent = nullptr;
   size_t cap_cbegin = 0, cap_ccount = 0, cap_cfirst = 0, cap_cnchild = 0, cap_cparent = 0;
   int *nch = nullptr, *off = nullptr;                        size_t cap_nch = 0, cap_off = 0;
+  int* bounds = nullptr;                                     size_t cap_bounds = 0;  // 8 octant starts per node of a level
   char* mom = nullptr;                                       size_t cap_mom = 0;     // Moments[]
   unsigned char* is_group = nullptr;                         size_t cap_isg = 0;
   int *gcell = nullptr, *gcell_sorted = nullptr;             size_t cap_gcell = 0, cap_gcells = 0;
