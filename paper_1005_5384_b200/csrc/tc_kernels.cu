@@ -39,10 +39,10 @@ namespace {
 #define TC_MAXKP 3
 #endif
 #ifndef TC_MINB
-#define TC_MINB 5
+#define TC_MINB 4
 #endif
 #ifndef TC_CELLCAP
-#define TC_CELLCAP 96
+#define TC_CELLCAP 192
 #endif
 #ifndef TC_WARPS
 #define TC_WARPS 4
