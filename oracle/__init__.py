@@ -43,6 +43,8 @@ def _load():
     L.orc_create.argtypes = [i64, vp, vp, i32, i32]
     L.orc_destroy.argtypes = [vp]
     L.orc_set_variant.argtypes = [vp, i32, i32]
+    L.orc_set_group_box.argtypes = [vp, i32]
+    L.orc_get_ext32.argtypes = [vp, vp]
     for f in ("orc_n_cells", "orc_n_leaves", "orc_n_groups"):
         getattr(L, f).restype = i64
         getattr(L, f).argtypes = [vp]
@@ -76,7 +78,7 @@ class Oracle:
     """fp64 CPU tree-code: own tree (O1-O4), own walk (O5), own evaluation (O6)."""
 
     def __init__(self, pos, mass, n_leaf: int = 16, n_group: int | None = None, open_rule: int = 0,
-                 quadrupole: bool = True):
+                 quadrupole: bool = True, group_box: bool = False):
         L = _load()
         self.pos = np.ascontiguousarray(pos, dtype=np.float32)
         self.mass = np.ascontiguousarray(mass, dtype=np.float32)
@@ -90,6 +92,9 @@ class Oracle:
         # variants: open_rule 1 = group cube to cell COM (R21); quadrupole False = monopole only (R22)
         L.orc_set_variant(self._h, int(open_rule), int(bool(quadrupole)))
         self.open_rule, self.quadrupole = int(open_rule), bool(quadrupole)
+        # variant R23: the group enters the opening test as its tight box (per-axis half extents)
+        L.orc_set_group_box(self._h, int(bool(group_box)))
+        self.group_box = bool(group_box)
         self.n_cells = int(L.orc_n_cells(self._h))
         self.n_leaves = int(L.orc_n_leaves(self._h))
         self.n_groups = int(L.orc_n_groups(self._h))
@@ -142,6 +147,12 @@ class Oracle:
         return b, h
 
     # ---- walk / forces ---------------------------------------------------
+    def ext32(self):
+        """fp32 half extents of every cell's tight box about its fp32 centre (R23): [n_cells,3]."""
+        e = np.zeros((self.n_cells, 3), np.float32)
+        _lib.orc_get_ext32(self._h, _p(e))
+        return e
+
     def walk(self, group: int, theta: float, shadow32: bool = False):
         """(cell_list, leaf_list, min_margin, n_flips, n_tests) of one group (O5)."""
         cap = self.n_cells

@@ -26,7 +26,9 @@
 //    direct sum  : N = 2, N = 3 closed forms; sum m a = 0
 //    variants    : R21 (opening test on the cell's centre of mass) and R22 (monopole-only cells), both off
 //                  by default: lists re-derived from the recursive definition, theta = 0, own cells open
-//                  in fp32, monopole closed form, error orders (tests/test_oracle_variants.py)
+//                  in fp32, monopole closed form, error orders (tests/test_oracle_variants.py);
+//                  R23 (the group enters the opening test as its tight box): hand-computed threshold of an
+//                  elongated group (tests/golden/group_box_threshold.txt), interval-gap brute force
 //  "parity unpinned": the opening RULE itself (R1) — the paper never prints
 //  its formula (PAPER.md:79 calls open_node, never defined) — and every value
 //  that lives only in Figs. 4-8.
@@ -56,6 +58,7 @@ struct OCell {
   double M, X[3];           // mass, centre of mass
   double Q[6];              // traceless quadrupole about X: xx,yy,zz,xy,xz,yz (R10)
   float b32[3], h32;        // fp32-rounded boundary (what an FP32 device stores)
+  float e32[3];             // R23: fp32 half extents of the tight box about b32, per axis, rounded up
 };
 
 struct Oracle {
@@ -64,6 +67,7 @@ struct Oracle {
   // variants (R21, R22): 0 = the default readings
   int open_rule = 0;   // 0: cube-to-cube distance (R1); 1: group cube to the cell's centre of mass (R21)
   int quadrupole = 1;  // 1: monopole + quadrupole (R10); 0: monopole only (R22)
+  int group_box = 0;   // 0: the group is its boundary cube (R9); 1: its tight box, per-axis half extents (R23)
   std::vector<double> x, y, z, m;  // inputs widened to fp64
   std::vector<int32_t> gx, gy, gz; // O1 integer grid coordinates
   double org[3], side;
@@ -154,6 +158,13 @@ void cell_properties(Oracle& T, OCell& c) {
   float hf = (float)far;
   if ((double)hf < far) hf = std::nextafterf(hf, std::numeric_limits<float>::infinity());
   c.h32 = hf;
+  // R23: the same containment argument per axis (the tight box seen from the rounded centre)
+  for (int k = 0; k < 3; k++) {
+    const double reach = std::max(c.bmax[k] - (double)c.b32[k], (double)c.b32[k] - c.bmin[k]);
+    float ef = (float)reach;
+    if ((double)ef < reach) ef = std::nextafterf(ef, std::numeric_limits<float>::infinity());
+    c.e32[k] = ef;
+  }
 }
 
 // ---- O2: recursive cubic subdivision (R4, R6, R7)
@@ -203,11 +214,14 @@ void find_groups(Oracle& T, int c) {
 // ---- O5: the opening test (List 2 PAPER.md:73-91 `open_node`; R1, R9, R14)
 //  fp64: d_k = max(0, |b_c,k - b_g,k| - h_c - h_g), open iff d^2 theta^2 <= (2 h_c)^2
 //  rule 1 (R21): the cell is represented by its centre of mass: d_k = max(0, |X_c,k - b_g,k| - h_g)
-inline bool open64(const OCell& c, const OCell& g, double theta, double* margin, int rule) {
+inline bool open64(const OCell& c, const OCell& g, double theta, double* margin, int rule, int gbox) {
   double d2 = 0.0;
   for (int k = 0; k < 3; k++) {
-    const double d = rule ? std::max(0.0, std::fabs(c.X[k] - g.b[k]) - g.h)
-                          : std::max(0.0, std::fabs(c.b[k] - g.b[k]) - c.h - g.h);
+    // the group's side of the test: half side of its boundary cube (R9), or, variant R23,
+    // the half extent of its tight box along this axis
+    const double hg = gbox ? (g.bmax[k] - g.bmin[k]) / 2.0 : g.h;
+    const double d = rule ? std::max(0.0, std::fabs(c.X[k] - g.b[k]) - hg)
+                          : std::max(0.0, std::fabs(c.b[k] - g.b[k]) - c.h - hg);
     d2 += d * d;
   }
   const double l = 2.0 * c.h;
@@ -220,10 +234,11 @@ inline bool open64(const OCell& c, const OCell& g, double theta, double* margin,
 //     d2 = fma(t_z,t_z, fma(t_y,t_y, t_x*t_x));  l = h_c + h_c
 //     open iff d2 * (theta*theta) <= l * l
 //  rule 1: the same sequence with the fp32 centre of mass in place of b_c and 0 in place of h_c
-inline bool open32(const OCell& c, const OCell& g, float theta, int rule) {
-  const float s = (rule ? 0.0f : c.h32) + g.h32;
+//  gbox (R23): s_k = h_c + e_g,k per axis in place of s
+inline bool open32(const OCell& c, const OCell& g, float theta, int rule, int gbox) {
   float t[3];
   for (int k = 0; k < 3; k++) {
+    const float s = (rule ? 0.0f : c.h32) + (gbox ? g.e32[k] : g.h32);
     const float u = (rule ? (float)c.X[k] : c.b32[k]) - g.b32[k];
     const float v = std::fabs(u) - s;
     t[k] = std::fmax(v, 0.0f);
@@ -261,8 +276,8 @@ void walk_group(const Oracle& T, int gcell, double theta, int mode, WalkOut& W) 
       if (ch < 0) continue;
       const OCell& C = T.cells[ch];
       double margin;
-      const bool o64 = open64(C, G, theta, &margin, T.open_rule);
-      const bool o32 = open32(C, G, (float)theta, T.open_rule);
+      const bool o64 = open64(C, G, theta, &margin, T.open_rule, T.group_box);
+      const bool o32 = open32(C, G, (float)theta, T.open_rule, T.group_box);
       W.n_tests++;
       W.min_margin = std::min(W.min_margin, margin);
       if (o64 != o32) W.n_flips++;
@@ -359,6 +374,9 @@ void orc_set_variant(void* h, int open_rule, int quadrupole) {
   T->open_rule = open_rule ? 1 : 0; T->quadrupole = quadrupole ? 1 : 0;
 }
 
+// variant R23: 1 = the group enters the opening test as its tight box
+void orc_set_group_box(void* h, int group_box) { ((Oracle*)h)->group_box = group_box ? 1 : 0; }
+
 int64_t orc_n_cells(void* h) { return (int64_t)((Oracle*)h)->cells.size(); }
 int64_t orc_n_leaves(void* h) { return ((Oracle*)h)->n_leaves; }
 int64_t orc_n_groups(void* h) { return (int64_t)((Oracle*)h)->groups.size(); }
@@ -413,6 +431,13 @@ void orc_get_bnd32(void* h, float* b32, float* h32) {
     for (int k = 0; k < 3; k++) b32[3 * c + k] = T->cells[c].b32[k];
     h32[c] = T->cells[c].h32;
   }
+}
+
+// R23: fp32 half extents of every cell's tight box about its fp32 centre: e32 [n_cells,3]
+void orc_get_ext32(void* h, float* e32) {
+  Oracle* T = (Oracle*)h;
+  for (size_t c = 0; c < T->cells.size(); c++)
+    for (int k = 0; k < 3; k++) e32[3 * c + k] = T->cells[c].e32[k];
 }
 
 // Walk one group (index into the group list).  Returns 0, or -1 if a list does not fit.
