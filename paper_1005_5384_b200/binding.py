@@ -26,7 +26,7 @@ TC_FLAG_HOST_ONLY = 1
 #: every symbol include/tc.h declares (checked by tests/test_abi.py)
 SYMBOLS = ["tc_create", "tc_create_ex", "tc_destroy", "tc_set_particles", "tc_build", "tc_forces",
            "tc_set_option", "tc_get_counts", "tc_get_stats", "tc_set_stream", "tc_sync",
-           "tc_last_error", "tc_get_tree", "tc_fp32_peak", "tc_direct"]
+           "tc_last_error", "tc_get_tree", "tc_get_group_boxes", "tc_fp32_peak", "tc_direct"]
 
 
 class tc_stats(C.Structure):
@@ -78,6 +78,7 @@ def lib():
     L.tc_last_error.restype = C.c_char_p
     L.tc_last_error.argtypes = [vp]
     L.tc_get_tree.argtypes = [vp] + [vp] * 6
+    L.tc_get_group_boxes.argtypes = [vp, vp]
     L.tc_fp32_peak.argtypes = [vp, C.POINTER(C.c_double)]
     L.tc_direct.argtypes = [vp, f32, vp, i64, vp, vp]
     _lib = L
@@ -158,6 +159,13 @@ def tc_get_tree(ctx) -> dict:
     out = dict(perm=np.zeros(n, np.int32), bnd=np.zeros((nc, 4), np.float32), xm=np.zeros((nc, 4), np.float32),
                q=np.zeros((nc, 6), np.float32), link=np.zeros((nc, 4), np.int32), groups=np.zeros(ng, np.int32))
     _check(ctx, lib().tc_get_tree(ctx, *[_ptr(out[k]) for k in ("perm", "bnd", "xm", "q", "link", "groups")]))
+    return out
+
+
+def tc_get_group_boxes(ctx) -> np.ndarray:
+    """fp32 half extents [n_groups,3] of every group's tight box (variant R23), groups in Morton order."""
+    out = np.zeros((tc_get_stats(ctx)["n_groups"], 3), np.float32)
+    _check(ctx, lib().tc_get_group_boxes(ctx, _ptr(out)))
     return out
 
 

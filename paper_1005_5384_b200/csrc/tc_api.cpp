@@ -26,7 +26,7 @@ struct tc_ctx {
   int n_group = 96;
   bool device_build = false;          // option "device_build": tc_build_gpu.cu instead of tc_build.cpp
   int stack_smem = 256;
-  int walk_only = 0, open_rule = 0, quadrupole = 1;
+  int walk_only = 0, open_rule = 0, quadrupole = 1, group_box = 0;
   bool two_pass = false;
   tc::TwoPassScratch tps;
   bool last_two_pass = false;
@@ -229,6 +229,10 @@ int tc_set_option(tc_ctx* c, const char* key, double v) {
     if (v != 0.0 && v != 1.0) return fail(c, TC_EINVAL, "tc_set_option: open_rule must be 0 or 1");
     c->open_rule = (int)v; return TC_OK;
   }
+  if (!std::strcmp(key, "group_box")) {
+    if (v != 0.0 && v != 1.0) return fail(c, TC_EINVAL, "tc_set_option: group_box must be 0 or 1");
+    c->group_box = (int)v; return TC_OK;
+  }
   if (!std::strcmp(key, "quadrupole")) {
     if (v != 0.0 && v != 1.0) return fail(c, TC_EINVAL, "tc_set_option: quadrupole must be 0 or 1");
     c->quadrupole = (int)v; return TC_OK;
@@ -377,6 +381,7 @@ int tc_build(tc_ctx* c, int n_leaf) {
     D.q0 = (const float4*)(b + T.lay.off_q0); D.q1 = (const float4*)(b + T.lay.off_q1);
     D.part = (const float4*)(b + T.lay.off_part); D.orig = (const int32_t*)(b + T.lay.off_orig);
     D.grp = (const int4*)(b + T.lay.off_grp);
+    D.gbox = (const float4*)(b + T.lay.off_gbox);
     D.n = c->n; D.n_cells = T.n_cells; D.n_groups = T.n_groups;
   }
   c->tree_host_valid = true;
@@ -417,7 +422,7 @@ int tc_forces(tc_ctx* c, float theta, float eps, float* acc, float* pot) {
   L.acc = acc_dev ? acc : c->d_acc;
   L.pot = pot ? (acc_dev ? pot : c->d_pot) : nullptr;
   L.n_pc = c->d_npc; L.n_pp = c->d_npp; L.counters = c->d_ctr; L.spill = c->d_spill; L.spill_cap = c->spill_cap;
-  L.stack_smem = c->stack_smem; L.n_sm = c->n_sm; L.flags = (c->walk_only ? 1 : 0) | (c->open_rule ? 2 : 0) | (c->quadrupole ? 0 : 4);
+  L.stack_smem = c->stack_smem; L.n_sm = c->n_sm; L.flags = (c->walk_only ? 1 : 0) | (c->open_rule ? 2 : 0) | (c->quadrupole ? 0 : 4) | (c->group_box ? 8 : 0);
   L.max_grid = (int)(warps / (size_t)tc::forces_warps_per_cta());
   // stream-ordered: no host synchronisation between queued calls; the overflow flag is sticky until collect()
   TC_CUDA(c, cudaMemsetAsync(c->d_ctr, 0, offsetof(tc::DeviceCounters, overflow), c->stream));
@@ -534,6 +539,16 @@ int tc_get_tree(tc_ctx* c, int32_t* perm, float* cell_bnd, float* cell_xm, float
     const int4* g = (const int4*)(b + T.lay.off_grp);
     for (int64_t i = 0; i < T.n_groups; i++) groups[i] = g[i].x;
   }
+  return TC_OK;
+}
+
+int tc_get_group_boxes(tc_ctx* c, float* half_ext) {
+  if (!c || !half_ext) return fail(c, TC_EINVAL, "tc_get_group_boxes: null argument");
+  const int e = tc_get_tree(c, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr);   // brings a device-built tree back
+  if (e != TC_OK) return e;
+  const tc::HostTree& T = c->tree;
+  const float4* gb = (const float4*)((const char*)T.packed + T.lay.off_gbox);
+  for (int64_t i = 0; i < T.n_groups; i++) { half_ext[3 * i] = gb[i].x; half_ext[3 * i + 1] = gb[i].y; half_ext[3 * i + 2] = gb[i].z; }
   return TC_OK;
 }
 

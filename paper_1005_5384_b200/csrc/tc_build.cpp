@@ -330,6 +330,7 @@ int build_host_tree(const float* pos, const float* mass, int64_t n, int n_leaf, 
   Y.off_part = off; off = align256(off + sizeof(float4) * (size_t)n);
   Y.off_orig = off; off = align256(off + sizeof(int32_t) * (size_t)n);
   Y.off_grp = off;  off = align256(off + sizeof(int4) * groups.size());
+  Y.off_gbox = off; off = align256(off + sizeof(float4) * groups.size());
   Y.bytes = off;
   char* base = (char*)alloc(alloc_user, Y.bytes);
   if (!base) { msg = "build: cannot allocate the packed tree buffer"; return TC_ENOMEM; }
@@ -340,6 +341,7 @@ int build_host_tree(const float* pos, const float* mass, int64_t n, int n_leaf, 
   float4* part = (float4*)(base + Y.off_part);
   int32_t* orig = (int32_t*)(base + Y.off_orig);
   int4* grp = (int4*)(base + Y.off_grp);
+  float4* gbox = (float4*)(base + Y.off_gbox);
   try { T.link.resize((size_t)nc * 4); T.q6.resize((size_t)nc * 6); } catch (...) { msg = "build: out of host memory"; return TC_ENOMEM; }
 
 #pragma omp parallel for schedule(static)
@@ -416,6 +418,17 @@ int build_host_tree(const float* pos, const float* mass, int64_t n, int n_leaf, 
     for (size_t g = 0; g < groups.size(); g++) {
       const int32_t c = groups[g];
       grp[g] = make_int4(c, c_begin[c], c_count[c], order[g]);
+      // variant R23: half extents of the tight box about the fp32 centre of the boundary cube, per axis,
+      // rounded towards +inf (the R20 construction axis by axis; their maximum is the cube's half side)
+      float e[3];
+      for (int k = 0; k < 3; k++) {
+        const double lo = (double)prop[c].bmin[k], hi = (double)prop[c].bmax[k];
+        const float bk = (float)(0.5 * (lo + hi));
+        const double reach = std::fmax(hi - (double)bk, (double)bk - lo);
+        e[k] = (float)reach;
+        if ((double)e[k] < reach) e[k] = std::nextafter(e[k], HUGE_VALF);
+      }
+      gbox[g] = make_float4(e[0], e[1], e[2], 0.f);
     }
   }
   lap("schedule");

@@ -288,11 +288,21 @@ __global__ void k_iota(unsigned int* a, int n) {
 }
 
 __global__ void k_pack_groups(const int* __restrict__ gcell_sorted, const unsigned int* __restrict__ sched, int ng,
-                              const int* __restrict__ c_begin, const int* __restrict__ c_count, int4* __restrict__ grp) {
+                              const int* __restrict__ c_begin, const int* __restrict__ c_count,
+                              const Moments* __restrict__ mom, int4* __restrict__ grp, float4* __restrict__ gbox) {
   const int g = blockIdx.x * blockDim.x + threadIdx.x;
   if (g >= ng) return;
   const int c = gcell_sorted[g];
   grp[g] = make_int4(c, c_begin[c], c_count[c], (int)sched[g]);
+  // variant R23: half extents of the tight box about the fp32 centre, per axis, rounded up
+  float e[3];
+#pragma unroll
+  for (int k = 0; k < 3; k++) {
+    const double lo = (double)mom[c].bmin[k], hi = (double)mom[c].bmax[k];
+    const float bk = (float)(0.5 * (lo + hi));
+    e[k] = __double2float_ru(fmax(hi - (double)bk, (double)bk - lo));
+  }
+  gbox[g] = make_float4(e[0], e[1], e[2], 0.f);
 }
 
 inline size_t align256(size_t x) { return (x + 255) & ~(size_t)255; }
@@ -514,6 +524,7 @@ int build_device_tree(const float4* src, int64_t n, int n_leaf, int n_group, Dev
   Y.off_part = off; off = align256(off + sizeof(float4) * (size_t)n);
   Y.off_orig = off; off = align256(off + sizeof(int32_t) * (size_t)n);
   Y.off_grp = off;  off = align256(off + sizeof(int4) * (size_t)ng);
+  Y.off_gbox = off; off = align256(off + sizeof(float4) * (size_t)ng);
   Y.bytes = off;
   if (*d_tree_cap < Y.bytes) {
     TCG_CUDA(cudaStreamSynchronize(st));
@@ -527,6 +538,7 @@ int build_device_tree(const float4* src, int64_t n, int n_leaf, int n_group, Dev
   D.q0 = (const float4*)(base + Y.off_q0);   D.q1 = (const float4*)(base + Y.off_q1);
   D.part = (const float4*)(base + Y.off_part); D.orig = (const int32_t*)(base + Y.off_orig);
   D.grp = (const int4*)(base + Y.off_grp);
+  D.gbox = (const float4*)(base + Y.off_gbox);
   D.n = n; D.n_cells = nc; D.n_groups = ng;
   TCG_GROW(S.link, S.cap_link, nc, false);
   TCG_GROW(S.q6, S.cap_q6, 6 * (size_t)nc, false);
@@ -534,7 +546,8 @@ int build_device_tree(const float4* src, int64_t n, int n_leaf, int n_group, Dev
                                            n_group, (float4*)D.bnd, (float4*)D.xm, (float4*)D.q0, (float4*)D.q1, S.link, S.q6);
   k_pack_particles<<<blocks(n), 256, 0, st>>>(src, S.idx, n, (float4*)D.part, (int*)D.orig);
   // after the two sorts: gcell_sorted = group cells in Morton order, gval = schedule
-  k_pack_groups<<<blocks(ng), 256, 0, st>>>(S.gcell_sorted, S.gval, (int)ng, S.c_begin, S.c_count, (int4*)D.grp);
+  k_pack_groups<<<blocks(ng), 256, 0, st>>>(S.gcell_sorted, S.gval, (int)ng, S.c_begin, S.c_count, (const Moments*)S.mom,
+                                            (int4*)D.grp, (float4*)D.gbox);
   TCG_CUDA(cudaGetLastError());
   TCG_CUDA(cudaStreamSynchronize(st));
   return TC_OK;

@@ -26,8 +26,10 @@ constexpr int kMaxLevel = 21;  // 3 x 21 = 63-bit Morton keys (R7)
 //   orig[i] = caller's index of tree-order particle i
 //   grp [g] = (cell, first_body, n_body, sched)  groups in Morton order; sched = index of the
 //             g-th group to RUN (costly groups first, tc_build.cpp)
+//   gbox[g] = (ex, ey, ez, 0)       half extents of the group's TIGHT box about bnd[cell].xyz, rounded up
+//             (variant R23, option "group_box"; max(ex,ey,ez) == |bnd[cell].w|)
 struct PackedLayout {
-  size_t off_bnd = 0, off_xm = 0, off_q0 = 0, off_q1 = 0, off_part = 0, off_orig = 0, off_grp = 0;
+  size_t off_bnd = 0, off_xm = 0, off_q0 = 0, off_q1 = 0, off_part = 0, off_orig = 0, off_grp = 0, off_gbox = 0;
   size_t bytes = 0;
 };
 
@@ -61,6 +63,7 @@ struct DeviceTree {
   const float4* part = nullptr;
   const int32_t* orig = nullptr;
   const int4* grp = nullptr;
+  const float4* gbox = nullptr;
   int64_t n = 0, n_cells = 0, n_groups = 0;
 };
 
@@ -84,7 +87,7 @@ struct ForceLaunch {
   uint32_t* spill = nullptr;  // device [n_warps_total * spill_cap]
   int spill_cap = 0;
   int stack_smem = 256;
-  int flags = 0;              // bit 0: walk_only (measurement aid), bit 1: COM opening rule (R21), bit 2: monopole only (R22)
+  int flags = 0;              // bit 0: walk_only (measurement aid), bit 1: COM opening rule (R21), bit 2: monopole only (R22), bit 3: group = its tight box (R23)
   int n_sm = 148;
   int max_grid = 0;           // CTAs the spill buffer has room for (0: no limit)
 };

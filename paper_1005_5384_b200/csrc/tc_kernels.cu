@@ -362,13 +362,13 @@ struct ListIO {
 };
 
 enum { kFused = 0, kCount = 1, kWrite = 2 };
-enum { kFlagWalkOnly = 1, kFlagComRule = 2, kFlagMonopole = 4 };   // run-time variants of a launch
+enum { kFlagWalkOnly = 1, kFlagComRule = 2, kFlagMonopole = 4, kFlagGroupBox = 8 };   // run-time variants of a launch
 
 template <int STK, bool kEps0, int MODE = kFused>
 __global__ void __launch_bounds__(kWarpsPerCta * 32, TC_MINB)
 forces_kernel(const float4* __restrict__ bnd, const float4* __restrict__ xm, const float4* __restrict__ q0,
               const float4* __restrict__ q1, const float4* __restrict__ part, const int32_t* __restrict__ orig,
-              const int4* __restrict__ grp, int n_groups, float theta, float eps,
+              const int4* __restrict__ grp, const float4* __restrict__ gbox, int n_groups, float theta, float eps,
               float* __restrict__ acc, float* __restrict__ pot, int32_t* __restrict__ out_npc,
               int32_t* __restrict__ out_npp, DeviceCounters* __restrict__ ctr, uint32_t* __restrict__ spill_all,
               int spill_cap, int flags, ListIO lio) {
@@ -380,6 +380,7 @@ forces_kernel(const float4* __restrict__ bnd, const float4* __restrict__ xm, con
   const float th2 = __fmul_rn(theta, theta);
   const unsigned lt_mask = (1u << lane) - 1u;
   const bool walk_only = flags & kFlagWalkOnly, com_rule = flags & kFlagComRule, mono = flags & kFlagMonopole;
+  const bool group_box = flags & kFlagGroupBox;
 
   // root: a leaf root is never tested (O5) — its bodies are the whole leaf list
   const float4 root_b = __ldg(bnd);
@@ -396,6 +397,9 @@ forces_kernel(const float4* __restrict__ bnd, const float4* __restrict__ xm, con
     const int4 G = __ldg(grp + g);           // (cell, first_body, n_body, -)
     const float4 gb = __ldg(bnd + G.x);
     const float gbx = gb.x, gby = gb.y, gbz = gb.z, gh = fabsf(gb.w);
+    // the group's side of the test: the half side of its cube (R9) or, variant R23, the half extents of its tight box
+    float ghx = gh, ghy = gh, ghz = gh;
+    if (group_box) { const float4 e = __ldg(gbox + g); ghx = e.x; ghy = e.y; ghz = e.z; }
 
     // groups larger than kPass particles (level-21 leaves, or a large N_group) repeat the walk per kPass
     for (int pb = 0; pb < G.z; pb += kPass) {
@@ -443,11 +447,12 @@ forces_kernel(const float4* __restrict__ bnd, const float4* __restrict__ xm, con
         // open_node (O5/R16): one fixed sequence of correctly rounded fp32 operations
         // (variant R21, com_rule: the cell's centre of mass in place of b_c, 0 in place of h_c in the distance)
         const float hc = fabsf(cb.w);
-        const float s = __fadd_rn(com_rule ? 0.f : hc, gh);
+        const float hs = com_rule ? 0.f : hc;
+        const float sx = __fadd_rn(hs, ghx), sy = __fadd_rn(hs, ghy), sz = __fadd_rn(hs, ghz);
         const float px = com_rule ? cx.x : cb.x, py = com_rule ? cx.y : cb.y, pz = com_rule ? cx.z : cb.z;
-        const float tx = fmaxf(__fsub_rn(fabsf(__fsub_rn(px, gbx)), s), 0.f);
-        const float ty = fmaxf(__fsub_rn(fabsf(__fsub_rn(py, gby)), s), 0.f);
-        const float tz = fmaxf(__fsub_rn(fabsf(__fsub_rn(pz, gbz)), s), 0.f);
+        const float tx = fmaxf(__fsub_rn(fabsf(__fsub_rn(px, gbx)), sx), 0.f);
+        const float ty = fmaxf(__fsub_rn(fabsf(__fsub_rn(py, gby)), sy), 0.f);
+        const float tz = fmaxf(__fsub_rn(fabsf(__fsub_rn(pz, gbz)), sz), 0.f);
         const float d2 = __fmaf_rn(tz, tz, __fmaf_rn(ty, ty, __fmul_rn(tx, tx)));
         const float l = __fadd_rn(hc, hc);
         const bool open = valid && (__fmul_rn(d2, th2) <= __fmul_rn(l, l));
@@ -631,7 +636,7 @@ int launch_t(const DeviceTree& T, const ForceLaunch& L, cudaStream_t st, int* ct
   // persistent grid: every SM full, groups handed out by an atomic counter
   // (never more CTAs than the spill buffer was sized for: forces_total_warps)
   const int grid = L.max_grid > 0 ? std::min(L.n_sm * per_sm, L.max_grid) : L.n_sm * per_sm;
-  kern<<<grid, kWarpsPerCta * 32, smem, st>>>(T.bnd, T.xm, T.q0, T.q1, T.part, T.orig, T.grp, (int)T.n_groups,
+  kern<<<grid, kWarpsPerCta * 32, smem, st>>>(T.bnd, T.xm, T.q0, T.q1, T.part, T.orig, T.grp, T.gbox, (int)T.n_groups,
                                                L.theta, L.eps, L.acc, L.pot, L.n_pc, L.n_pp, L.counters, L.spill,
                                                L.spill_cap, L.flags, lio);
   return (int)cudaGetLastError();

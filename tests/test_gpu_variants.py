@@ -18,8 +18,10 @@ def _built():
     tc_build.build()
 
 
-def _run(pos, mass, theta, eps, n_leaf, n_group, open_rule, quadrupole, two_pass=0):
+def _run(pos, mass, theta, eps, n_leaf, n_group, open_rule, quadrupole, two_pass=0, group_box=0, device_build=0):
     with B.TreeCode(n_group=n_group) as tc:
+        tc.set_option("group_box", group_box)
+        tc.set_option("device_build", device_build)
         tc.set_option("open_rule", open_rule)
         tc.set_option("quadrupole", quadrupole)
         tc.set_option("two_pass", two_pass)
@@ -39,6 +41,34 @@ def test_variants_match_the_oracle_variant(open_rule, quadrupole, name, n_leaf, 
     ref = o.forces(theta, eps, shadow32=True, stats=True)
     check(acc, pot, n_pc, n_pp, ref)
     assert st["n_tests_total"] == int(ref["tests"].sum())
+
+
+@pytest.mark.parametrize("open_rule,device_build,two_pass", [(0, 0, 0), (1, 0, 0), (0, 1, 0), (0, 0, 1)])
+@pytest.mark.parametrize("name,n_leaf,n_group", [("plummer_1k", 16, 64), ("plummer_64k", 16, 96), ("cube_64k", 4, 32)])
+def test_group_box_matches_the_oracle_variant(open_rule, device_build, two_pass, name, n_leaf, n_group):
+    """R23 (option "group_box"): the group enters the opening test as its tight box — host and device builds,
+    with the COM rule, in the two-pass pipeline; counts exact against the oracle's fp32 shadow of R23."""
+    pos, mass, theta, eps, _ = inputs.make(name)
+    acc, pot, n_pc, n_pp, st = _run(pos, mass, theta, eps, n_leaf, n_group, open_rule, 1, two_pass=two_pass,
+                                    group_box=1, device_build=device_build)
+    o = Oracle(pos, mass, n_leaf, n_group, open_rule=open_rule, group_box=True)
+    ref = o.forces(theta, eps, shadow32=True, stats=True)
+    check(acc, pot, n_pc, n_pp, ref)
+    assert st["n_tests_total"] == int(ref["tests"].sum())
+    base = Oracle(pos, mass, n_leaf, n_group, open_rule=open_rule).forces(theta, eps, shadow32=True)
+    assert ref["interactions"] < base["interactions"]
+
+
+def test_group_box_device_build_boxes_identical():
+    pos, mass, *_ = inputs.make("plummer_64k")
+    out = []
+    for dev in (0, 1):
+        with B.TreeCode(n_group=96) as tc:
+            tc.set_option("device_build", dev)
+            tc.set_particles(pos, mass)
+            tc.build(16)
+            out.append(B.tc_get_group_boxes(tc.ctx))
+    assert np.array_equal(out[0], out[1])
 
 
 def test_variants_in_the_two_pass_pipeline_and_eps0():

@@ -25,6 +25,7 @@ def _compare(pos, mass, n_leaf, n_group):
         tc.set_particles(pos, mass)
         tc.build(n_leaf)
         s, tr = tc.stats(), tc.tree()
+        gbox = B.tc_get_group_boxes(tc.ctx)
     o = Oracle(pos, mass, n_leaf, n_group)
     assert (s["n_cells"], s["n_leaves"], s["n_groups"], s["depth"]) == (o.n_cells, o.n_leaves, o.n_groups, o.depth)
     n = len(mass)
@@ -65,6 +66,9 @@ def _compare(pos, mass, n_leaf, n_group):
     assert (np.abs(tr["q"] - oc["Q"][idx]) / qs).max() <= 2e-7
     # groups in the same (Morton) order
     assert np.array_equal(idx[tr["groups"]], o.groups())
+    # tight boxes of the groups (variant R23): bit-identical fp32 half extents, their maximum is the cube's half side
+    assert np.array_equal(gbox, o.ext32()[o.groups()])
+    assert np.array_equal(gbox.max(axis=1), tr["bnd"][tr["groups"], 3])
 
 
 @pytest.mark.parametrize("name,n_group", [("plummer_1k", 16), ("plummer_1k", 64), ("plummer_64k", 64), ("cube_64k", 16)])
