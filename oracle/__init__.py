@@ -206,3 +206,35 @@ def direct(pos, mass, eps: float, targets=None):
     pot = np.zeros(nt)
     L.orc_direct(n, _p(pos), _p(mass), float(eps), nt, _p(t), _p(acc), _p(pot))
     return acc, pot
+
+
+# ---- time integration (BASELINE.json config 5; the paper leaves it on the host) -------------
+def leapfrog_kdk(pos, vel, dt: float, steps: int, force, acc0=None):
+    """Kick-drift-kick leapfrog in fp64, step by step as BASELINE.json config 5 writes it:
+
+        v += a dt/2 ;  x += v dt ;  a = force(x) ;  v += a dt/2
+
+    ``force(x64) -> (acc64, pot64)`` is any force law (``tree_force`` below, or an exact one in the pins).
+    Returns (pos, vel, acc, pot) after ``steps`` steps; the inputs are not modified.
+    Pins (tests/test_oracle_leapfrog.py): two-body circular orbit closed form, second-order convergence,
+    exact time reversibility, momentum conservation.
+    """
+    x = np.array(pos, dtype=np.float64, copy=True)
+    v = np.array(vel, dtype=np.float64, copy=True)
+    a, p = force(x) if acc0 is None else (np.array(acc0, dtype=np.float64, copy=True), None)
+    for _ in range(int(steps)):
+        v += a * (0.5 * dt)
+        x += v * dt
+        a, p = force(x)
+        v += a * (0.5 * dt)
+    return x, v, a, p
+
+
+def tree_force(mass, theta: float, eps: float, n_leaf: int = 16, n_group=None, shadow32: bool = True, **variants):
+    """Force law for ``leapfrog_kdk``: a new Oracle tree on the positions ROUNDED TO fp32 (what the library is
+    handed each step), opening decisions in the fp32 shadow by default (R16)."""
+    def f(x64):
+        o = Oracle(x64.astype(np.float32), mass, n_leaf, n_group, **variants)
+        r = o.forces(theta, eps, shadow32=shadow32)
+        return r["acc"], r["pot"]
+    return f

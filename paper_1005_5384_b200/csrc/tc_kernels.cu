@@ -364,7 +364,8 @@ struct ListIO {
 enum { kFused = 0, kCount = 1, kWrite = 2 };
 enum { kFlagWalkOnly = 1, kFlagComRule = 2, kFlagMonopole = 4, kFlagGroupBox = 8 };   // run-time variants of a launch
 
-template <int STK, bool kEps0, int MODE = kFused>
+// kPlain: the launch uses none of the variant readings (R21-R23), so their selects are compiled out
+template <int STK, bool kEps0, int MODE = kFused, bool kPlain = false>
 __global__ void __launch_bounds__(kWarpsPerCta * 32, TC_MINB)
 forces_kernel(const float4* __restrict__ bnd, const float4* __restrict__ xm, const float4* __restrict__ q0,
               const float4* __restrict__ q1, const float4* __restrict__ part, const int32_t* __restrict__ orig,
@@ -379,8 +380,9 @@ forces_kernel(const float4* __restrict__ bnd, const float4* __restrict__ xm, con
   const float eps2 = eps * eps;
   const float th2 = __fmul_rn(theta, theta);
   const unsigned lt_mask = (1u << lane) - 1u;
-  const bool walk_only = flags & kFlagWalkOnly, com_rule = flags & kFlagComRule, mono = flags & kFlagMonopole;
-  const bool group_box = flags & kFlagGroupBox;
+  const bool walk_only = flags & kFlagWalkOnly;
+  const bool com_rule = !kPlain && (flags & kFlagComRule), mono = !kPlain && (flags & kFlagMonopole);
+  const bool group_box = !kPlain && (flags & kFlagGroupBox);
 
   // root: a leaf root is never tested (O5) — its bodies are the whole leaf list
   const float4 root_b = __ldg(bnd);
@@ -441,9 +443,9 @@ forces_kernel(const float4* __restrict__ bnd, const float4* __restrict__ xm, con
         const uint32_t packed = (slot < npop) ? sm.stack[ssz - 1 - slot] : 0u;
         ssz -= npop;
         const bool valid = (slot < npop) && (k <= (int)(packed & 7u));
-        const int c = (int)(packed >> 3) + k;
-        float4 cb = make_float4(0.f, 0.f, 0.f, 0.f), cx = cb, c0 = cb, c1 = cb;
-        if (valid) { cb = __ldg(bnd + c); cx = __ldg(xm + c); c0 = __ldg(q0 + c); c1 = __ldg(q1 + c); }
+        // lanes without a child load cell 0 (the root always exists); `valid` masks everything they compute
+        const int c = valid ? (int)(packed >> 3) + k : 0;
+        const float4 cb = __ldg(bnd + c), cx = __ldg(xm + c), c0 = __ldg(q0 + c), c1 = __ldg(q1 + c);
         // open_node (O5/R16): one fixed sequence of correctly rounded fp32 operations
         // (variant R21, com_rule: the cell's centre of mass in place of b_c, 0 in place of h_c in the distance)
         const float hc = fabsf(cb.w);
@@ -622,9 +624,9 @@ leaf_kernel(const float4* __restrict__ part, const int32_t* __restrict__ orig, c
   }
 }
 
-template <int STK, bool kEps0, int MODE = kFused>
+template <int STK, bool kEps0, int MODE = kFused, bool kPlain = false>
 int launch_t(const DeviceTree& T, const ForceLaunch& L, cudaStream_t st, int* ctas_per_sm_out, ListIO lio = ListIO()) {
-  auto kern = forces_kernel<STK, kEps0, MODE>;
+  auto kern = forces_kernel<STK, kEps0, MODE, kPlain>;
   const size_t smem = sizeof(WarpSmem<STK>) * kWarpsPerCta;
   cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
   if (e != cudaSuccess) return (int)e;
@@ -645,6 +647,8 @@ int launch_t(const DeviceTree& T, const ForceLaunch& L, cudaStream_t st, int* ct
 int dispatch(const DeviceTree& T, const ForceLaunch& L, cudaStream_t st, int* per_sm) {
   const bool eps0 = (L.eps * L.eps == 0.f);
   if (L.stack_smem == 64) return eps0 ? launch_t<64, true>(T, L, st, per_sm) : launch_t<64, false>(T, L, st, per_sm);
+  if ((L.flags & (kFlagComRule | kFlagMonopole | kFlagGroupBox)) == 0)   // the default readings: no variant selects
+    return eps0 ? launch_t<256, true, kFused, true>(T, L, st, per_sm) : launch_t<256, false, kFused, true>(T, L, st, per_sm);
   return eps0 ? launch_t<256, true>(T, L, st, per_sm) : launch_t<256, false>(T, L, st, per_sm);
 }
 
