@@ -168,6 +168,22 @@ const char* tc_last_error(const tc_ctx* ctx);
 int tc_get_tree(tc_ctx* ctx, int32_t* perm, float* cell_bnd, float* cell_xm, float* cell_q,
                 int32_t* cell_link, int32_t* groups);
 
+/* `steps` kick-drift-kick leapfrog steps entirely on the device (BASELINE.json config 5;
+ * the paper leaves time integration to the host).  Per step, in fp32:
+ *     v += a dt/2 ;  x += v dt ;  tc_set_particles(x, mass) ; tc_build(n_leaf) ; a = tc_forces(theta, eps) ;  v += a dt/2
+ *   pos, vel, acc [n,3], mass, pot [n] (pot may be NULL): DEVICE arrays owned by the caller, pos / vel / acc / pot
+ *   16-byte aligned; pos, vel, acc, pot are updated in place and hold x, v, a(x), phi(x) of the last step on return.
+ *   have_acc != 0: acc already holds a(pos) (e.g. from a previous call) and the initial force evaluation is
+ *   skipped; with have_acc == 0 (or steps == 0) the forces at the start are evaluated first.
+ * The tree is rebuilt every step by the context's builder (option "device_build": nothing leaves the device;
+ * default host build: positions go to the host and the packed tree comes back each step, as in the paper).
+ * Stream-ordered like tc_forces with device pointers: call tc_sync before reading the arrays elsewhere.
+ * tc_get_stats / tc_get_counts then describe the LAST force evaluation.
+ * Errors: TC_EINVAL (null / host pointer / misaligned / n < 1 / steps < 0 / non-finite dt, theta, eps; a particle
+ * that left the finite range is reported by the tc_set_particles of that step), TC_ESTATE (host-only context). */
+int tc_leapfrog(tc_ctx* ctx, float* pos, float* vel, const float* mass, int64_t n, float dt, int steps, int n_leaf,
+                float theta, float eps, float* acc, float* pot, int have_acc);
+
 /* Half extents of every group's TIGHT box about the centre of its boundary cube (variant R23, option
  * "group_box"), fp32, rounded up so that the box contains every particle of the group:
  *   half_ext [n_groups,3]  HOST array, groups in Morton order (as `groups` of tc_get_tree).

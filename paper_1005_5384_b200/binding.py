@@ -26,7 +26,7 @@ TC_FLAG_HOST_ONLY = 1
 #: every symbol include/tc.h declares (checked by tests/test_abi.py)
 SYMBOLS = ["tc_create", "tc_create_ex", "tc_destroy", "tc_set_particles", "tc_build", "tc_forces",
            "tc_set_option", "tc_get_counts", "tc_get_stats", "tc_set_stream", "tc_sync",
-           "tc_last_error", "tc_get_tree", "tc_get_group_boxes", "tc_fp32_peak", "tc_direct"]
+           "tc_last_error", "tc_get_tree", "tc_get_group_boxes", "tc_leapfrog", "tc_fp32_peak", "tc_direct"]
 
 
 class tc_stats(C.Structure):
@@ -79,6 +79,7 @@ def lib():
     L.tc_last_error.argtypes = [vp]
     L.tc_get_tree.argtypes = [vp] + [vp] * 6
     L.tc_get_group_boxes.argtypes = [vp, vp]
+    L.tc_leapfrog.argtypes = [vp, vp, vp, vp, i64, f32, i32, i32, f32, f32, vp, vp, i32]
     L.tc_fp32_peak.argtypes = [vp, C.POINTER(C.c_double)]
     L.tc_direct.argtypes = [vp, f32, vp, i64, vp, vp]
     _lib = L
@@ -132,7 +133,8 @@ def tc_set_option(ctx, key: str, value: float):
     _check(ctx, lib().tc_set_option(ctx, key.encode(), float(value)))
 
 
-def tc_get_counts(ctx, n: int):
+def tc_get_counts(ctx, n: int | None = None):
+    n = tc_get_stats(ctx)["n"]          # the library writes one entry per particle of the built tree
     n_pc = np.zeros(n, np.int32)
     n_pp = np.zeros(n, np.int32)
     _check(ctx, lib().tc_get_counts(ctx, _ptr(n_pc), _ptr(n_pp)))
@@ -167,6 +169,13 @@ def tc_get_group_boxes(ctx) -> np.ndarray:
     out = np.zeros((tc_get_stats(ctx)["n_groups"], 3), np.float32)
     _check(ctx, lib().tc_get_group_boxes(ctx, _ptr(out)))
     return out
+
+
+def tc_leapfrog(ctx, pos, vel, mass, dt: float, steps: int, n_leaf: int, theta: float, eps: float, acc, pot=None,
+                have_acc: bool = False):
+    """`steps` KDK steps on the device; pos, vel, mass, acc, pot are torch CUDA tensors updated in place."""
+    _check(ctx, lib().tc_leapfrog(ctx, _ptr(pos), _ptr(vel), _ptr(mass), int(mass.shape[0]), float(dt), int(steps),
+                                  int(n_leaf), float(theta), float(eps), _ptr(acc), _ptr(pot), int(bool(have_acc))))
 
 
 def tc_direct(ctx, eps: float, targets, acc, pot=None):
@@ -238,7 +247,7 @@ class TreeCode:
         return acc, pot
 
     def counts(self):
-        return tc_get_counts(self.ctx, self.n)
+        return tc_get_counts(self.ctx)
 
     def stats(self):
         return tc_get_stats(self.ctx)

@@ -502,6 +502,37 @@ int tc_direct(tc_ctx* c, float eps, const int64_t* targets, int64_t n_targets, d
   return TC_OK;
 }
 
+int tc_leapfrog(tc_ctx* c, float* pos, float* vel, const float* mass, int64_t n, float dt, int steps, int n_leaf,
+                float theta, float eps, float* acc, float* pot, int have_acc) {
+  if (!c) return TC_EINVAL;
+  if (c->host_only) return fail(c, TC_ESTATE, "tc_leapfrog: host-only context has no device (there is no CPU fallback)");
+  if (!pos || !vel || !mass || !acc) return fail(c, TC_EINVAL, "tc_leapfrog: null argument");
+  if (n < 1 || n > 2147483647LL) return fail(c, TC_EINVAL, "tc_leapfrog: n must be in [1, 2^31-1]");
+  if (steps < 0 || !std::isfinite(dt)) return fail(c, TC_EINVAL, "tc_leapfrog: steps must be >= 0 and dt finite");
+  const void* ptrs[5] = {pos, vel, mass, acc, pot};
+  for (int k = 0; k < 5; k++) {
+    if (!ptrs[k]) continue;
+    if (!is_device_ptr(c, ptrs[k])) return fail(c, TC_EINVAL, "tc_leapfrog: pos, vel, mass, acc and pot must be DEVICE pointers");
+    if (k != 2 && (reinterpret_cast<uintptr_t>(ptrs[k]) & 15u)) return fail(c, TC_EINVAL, "tc_leapfrog: arrays must be 16-byte aligned");
+  }
+  auto force = [&]() -> int {          // the user's three calls, with device pointers: nothing crosses PCIe with device_build
+    int e = tc_set_particles(c, pos, mass, n);
+    if (e == TC_OK) e = tc_build(c, n_leaf);
+    if (e == TC_OK) e = tc_forces(c, theta, eps, acc, pot);
+    return e;
+  };
+  if (!have_acc || steps == 0) { const int e = force(); if (e != TC_OK) return e; }
+  for (int s = 0; s < steps; s++) {
+    int le = tc::launch_kick_drift(pos, vel, acc, n, dt, c->n_sm, c->stream);
+    if (le != 0) return cuda_fail(c, (cudaError_t)le, "kick-drift kernel launch");
+    const int e = force();
+    if (e != TC_OK) return e;
+    le = tc::launch_kick(vel, acc, n, dt, c->n_sm, c->stream);
+    if (le != 0) return cuda_fail(c, (cudaError_t)le, "kick kernel launch");
+  }
+  return TC_OK;
+}
+
 int tc_fp32_peak(tc_ctx* c, double* tflops) {
   if (!c || !tflops) return fail(c, TC_EINVAL, "tc_fp32_peak: null argument");
   if (c->host_only) return fail(c, TC_ESTATE, "tc_fp32_peak: host-only context has no device");

@@ -149,6 +149,10 @@ int pack_src_device(const float* pos, const float* mass, int64_t n, float4* out,
 // acc [n_t,3] / pot [n_t] device fp64 (zeroed inside).  Returns a cudaError_t as int.
 int launch_direct(const float4* src, long long n, const long long* targets, long long n_t, float eps, double* acc,
                   double* pot, int n_sm, void* stream);
+// Leapfrog pieces (tc_leapfrog): v += a dt/2 ; x += v dt  and  v += a dt/2 over [n,3] device arrays
+// (16-byte aligned).  Return a cudaError_t as int.
+int launch_kick_drift(float* pos, float* vel, const float* acc, long long n, float dt, int n_sm, void* stream);
+int launch_kick(float* vel, const float* acc, long long n, float dt, int n_sm, void* stream);
 // FFMA-only microbenchmark (tc_fp32_peak): returns a cudaError_t as int, *tflops on success.
 int measure_fp32_peak(int n_sm, void* stream, double* tflops);
 

@@ -881,6 +881,62 @@ int launch_direct(const float4* src, long long n, const long long* targets, long
   return (int)cudaGetLastError();
 }
 
+// ---- tc_leapfrog: the kicks and the drift of a KDK step (BASELINE.json config 5), element-wise over [3n]
+namespace {
+// v += a dt/2 ; x += v dt   (HBM-bound: 3 reads + 2 writes of 4 bytes per element, float4-vectorised body)
+__global__ void __launch_bounds__(256) kick_drift_kernel(float* __restrict__ x, float* __restrict__ v,
+                                                         const float* __restrict__ a, long long n3, float hdt, float dt) {
+  const long long stride = (long long)gridDim.x * blockDim.x;
+  const long long n4 = n3 >> 2;
+  float4* x4 = reinterpret_cast<float4*>(x);
+  float4* v4 = reinterpret_cast<float4*>(v);
+  const float4* a4 = reinterpret_cast<const float4*>(a);
+  for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n4; i += stride) {
+    float4 xv = x4[i], vv = v4[i];
+    const float4 av = __ldg(a4 + i);
+    vv.x = __fmaf_rn(av.x, hdt, vv.x); vv.y = __fmaf_rn(av.y, hdt, vv.y);
+    vv.z = __fmaf_rn(av.z, hdt, vv.z); vv.w = __fmaf_rn(av.w, hdt, vv.w);
+    xv.x = __fmaf_rn(vv.x, dt, xv.x); xv.y = __fmaf_rn(vv.y, dt, xv.y);
+    xv.z = __fmaf_rn(vv.z, dt, xv.z); xv.w = __fmaf_rn(vv.w, dt, xv.w);
+    v4[i] = vv; x4[i] = xv;
+  }
+  for (long long i = 4 * n4 + (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n3; i += stride) {   // ragged tail
+    const float vv = __fmaf_rn(a[i], hdt, v[i]);
+    v[i] = vv; x[i] = __fmaf_rn(vv, dt, x[i]);
+  }
+}
+// v += a dt/2
+__global__ void __launch_bounds__(256) kick_kernel(float* __restrict__ v, const float* __restrict__ a, long long n3, float hdt) {
+  const long long stride = (long long)gridDim.x * blockDim.x;
+  const long long n4 = n3 >> 2;
+  float4* v4 = reinterpret_cast<float4*>(v);
+  const float4* a4 = reinterpret_cast<const float4*>(a);
+  for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n4; i += stride) {
+    float4 vv = v4[i];
+    const float4 av = __ldg(a4 + i);
+    vv.x = __fmaf_rn(av.x, hdt, vv.x); vv.y = __fmaf_rn(av.y, hdt, vv.y);
+    vv.z = __fmaf_rn(av.z, hdt, vv.z); vv.w = __fmaf_rn(av.w, hdt, vv.w);
+    v4[i] = vv;
+  }
+  for (long long i = 4 * n4 + (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n3; i += stride)
+    v[i] = __fmaf_rn(a[i], hdt, v[i]);
+}
+}  // namespace
+
+// pos / vel / acc must be 16-byte aligned (checked by tc_leapfrog)
+int launch_kick_drift(float* pos, float* vel, const float* acc, long long n, float dt, int n_sm, void* stream) {
+  const long long n3 = 3 * n;
+  const int grid = (int)std::min<long long>((n3 / 4 + 255) / 256 + 1, 8LL * n_sm);
+  kick_drift_kernel<<<grid, 256, 0, (cudaStream_t)stream>>>(pos, vel, acc, n3, 0.5f * dt, dt);
+  return (int)cudaGetLastError();
+}
+int launch_kick(float* vel, const float* acc, long long n, float dt, int n_sm, void* stream) {
+  const long long n3 = 3 * n;
+  const int grid = (int)std::min<long long>((n3 / 4 + 255) / 256 + 1, 8LL * n_sm);
+  kick_kernel<<<grid, 256, 0, (cudaStream_t)stream>>>(vel, acc, n3, 0.5f * dt);
+  return (int)cudaGetLastError();
+}
+
 // ---- tc_fp32_peak: what the FP32 pipe of this device sustains with nothing but FFMA in flight
 namespace {
 __global__ void __launch_bounds__(256) ffma_peak_kernel(float* out, int n, float s) {

@@ -2,9 +2,11 @@
 
 The paper keeps time integration on the host and only mentions it; BASELINE.json
 config 5 prescribes 10 kick-drift-kick steps with a host tree rebuild each step.  This module is
-harness code, not part of the hot path: positions / velocities live in torch device tensors, the
-kicks and drifts are plain elementwise torch ops, and every force evaluation is one
-``tc_set_particles`` + ``tc_build`` + ``tc_forces`` through the C ABI (device pointers).
+harness code, not part of the hot path: positions / velocities live in torch device tensors and every
+force evaluation is one ``tc_set_particles`` + ``tc_build`` + ``tc_forces`` through the C ABI (device
+pointers).  The kicks and the drift are either plain elementwise torch ops (default) or, with
+``native=True``, the library's own ``tc_leapfrog`` (device-side KDK), called one step at a
+time so that the energy can be logged between steps.
 """
 from __future__ import annotations
 
@@ -24,7 +26,7 @@ def energy(mass, vel, pot):
 
 
 def leapfrog_kdk(tc: "B.TreeCode", pos, vel, mass, dt: float, steps: int, theta: float, eps: float,
-                 n_leaf: int = 16, log=None):
+                 n_leaf: int = 16, log=None, native: bool = False):
     """Advance (pos, vel) in place by `steps` KDK steps; returns a list of per-step dicts.
 
     v += a dt/2 ; x += v dt ; rebuild tree ; a = forces(x) ; v += a dt/2     (BASELINE.json config 5)
@@ -50,10 +52,15 @@ def leapfrog_kdk(tc: "B.TreeCode", pos, vel, mass, dt: float, steps: int, theta:
     for k in range(1, steps + 1):
         torch.cuda.synchronize(dev)
         t0 = time.perf_counter()
-        vel.add_(acc, alpha=0.5 * dt)
-        pos.add_(vel, alpha=dt)
-        st = force()
-        vel.add_(acc, alpha=0.5 * dt)
+        if native:
+            B.tc_leapfrog(tc.ctx, pos, vel, mass, dt, 1, n_leaf, theta, eps, acc, pot, have_acc=True)
+            tc.sync()
+            st = tc.stats()
+        else:
+            vel.add_(acc, alpha=0.5 * dt)
+            pos.add_(vel, alpha=dt)
+            st = force()
+            vel.add_(acc, alpha=0.5 * dt)
         torch.cuda.synchronize(dev)
         wall = (time.perf_counter() - t0) * 1e3
         e = energy(mass, vel, pot)[2]

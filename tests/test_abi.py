@@ -41,6 +41,9 @@ def test_no_cpu_fallback_host_only_refuses_forces():
         with pytest.raises(B.TcError) as e:
             tc.forces(0.5, 0.01)
         assert e.value.code == B.TC_ESTATE
+        with pytest.raises(B.TcError) as e:                       # no CPU leapfrog either
+            B.tc_leapfrog(tc.ctx, pos, pos.copy(), mass, 0.01, 1, 8, 0.5, 0.01, np.zeros_like(pos))
+        assert e.value.code == B.TC_ESTATE
 
 
 def test_error_codes():
