@@ -122,6 +122,12 @@ int tc_forces(tc_ctx* ctx, float theta, float eps, float* acc, float* pot);
  *                 still conservative, about 1 % fewer interactions.  Combines with "open_rule".
  *   "quadrupole"  1 (default: monopole + quadrupole) or 0: monopole-only cells (variant R22, the expansion of
  *                 the Hamada et al. code the paper compares with).
+ *   "shard_count", "shard_rank"   multi-GPU sharding of ONE force evaluation (groups are independent
+ *                 given the read-only tree): with shard_count = k > 1 tc_forces evaluates only the
+ *                 groups at positions rank, rank + k, ... of the cost-ordered schedule.  acc, pot and the counts
+ *                 of every particle OUTSIDE the shard are then ZERO on return, so the k shards (one context per
+ *                 GPU, each holding the same particles and tree) combine by summation (one all-reduce); the
+ *                 totals in tc_stats are per shard.  Default 1 / 0.  Fused kernel only (TC_EINVAL with two_pass).
  *   "two_pass"    0 (default: the fused kernel) or 1: the paper-literal pipeline —
  *                 walk-count kernel, scan of the list sizes, walk-write kernel (lists in global memory),
  *                 body-node kernel, body-leaf kernel; same lists, same counts, same results up to

@@ -27,6 +27,7 @@ struct tc_ctx {
   bool device_build = false;          // option "device_build": tc_build_gpu.cu instead of tc_build.cpp
   int stack_smem = 256;
   int walk_only = 0, open_rule = 0, quadrupole = 1, group_box = 0;
+  int shard_rank = 0, shard_count = 1;
   bool two_pass = false;
   tc::TwoPassScratch tps;
   bool last_two_pass = false;
@@ -229,6 +230,14 @@ int tc_set_option(tc_ctx* c, const char* key, double v) {
     if (v != 0.0 && v != 1.0) return fail(c, TC_EINVAL, "tc_set_option: open_rule must be 0 or 1");
     c->open_rule = (int)v; return TC_OK;
   }
+  if (!std::strcmp(key, "shard_count")) {
+    if (!(v >= 1.0) || v > 65536.0 || v != std::floor(v)) return fail(c, TC_EINVAL, "tc_set_option: shard_count must be an integer in [1, 65536]");
+    c->shard_count = (int)v; return TC_OK;
+  }
+  if (!std::strcmp(key, "shard_rank")) {
+    if (!(v >= 0.0) || v > 65535.0 || v != std::floor(v)) return fail(c, TC_EINVAL, "tc_set_option: shard_rank must be an integer in [0, 65535]");
+    c->shard_rank = (int)v; return TC_OK;
+  }
   if (!std::strcmp(key, "group_box")) {
     if (v != 0.0 && v != 1.0) return fail(c, TC_EINVAL, "tc_set_option: group_box must be 0 or 1");
     c->group_box = (int)v; return TC_OK;
@@ -396,6 +405,8 @@ int tc_forces(tc_ctx* c, float theta, float eps, float* acc, float* pot) {
   if (!acc) return fail(c, TC_EINVAL, "tc_forces: acc is null");
   if (!(theta >= 0.f) || !std::isfinite(theta) || !(eps >= 0.f) || !std::isfinite(eps))
     return fail(c, TC_EINVAL, "tc_forces: theta and eps must be finite and >= 0");
+  if (c->shard_count > 1 && c->shard_rank >= c->shard_count) return fail(c, TC_EINVAL, "tc_forces: shard_rank must be < shard_count");
+  if (c->shard_count > 1 && c->two_pass) return fail(c, TC_EINVAL, "tc_forces: sharding runs the fused kernel only (two_pass must be 0)");
   const int64_t n = c->n;
   const bool acc_dev = is_device_ptr(c, acc), pot_dev = pot ? is_device_ptr(c, pot) : acc_dev;
   if (pot && acc_dev != pot_dev) return fail(c, TC_EINVAL, "tc_forces: acc and pot must both be host or both be device pointers");
@@ -424,6 +435,13 @@ int tc_forces(tc_ctx* c, float theta, float eps, float* acc, float* pot) {
   L.n_pc = c->d_npc; L.n_pp = c->d_npp; L.counters = c->d_ctr; L.spill = c->d_spill; L.spill_cap = c->spill_cap;
   L.stack_smem = c->stack_smem; L.n_sm = c->n_sm; L.flags = (c->walk_only ? 1 : 0) | (c->open_rule ? 2 : 0) | (c->quadrupole ? 0 : 4) | (c->group_box ? 8 : 0);
   L.max_grid = (int)(warps / (size_t)tc::forces_warps_per_cta());
+  L.shard_rank = c->shard_count > 1 ? c->shard_rank : 0; L.shard_count = c->shard_count;
+  if (c->shard_count > 1) {   // entries outside the shard are ZERO, so the shards of all ranks combine by summation
+    TC_CUDA(c, cudaMemsetAsync(L.acc, 0, sizeof(float) * 3 * (size_t)n, c->stream));
+    if (L.pot) TC_CUDA(c, cudaMemsetAsync(L.pot, 0, sizeof(float) * (size_t)n, c->stream));
+    TC_CUDA(c, cudaMemsetAsync(L.n_pc, 0, sizeof(int32_t) * (size_t)n, c->stream));
+    TC_CUDA(c, cudaMemsetAsync(L.n_pp, 0, sizeof(int32_t) * (size_t)n, c->stream));
+  }
   // stream-ordered: no host synchronisation between queued calls; the overflow flag is sticky until collect()
   TC_CUDA(c, cudaMemsetAsync(c->d_ctr, 0, offsetof(tc::DeviceCounters, overflow), c->stream));
   TC_CUDA(c, cudaEventRecord(c->ev0, c->stream));

@@ -90,6 +90,7 @@ struct ForceLaunch {
   int flags = 0;              // bit 0: walk_only (measurement aid), bit 1: COM opening rule (R21), bit 2: monopole only (R22), bit 3: group = its tight box (R23)
   int n_sm = 148;
   int max_grid = 0;           // CTAs the spill buffer has room for (0: no limit)
+  int shard_rank = 0, shard_count = 1;   // this launch runs schedule positions rank, rank + count, ... (fused kernel)
 };
 
 // Launches the fused walk+evaluate kernel on `stream` (a cudaStream_t).  Returns a

@@ -372,7 +372,7 @@ forces_kernel(const float4* __restrict__ bnd, const float4* __restrict__ xm, con
               const int4* __restrict__ grp, const float4* __restrict__ gbox, int n_groups, float theta, float eps,
               float* __restrict__ acc, float* __restrict__ pot, int32_t* __restrict__ out_npc,
               int32_t* __restrict__ out_npp, DeviceCounters* __restrict__ ctr, uint32_t* __restrict__ spill_all,
-              int spill_cap, int flags, ListIO lio) {
+              int spill_cap, int flags, ListIO lio, int shard_rank, int shard_count) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   WarpSmem<STK>& sm = reinterpret_cast<WarpSmem<STK>*>(smem_raw)[warp];
@@ -394,7 +394,10 @@ forces_kernel(const float4* __restrict__ bnd, const float4* __restrict__ xm, con
     int g = 0;
     if (lane == 0) g = (int)atomicAdd(&ctr->next_group, 1u);
     g = __shfl_sync(kFull, g, 0);
-    if (g >= n_groups) break;
+    // multi-GPU sharding: this launch takes the schedule positions rank, rank + count, ...
+    // (neighbours in the cost-ordered schedule cost about the same, so the shards are balanced)
+    if (g >= (n_groups - shard_rank + shard_count - 1) / shard_count) break;
+    g = g * shard_count + shard_rank;
     g = __ldg(&grp[g].w);                    // schedule: costly groups first (tc_build)
     const int4 G = __ldg(grp + g);           // (cell, first_body, n_body, -)
     const float4 gb = __ldg(bnd + G.x);
@@ -640,7 +643,7 @@ int launch_t(const DeviceTree& T, const ForceLaunch& L, cudaStream_t st, int* ct
   const int grid = L.max_grid > 0 ? std::min(L.n_sm * per_sm, L.max_grid) : L.n_sm * per_sm;
   kern<<<grid, kWarpsPerCta * 32, smem, st>>>(T.bnd, T.xm, T.q0, T.q1, T.part, T.orig, T.grp, T.gbox, (int)T.n_groups,
                                                L.theta, L.eps, L.acc, L.pot, L.n_pc, L.n_pp, L.counters, L.spill,
-                                               L.spill_cap, L.flags, lio);
+                                               L.spill_cap, L.flags, lio, L.shard_rank, L.shard_count);
   return (int)cudaGetLastError();
 }
 

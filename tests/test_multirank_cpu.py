@@ -55,6 +55,37 @@ def test_two_ranks_gloo(tmp_path):
     assert r[0]["first"][0] != r[0]["first"][1]           # different spheres per rank
 
 
+def _shard_worker(rank, world, port, out_dir):
+    """Rank r holds the results of its shard (here: the ORACLE restricted to the groups r, r + world, ... —
+    no GPU in this test), zeros elsewhere; parallel.combine must hand every rank the full result."""
+    sys.path.insert(0, ROOT)
+    import oracle
+    from paper_1005_5384_b200 import inputs, parallel
+    dist.init_process_group("gloo", init_method=f"tcp://127.0.0.1:{port}", rank=rank, world_size=world)
+    pos, mass, theta, eps, n_leaf = inputs.make("plummer_1k")
+    o = oracle.Oracle(pos, mass, n_leaf, 32)
+    mine = np.array(list(parallel.shard_of(rank, world, o.n_groups)), dtype=np.int64)
+    r = o.forces(theta, eps, groups=mine)
+    acc = torch.from_numpy(np.nan_to_num(r["acc"], nan=0.0))
+    pot = torch.from_numpy(np.nan_to_num(r["pot"], nan=0.0))
+    npc = torch.from_numpy(np.maximum(r["n_pc"], 0))
+    parallel.combine(acc, pot, counts=(npc,))
+    full = o.forces(theta, eps)
+    ok = bool(np.array_equal(acc.numpy(), full["acc"]) and np.array_equal(pot.numpy(), full["pot"])
+              and np.array_equal(npc.numpy(), full["n_pc"]))
+    with open(os.path.join(out_dir, f"s{rank}.json"), "w") as f:
+        json.dump({"ok": ok, "mine": len(mine), "groups": o.n_groups}, f)
+    dist.destroy_process_group()
+
+
+def test_sharded_force_evaluation_combines_to_the_whole(tmp_path):
+    world, port = 2, _free_port()
+    mp.spawn(_shard_worker, args=(world, port, str(tmp_path)), nprocs=world, join=True)
+    r = [json.load(open(tmp_path / f"s{k}.json")) for k in range(world)]
+    assert all(x["ok"] for x in r)
+    assert r[0]["mine"] + r[1]["mine"] == r[0]["groups"] and abs(r[0]["mine"] - r[1]["mine"]) <= 1
+
+
 def test_reference_arm_runs_on_rank0_only():
     """Under torchrun the oracle arm prints on rank 0; other ranks exit 0 without work."""
     env = dict(os.environ, RANK="1", WORLD_SIZE="2", LOCAL_RANK="1")
