@@ -181,10 +181,11 @@ template <int KP>
 __device__ __forceinline__ void eval_cells_k(const CellRec* __restrict__ rec, int cnt, float eps2, const Lanes& L,
                                              const Pos2 (&P)[kMaxKP], Acc2 (&A)[kMaxKP]) {
   if (!L.active) return;
+  // pointer walk (one add per record, no index multiply): slice s takes records s, s + S, ...
+  const CellRec* r0 = rec + L.s;
+  const CellRec* const end = rec + cnt;
   const int st = L.S;
-  int e = L.s;
-  for (; e + st < cnt; e += 2 * st) {            // two records in flight
-    const CellRec* r0 = rec + e;
+  for (; r0 + st < end; r0 += 2 * st) {          // two records in flight
     const CellRec* r1 = r0 + st;
     const float4 a0 = r0->xm, b0 = r0->q0; const float2 c0 = r0->q1;
     const float4 a1 = r1->xm, b1 = r1->q0; const float2 c1 = r1->q1;
@@ -193,8 +194,7 @@ __device__ __forceinline__ void eval_cells_k(const CellRec* __restrict__ rec, in
 #pragma unroll
     for (int j = 0; j < KP; j++) pc_interact(P[j], eps2, a1, b1, c1, A[j]);
   }
-  if (e < cnt) {
-    const CellRec* r0 = rec + e;
+  if (r0 < end) {
     const float4 a0 = r0->xm, b0 = r0->q0; const float2 c0 = r0->q1;
 #pragma unroll
     for (int j = 0; j < KP; j++) pc_interact(P[j], eps2, a0, b0, c0, A[j]);
@@ -240,18 +240,19 @@ template <int KP, bool kEps0>
 __device__ __forceinline__ void eval_bodies_k(const float4* __restrict__ body, int cnt, float eps2, const Lanes& L,
                                               const Pos2 (&P)[kMaxKP], Acc2 (&A)[kMaxKP]) {
   if (!L.active) return;
+  const float4* b = body + L.s;                  // pointer walk, as in eval_cells_k
+  const float4* const end = body + cnt;
   const int st = L.S;
-  int e = L.s;
-  for (; e + 3 * st < cnt; e += 4 * st) {        // four bodies in flight
-    const float4 b0 = body[e], b1 = body[e + st], b2 = body[e + 2 * st], b3 = body[e + 3 * st];
+  for (; b + 3 * st < end; b += 4 * st) {        // four bodies in flight
+    const float4 b0 = b[0], b1 = b[st], b2 = b[2 * st], b3 = b[3 * st];
 #pragma unroll
     for (int j = 0; j < KP; j++) {
       pp_interact<kEps0>(P[j], eps2, b0, A[j]); pp_interact<kEps0>(P[j], eps2, b1, A[j]);
       pp_interact<kEps0>(P[j], eps2, b2, A[j]); pp_interact<kEps0>(P[j], eps2, b3, A[j]);
     }
   }
-  for (; e < cnt; e += st) {
-    const float4 b0 = body[e];
+  for (; b < end; b += st) {
+    const float4 b0 = b[0];
 #pragma unroll
     for (int j = 0; j < KP; j++) pp_interact<kEps0>(P[j], eps2, b0, A[j]);
   }
