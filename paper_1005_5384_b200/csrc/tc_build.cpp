@@ -114,6 +114,17 @@ inline size_t align256(size_t x) { return (x + 255) & ~(size_t)255; }
 
 }  // namespace
 
+void* HostScratch::get(int k, size_t bytes) {
+  if (cap[k] < bytes) {
+    std::free(buf[k]); buf[k] = nullptr; cap[k] = 0;
+    const size_t want = bytes + bytes / 8 + 64;
+    buf[k] = std::malloc(want);
+    if (buf[k]) cap[k] = want;
+  }
+  return buf[k];
+}
+HostScratch::~HostScratch() { for (void* p : buf) std::free(p); }
+
 int build_host_tree(const float* pos, const float* mass, int64_t n, int n_leaf, int n_group,
                     HostTree& T, PackedAlloc alloc, void* alloc_user, std::string& msg) {
   if (n < 1 || n_leaf < 1 || n_group < 1) { msg = "build: n, n_leaf, n_group must be >= 1"; return TC_EINVAL; }
@@ -146,9 +157,10 @@ int build_host_tree(const float* pos, const float* mass, int64_t n, int n_leaf, 
   const double gmax = std::ldexp(1.0, 21) - 1.0;
 
   // key buffers: plain arrays (no zero fill; every element is written below)
-  std::unique_ptr<KeyIdx[]> keys_buf(new (std::nothrow) KeyIdx[(size_t)n]), tmp_buf(new (std::nothrow) KeyIdx[(size_t)n]);
-  if (!keys_buf || !tmp_buf) { msg = "build: out of host memory"; return TC_ENOMEM; }
-  KeyIdx* keys = keys_buf.get();
+  // (from the context's grow-only scratch: a rebuild touches no fresh pages)
+  KeyIdx* keys = static_cast<KeyIdx*>(T.scratch.get(0, sizeof(KeyIdx) * (size_t)n));
+  KeyIdx* tmp_keys = static_cast<KeyIdx*>(T.scratch.get(1, sizeof(KeyIdx) * (size_t)n));
+  if (!keys || !tmp_keys) { msg = "build: out of host memory"; return TC_ENOMEM; }
   uint64_t key_or = 0;
 #pragma omp parallel for schedule(static) reduction(| : key_or)
   for (int64_t i = 0; i < n; i++) {
@@ -164,9 +176,8 @@ int build_host_tree(const float* pos, const float* mass, int64_t n, int n_leaf, 
     key_or |= key;
   }
   lap("keys");
-  radix_sort(keys, tmp_buf.get(), n, key_or, n_leaf);
+  radix_sort(keys, tmp_keys, n, key_or, n_leaf);
   lap("sort");
-  tmp_buf.reset();
 
   // ---- O2: breadth-first split of sorted key ranges
   // cell arrays (struct of vectors), breadth-first, children contiguous
@@ -237,8 +248,8 @@ int build_host_tree(const float* pos, const float* mass, int64_t n, int n_leaf, 
   // ---- O3: cell properties, fp64, bottom-up.  Leaves: direct sums
   // over members.  Nodes: union of the children's boxes, parallel-axis shift of the
   // children's moments to the node's centre of mass.
-  std::vector<CellProp> prop;
-  try { prop.resize((size_t)nc); } catch (...) { msg = "build: out of host memory"; return TC_ENOMEM; }
+  CellProp* prop = static_cast<CellProp*>(T.scratch.get(2, sizeof(CellProp) * (size_t)nc));   // every entry is written below
+  if (!prop) { msg = "build: out of host memory"; return TC_ENOMEM; }
   int64_t n_leaves = 0;
   for (int L = n_levels - 1; L >= 0; L--) {
     const int64_t b = level_start[L], e = level_start[L + 1];

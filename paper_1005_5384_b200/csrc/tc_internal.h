@@ -33,6 +33,18 @@ struct PackedLayout {
   size_t bytes = 0;
 };
 
+// Grow-only scratch of the host builder, kept between builds so that a rebuild (every step of a
+// simulation) does not fault ~60 MB of fresh pages in again.  Contents are undefined between builds.
+struct HostScratch {
+  void* buf[3] = {nullptr, nullptr, nullptr};
+  size_t cap[3] = {0, 0, 0};
+  void* get(int k, size_t bytes);  // >= bytes of uninitialised storage, nullptr on failure
+  HostScratch() = default;
+  HostScratch(const HostScratch&) = delete;
+  HostScratch& operator=(const HostScratch&) = delete;
+  ~HostScratch();
+};
+
 struct HostTree {
   int64_t n = 0;
   int32_t n_leaf = 0, n_group = 0;
@@ -45,6 +57,7 @@ struct HostTree {
   void* packed = nullptr;  // lay.bytes, owned by the ctx (pinned or malloc)
   size_t packed_cap = 0;
   bool packed_pinned = false;
+  HostScratch scratch;     // sort keys (2x) and per-cell moments of build_host_tree
 };
 
 // Host builder (tc_build.cpp).  pos [n,3], mass [n] host fp32.  Allocates/reuses
