@@ -181,13 +181,15 @@ int build_host_tree(const float* pos, const float* mass, int64_t n, int n_leaf, 
 
   // ---- O2: breadth-first split of sorted key ranges
   // cell arrays (struct of vectors), breadth-first, children contiguous
-  std::vector<int32_t> c_begin, c_count, c_first_child, c_nchild;
+  std::vector<int32_t>&c_begin = T.scratch.c_begin, &c_count = T.scratch.c_count, &c_first_child = T.scratch.c_first_child,
+                      &c_nchild = T.scratch.c_nchild;   // capacity survives between builds
+  c_begin.clear(); c_count.clear(); c_first_child.clear(); c_nchild.clear();
   std::vector<int64_t> level_start;  // first cell id of every level (+ end sentinel)
   c_begin.push_back(0); c_count.push_back((int32_t)n); c_first_child.push_back(-1); c_nchild.push_back(0);
   level_start.push_back(0);
   int64_t lvl_b = 0, lvl_e = 1;
   int level = 0;
-  std::vector<int32_t> nch;
+  std::vector<int32_t>& nch = T.scratch.nch;
   while (true) {
     level_start.push_back(lvl_e);
     if (level == kMaxLevel) break;
@@ -318,7 +320,8 @@ int build_host_tree(const float* pos, const float* mass, int64_t n, int n_leaf, 
 
   lap("moments");
   // ---- O4: groups = maximal cells with count <= N_group, or leaves, Morton order
-  std::vector<int32_t> groups;
+  std::vector<int32_t>& groups = T.scratch.groups;
+  groups.clear();
   {
     std::vector<int32_t> st;
     st.push_back(0);
