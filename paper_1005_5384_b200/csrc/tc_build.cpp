@@ -49,11 +49,12 @@ struct KeyIdx {
 // its low 24 bits ordered when it is longer than `n_leaf` (it is then split below level 13), which is
 // rare — those runs are finished with std::stable_sort.  Shorter runs end up inside one leaf, where the
 // order of the members is immaterial (it stays the caller's order).
-void radix_sort(KeyIdx* a, KeyIdx* tmp, int64_t n, uint64_t key_or, int n_leaf) {
+// Returns the buffer that holds the sorted array (`a` or `tmp`: no copy back after an odd number of passes).
+KeyIdx* radix_sort(KeyIdx* a, KeyIdx* tmp, int64_t n, uint64_t key_or, int n_leaf) {
   constexpr int BITS = 13, R = 1 << BITS, LOW = 63 - 3 * BITS;
   if (n < 8192) {   // small inputs: the histograms would cost more than the sort
     std::stable_sort(a, a + n, [](const KeyIdx& x, const KeyIdx& y) { return x.key < y.key; });
-    return;
+    return a;
   }
   int nthreads = 1;
 #ifdef _OPENMP
@@ -91,7 +92,7 @@ void radix_sort(KeyIdx* a, KeyIdx* tmp, int64_t n, uint64_t key_or, int n_leaf) 
     }
     std::swap(src, dst);
   }
-  if (src != a) std::memcpy(a, src, sizeof(KeyIdx) * (size_t)n);
+  a = src;
   // finish the long runs (parallel over run starts; runs are disjoint)
 #pragma omp parallel for schedule(dynamic, 65536)
   for (int64_t i = 0; i < n; i++) {
@@ -103,6 +104,7 @@ void radix_sort(KeyIdx* a, KeyIdx* tmp, int64_t n, uint64_t key_or, int n_leaf) 
     while (j < n && (a[j].key >> LOW) == pre) j++;
     std::stable_sort(a + i, a + j, [](const KeyIdx& x, const KeyIdx& y) { return x.key < y.key; });
   }
+  return a;
 }
 
 struct CellProp {   // fp64 moments, fp32-exact bounding box
@@ -147,6 +149,7 @@ int build_host_tree(const float* pos, const float* mass, int64_t n, int n_leaf, 
     }
     lo[0] = l0; lo[1] = l1; lo[2] = l2; hi[0] = h0; hi[1] = h1; hi[2] = h2;
   }
+  lap("bbox");
   double ext = 0.0;
   for (int k = 0; k < 3; k++) ext = std::max(ext, hi[k] - lo[k]);
   double side = ext * (1.0 + std::ldexp(1.0, -20));
@@ -176,8 +179,21 @@ int build_host_tree(const float* pos, const float* mass, int64_t n, int n_leaf, 
     key_or |= key;
   }
   lap("keys");
-  radix_sort(keys, tmp_keys, n, key_or, n_leaf);
+  {
+    KeyIdx* const sorted = radix_sort(keys, tmp_keys, n, key_or, n_leaf);
+    if (sorted != keys) std::swap(keys, tmp_keys);
+  }
   lap("sort");
+  // particles in tree (Morton) order, staged in the sort's other buffer (same 16 bytes per element): the
+  // moments and the pack below read them sequentially instead of gathering through keys[t].idx
+  static_assert(sizeof(KeyIdx) == sizeof(float4), "the sort scratch doubles as the sorted particle array");
+  float4* sp = reinterpret_cast<float4*>(tmp_keys);
+#pragma omp parallel for schedule(static)
+  for (int64_t t = 0; t < n; t++) {
+    const int64_t i = keys[t].idx;
+    sp[t] = make_float4(pos[3 * i], pos[3 * i + 1], pos[3 * i + 2], mass[i]);
+  }
+  lap("gather");
 
   // ---- O2: breadth-first split of sorted key ranges
   // cell arrays (struct of vectors), breadth-first, children contiguous
@@ -264,10 +280,11 @@ int build_host_tree(const float* pos, const float* mass, int64_t n, int n_leaf, 
         float mn[3] = {INFINITY, INFINITY, INFINITY}, mx[3] = {-INFINITY, -INFINITY, -INFINITY};
         const int64_t pb = c_begin[c], pe = pb + c_count[c];
         for (int64_t t = pb; t < pe; t++) {
-          const int64_t i = keys[t].idx;
-          const double m = (double)mass[i];
+          const float4 b = sp[t];
+          const float xyz[3] = {b.x, b.y, b.z};
+          const double m = (double)b.w;
           for (int k = 0; k < 3; k++) {
-            const float v = pos[3 * i + k];
+            const float v = xyz[k];
             mn[k] = std::min(mn[k], v); mx[k] = std::max(mx[k], v);
             S[k] += m * (double)v;
           }
@@ -279,10 +296,9 @@ int build_host_tree(const float* pos, const float* mass, int64_t n, int n_leaf, 
           P.X[k] = (M > 0.0) ? S[k] / M : ((double)mn[k] + (double)mx[k]) / 2.0;
         double Q[6] = {0, 0, 0, 0, 0, 0};
         for (int64_t t = pb; t < pe; t++) {
-          const int64_t i = keys[t].idx;
-          const double m = (double)mass[i];
-          const double yx = (double)pos[3 * i] - P.X[0], yy = (double)pos[3 * i + 1] - P.X[1],
-                       yz = (double)pos[3 * i + 2] - P.X[2];
+          const float4 b = sp[t];
+          const double m = (double)b.w;
+          const double yx = (double)b.x - P.X[0], yy = (double)b.y - P.X[1], yz = (double)b.z - P.X[2];
           const double y2 = yx * yx + yy * yy + yz * yz;
           Q[0] += m * (3.0 * yx * yx - y2); Q[1] += m * (3.0 * yy * yy - y2); Q[2] += m * (3.0 * yz * yz - y2);
           Q[3] += m * (3.0 * yx * yy); Q[4] += m * (3.0 * yx * yz); Q[5] += m * (3.0 * yy * yz);
@@ -392,9 +408,8 @@ int build_host_tree(const float* pos, const float* mass, int64_t n, int n_leaf, 
   }
 #pragma omp parallel for schedule(static)
   for (int64_t t = 0; t < n; t++) {
-    const int64_t i = keys[t].idx;
-    part[t] = make_float4(pos[3 * i], pos[3 * i + 1], pos[3 * i + 2], mass[i]);
-    orig[t] = (int32_t)i;
+    part[t] = sp[t];
+    orig[t] = (int32_t)keys[t].idx;
   }
   lap("pack");
   // Schedule (grp[i].w = i-th group to run): the persistent kernel hands groups out through an
@@ -418,6 +433,7 @@ int build_host_tree(const float* pos, const float* mass, int64_t n, int n_leaf, 
     const size_t ng = groups.size();
     std::vector<int32_t> cls(ng);
     int32_t cmax = 0;
+#pragma omp parallel for schedule(static) reduction(max : cmax)
     for (size_t g = 0; g < ng; g++) {
       const int64_t cnt = c_count[groups[g]];
       const double cost = (double)(cnt / kPass) * pass_cost[kPass] + pass_cost[cnt % kPass];
@@ -429,7 +445,8 @@ int build_host_tree(const float* pos, const float* mass, int64_t n, int n_leaf, 
     for (size_t k = 1; k < start.size(); k++) start[k] += start[k - 1];
     std::vector<int32_t> order(ng);
     for (size_t g = 0; g < ng; g++) order[(size_t)start[(size_t)(cmax - cls[g])]++] = (int32_t)g;
-    for (size_t g = 0; g < groups.size(); g++) {
+#pragma omp parallel for schedule(static)
+    for (size_t g = 0; g < ng; g++) {
       const int32_t c = groups[g];
       grp[g] = make_int4(c, c_begin[c], c_count[c], order[g]);
       // variant R23: half extents of the tight box about the fp32 centre of the boundary cube, per axis,
