@@ -98,3 +98,15 @@ def test_degenerate_inputs():
     line = np.zeros((64, 3), np.float32)
     line[:, 0] = np.linspace(-1, 1, 64)                                 # collinear: two axes have zero extent
     _compare(line, np.ones(64, np.float32), 4, 8)
+
+
+def test_deep_clusters_through_the_radix_sort_fixup():
+    """n large enough for the parallel radix sort (3 passes of 11 bits = 11 levels): a tight cluster and a
+    coincident clump make cells far below level 11, i.e. long runs of equal prefixes that the fix-up must order."""
+    rng = np.random.default_rng(9)
+    n = 70000
+    pos = rng.uniform(-1, 1, (n, 3)).astype(np.float32)
+    pos[:9000] = (np.array([0.3, -0.2, 0.1]) + 1e-5 * rng.standard_normal((9000, 3))).astype(np.float32)   # levels 15-18
+    pos[9000:9300] = pos[9000]                                                                            # level-21 leaf
+    mass = np.full(n, 1.0 / n, np.float32)
+    _compare(pos, mass, 8, 32)
