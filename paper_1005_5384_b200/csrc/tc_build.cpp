@@ -218,20 +218,25 @@ int build_host_tree(const float* pos, const float* mass, int64_t n, int n_leaf, 
     const int shift = 3 * (kMaxLevel - 1 - level);
     const int64_t nl = lvl_e - lvl_b;
     nch.assign((size_t)nl + 1, 0);
-    // pass 1: number of non-empty octants of every node of this level
+    // pass 1: the non-empty octants of every node of this level; their starts are kept for pass 2
+    std::vector<int32_t>& bounds = T.scratch.bounds;
+    if (bounds.size() < (size_t)nl * 9) bounds.resize((size_t)nl * 9);
+    int32_t* const bnds = bounds.data();
 #pragma omp parallel for schedule(dynamic, 256)
     for (int64_t c = lvl_b; c < lvl_e; c++) {
       if (c_count[c] <= n_leaf) continue;  // leaf (R4: <=)
       const KeyIdx* kb = keys + c_begin[c];
       const KeyIdx* ke = kb + c_count[c];
+      int32_t* bd = bnds + 9 * (size_t)(c - lvl_b);
       int cnt = 0;
       const KeyIdx* p = kb;
       while (p < ke) {
         const uint64_t o = (p->key >> shift) & 7;
+        bd[cnt++] = (int32_t)(p - keys);
         // first key of this cell with octant > o
         p = std::partition_point(p, ke, [&](const KeyIdx& q) { return ((q.key >> shift) & 7) <= o; });
-        cnt++;
       }
+      bd[cnt] = (int32_t)(ke - keys);
       nch[(size_t)(c - lvl_b)] = cnt;
     }
     int64_t total = 0;
@@ -249,17 +254,8 @@ int build_host_tree(const float* pos, const float* mass, int64_t n, int n_leaf, 
       if (k == 0) continue;
       const int64_t first = lvl_e + nch[(size_t)(c - lvl_b)];
       c_first_child[c] = (int32_t)first; c_nchild[c] = k;
-      const KeyIdx* k0 = keys;
-      const KeyIdx* kb = k0 + c_begin[c];
-      const KeyIdx* ke = kb + c_count[c];
-      const KeyIdx* p = kb;
-      int j = 0;
-      while (p < ke) {
-        const uint64_t o = (p->key >> shift) & 7;
-        const KeyIdx* q = std::partition_point(p, ke, [&](const KeyIdx& r) { return ((r.key >> shift) & 7) <= o; });
-        c_begin[first + j] = (int32_t)(p - k0); c_count[first + j] = (int32_t)(q - p);
-        j++; p = q;
-      }
+      const int32_t* bd = bnds + 9 * (size_t)(c - lvl_b);
+      for (int j = 0; j < k; j++) { c_begin[first + j] = bd[j]; c_count[first + j] = bd[j + 1] - bd[j]; }
     }
     lvl_b = lvl_e; lvl_e = new_e; level++;
   }

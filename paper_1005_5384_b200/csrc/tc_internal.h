@@ -40,7 +40,7 @@ struct HostScratch {
   size_t cap[3] = {0, 0, 0};
   void* get(int k, size_t bytes);  // >= bytes of uninitialised storage, nullptr on failure
   // per-cell arrays of the breadth-first split and the group list: cleared, not freed, between builds
-  std::vector<int32_t> c_begin, c_count, c_first_child, c_nchild, nch, groups;
+  std::vector<int32_t> c_begin, c_count, c_first_child, c_nchild, nch, groups, bounds;
   HostScratch() = default;
   HostScratch(const HostScratch&) = delete;
   HostScratch& operator=(const HostScratch&) = delete;
