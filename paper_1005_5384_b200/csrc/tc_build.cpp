@@ -44,6 +44,45 @@ struct KeyIdx {
   uint32_t idx;
 };
 
+// O1: integer grid coordinates and 63-bit Morton keys of all particles; returns the OR of all keys.
+// One body, two instantiations: baseline x86-64, and AVX2 + BMI2 (vectorised floor / min / max, bit
+// interleave by PDEP), chosen at run time — the arithmetic is the same correctly rounded fp64 sequence.
+#define TC_KEYS_BODY(SPREAD)                                                                        \
+  uint64_t key_or = 0;                                                                              \
+  _Pragma("omp parallel for schedule(static) reduction(| : key_or)")                                \
+  for (int64_t i = 0; i < n; i++) {                                                                 \
+    uint64_t g[3];                                                                                  \
+    for (int k = 0; k < 3; k++) {                                                                   \
+      double v = std::floor(((double)pos[3 * i + k] - org[k]) * scale);                             \
+      v = std::min(std::max(v, 0.0), gmax);                                                         \
+      g[k] = (uint64_t)v;                                                                           \
+    }                                                                                               \
+    /* octant o = 4 bx + 2 by + bz at every level  ->  x is the most significant of each triple */  \
+    const uint64_t key = (SPREAD(g[0]) << 2) | (SPREAD(g[1]) << 1) | SPREAD(g[2]);                  \
+    keys[i].key = key; keys[i].idx = (uint32_t)i;                                                   \
+    key_or |= key;                                                                                  \
+  }                                                                                                 \
+  return key_or;
+
+uint64_t compute_keys_base(const float* pos, int64_t n, const double* org, double scale, double gmax, KeyIdx* keys) {
+  TC_KEYS_BODY(spread21)
+}
+#if defined(__x86_64__) && defined(__GNUC__)
+#define TC_PDEP21(x) __builtin_ia32_pdep_di((x), 0x1249249249249249ull)
+#pragma GCC push_options
+#pragma GCC target("avx2,bmi2")
+uint64_t compute_keys_v3(const float* pos, int64_t n, const double* org, double scale, double gmax, KeyIdx* keys) {
+  TC_KEYS_BODY(TC_PDEP21)
+}
+#pragma GCC pop_options
+#endif
+uint64_t compute_keys(const float* pos, int64_t n, const double* org, double scale, double gmax, KeyIdx* keys) {
+#if defined(__x86_64__) && defined(__GNUC__)
+  if (__builtin_cpu_supports("avx2") && __builtin_cpu_supports("bmi2")) return compute_keys_v3(pos, n, org, scale, gmax, keys);
+#endif
+  return compute_keys_base(pos, n, org, scale, gmax, keys);
+}
+
 // Sort of (key, idx) by key, stable (equal keys keep ascending idx).  Three LSD radix passes of BITS
 // bits order the keys by their top 3 BITS bits (BITS tree levels); a run of equal prefixes only needs
 // its low bits ordered when it is longer than `n_leaf` (it is then split below level BITS), which is
@@ -170,20 +209,7 @@ int build_host_tree(const float* pos, const float* mass, int64_t n, int n_leaf, 
   KeyIdx* keys = static_cast<KeyIdx*>(T.scratch.get(0, sizeof(KeyIdx) * (size_t)n));
   KeyIdx* tmp_keys = static_cast<KeyIdx*>(T.scratch.get(1, sizeof(KeyIdx) * (size_t)n));
   if (!keys || !tmp_keys) { msg = "build: out of host memory"; return TC_ENOMEM; }
-  uint64_t key_or = 0;
-#pragma omp parallel for schedule(static) reduction(| : key_or)
-  for (int64_t i = 0; i < n; i++) {
-    uint64_t g[3];
-    for (int k = 0; k < 3; k++) {
-      double v = std::floor(((double)pos[3 * i + k] - org[k]) * scale);
-      v = std::min(std::max(v, 0.0), gmax);
-      g[k] = (uint64_t)v;
-    }
-    // octant o = 4 bx + 2 by + bz at every level  ->  x is the most significant of each triple
-    const uint64_t key = (spread21(g[0]) << 2) | (spread21(g[1]) << 1) | spread21(g[2]);
-    keys[i].key = key; keys[i].idx = (uint32_t)i;
-    key_or |= key;
-  }
+  const uint64_t key_or = compute_keys(pos, n, org, scale, gmax, keys);
   lap("keys");
   {
     KeyIdx* const sorted = radix_sort(keys, tmp_keys, n, key_or, n_leaf);
