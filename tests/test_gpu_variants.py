@@ -97,3 +97,27 @@ def test_com_rule_trades_accuracy_for_interactions_1m():
           % (out[0] + out[1]))
     assert out[1][1] < 0.75 * out[0][1] and out[1][0] < out[0][0]
     assert out[0][2] < out[1][2] < 6 * out[0][2]
+
+
+def test_group_box_1m_sampled_groups():
+    """R23 at config 3 (full size, the launch configuration of bench.py): counts exact and forces within the bars on
+    sampled groups; fewer interactions than the cube rule."""
+    pos, mass, theta, eps, n_leaf = inputs.make("plummer_1m")
+    with B.TreeCode() as tc:                                   # default N_group (96)
+        tc.set_particles(pos, mass)
+        tc.build(n_leaf)
+        n_group = tc.stats()["n_group"]
+        tc.forces(theta, eps)
+        base = tc.stats()
+        tc.set_option("group_box", 1)
+        acc, pot = tc.forces(theta, eps)
+        tc.forces(theta, eps)
+        n_pc, n_pp = tc.counts()
+        st = tc.stats()
+    o = Oracle(pos, mass, n_leaf, n_group, group_box=True)
+    gsel = np.sort(np.random.default_rng(23).choice(o.n_groups, 192, replace=False)).astype(np.int64)
+    ref = o.forces(theta, eps, shadow32=True, groups=gsel)
+    check(acc, pot, n_pc, n_pp, ref, ref["n_pc"] >= 0)
+    tot, tot0 = st["n_pc_total"] + st["n_pp_total"], base["n_pc_total"] + base["n_pp_total"]
+    print("group_box at config 3: %.3f ms, %.4e interactions (cube rule: %.3f ms, %.4e)" % (st["t_gpu_ms"], tot, base["t_gpu_ms"], tot0))
+    assert tot < tot0 and st["n_tests_total"] < base["n_tests_total"]
