@@ -50,6 +50,7 @@ struct tc_ctx {
   bool tree_host_valid = false;       // the host copy of the packed tree (tc_get_tree) is current
   bool host_particles_valid = false;  // pos/mass below hold the current particles (else only d_src does)
   float4* h_src = nullptr; int64_t h_src_cap = 0;     // pinned staging of (x,y,z,m) for the device build
+  float* d_raw = nullptr; int64_t raw_cap = 0;        // device landing area of PINNED host inputs (pos [3n] | mass [n])
   unsigned int* d_flags = nullptr;
   // tc_direct scratch
   float4* d_src = nullptr; int64_t src_cap = 0; bool src_valid = false;
@@ -67,6 +68,14 @@ int cuda_fail(tc_ctx* c, cudaError_t e, const char* what) {
               std::string(what) + ": " + cudaGetErrorString(e));
 }
 #define TC_CUDA(c, call) do { cudaError_t e_ = (call); if (e_ != cudaSuccess) return cuda_fail(c, e_, #call); } while (0)
+
+// page-locked host memory (cudaHostAlloc / cudaHostRegister, e.g. torch pin_memory): DMA reads it directly
+bool is_pinned_host_ptr(const tc_ctx* c, const void* p) {
+  if (c->host_only || !p) return false;
+  cudaPointerAttributes a;
+  if (cudaPointerGetAttributes(&a, p) != cudaSuccess) { cudaGetLastError(); return false; }
+  return a.type == cudaMemoryTypeHost;
+}
 
 bool is_device_ptr(const tc_ctx* c, const void* p) {
   if (c->host_only || !p) return false;
@@ -203,7 +212,7 @@ void tc_destroy(tc_ctx* c) {
     c->dscr.release();
     c->tps.release();
     if (c->h_src) cudaFreeHost(c->h_src);
-    cudaFree(c->d_flags);
+    cudaFree(c->d_flags); cudaFree(c->d_raw);
     cudaFree(c->d_src); cudaFree(c->d_tgt); cudaFree(c->d_dacc); cudaFree(c->d_dpot);
     if (c->ev0) cudaEventDestroy(c->ev0);
     if (c->ev1) cudaEventDestroy(c->ev1);
@@ -293,9 +302,24 @@ int tc_set_particles(tc_ctx* c, const float* pos, const float* mass, int64_t n) 
     }
     if (!c->d_flags) TC_CUDA(c, cudaMalloc((void**)&c->d_flags, sizeof(unsigned int)));
   }
-  if (dev_mode && pos_dev && mass_dev) {
-    // device inputs, device build: nothing travels; interleave + validate in one kernel
-    const int le = tc::pack_src_device(pos, mass, n, c->d_src, c->d_flags, c->stream);
+  // device build with PINNED host inputs: DMA them as they are and let the pack kernel interleave and validate —
+  // no host pass over the particles at all (pageable inputs keep the parallel staging pass below, which is
+  // faster than the driver's own staging of pageable memory)
+  const bool pos_pin = dev_mode && !pos_dev && is_pinned_host_ptr(c, pos), mass_pin = dev_mode && !mass_dev && is_pinned_host_ptr(c, mass);
+  if (dev_mode && (pos_dev || pos_pin) && (mass_dev || mass_pin)) {
+    const float* dp = pos; const float* dm = mass;
+    if (pos_pin || mass_pin) {
+      if (c->raw_cap < n) {
+        TC_CUDA(c, cudaStreamSynchronize(c->stream));
+        cudaFree(c->d_raw); c->d_raw = nullptr; c->raw_cap = 0;
+        TC_CUDA(c, cudaMalloc((void**)&c->d_raw, sizeof(float) * 4 * (size_t)n));
+        c->raw_cap = n;
+      }
+      if (pos_pin) { TC_CUDA(c, cudaMemcpyAsync(c->d_raw, pos, sizeof(float) * 3 * (size_t)n, cudaMemcpyHostToDevice, c->stream)); dp = c->d_raw; }
+      if (mass_pin) { TC_CUDA(c, cudaMemcpyAsync(c->d_raw + 3 * (size_t)n, mass, sizeof(float) * (size_t)n, cudaMemcpyHostToDevice, c->stream)); dm = c->d_raw + 3 * (size_t)n; }
+    }
+    // device (or landed) inputs, device build: interleave + validate in one kernel
+    const int le = tc::pack_src_device(dp, dm, n, c->d_src, c->d_flags, c->stream);
     if (le != 0) return cuda_fail(c, (cudaError_t)le, "tc_set_particles: pack kernel");
     unsigned int flags = 0;
     TC_CUDA(c, cudaMemcpyAsync(&flags, c->d_flags, sizeof(flags), cudaMemcpyDeviceToHost, c->stream));

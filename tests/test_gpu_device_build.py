@@ -150,3 +150,35 @@ def test_device_build_rejects_bad_particles_and_switches_back_to_host():
         acc, pot = tc.forces(0.5, 0.01)
         n_pc, n_pp = tc.counts()
     check(acc, pot, n_pc, n_pp, Oracle(pos, mass, 16, 96).forces(0.5, 0.01, shadow32=True))
+
+
+def test_pinned_host_inputs_take_the_direct_dma_path_and_bad_values_are_still_refused():
+    """Device build with PAGE-LOCKED host inputs: DMA + pack kernel, no host pass — same tree, same forces as with
+    pageable inputs; validation now happens in the pack kernel."""
+    import torch
+    pos, mass, theta, eps, n_leaf = inputs.make("plummer_64k")
+    p_pin, m_pin = torch.from_numpy(pos).pin_memory().numpy(), torch.from_numpy(mass).pin_memory().numpy()
+    out = []
+    for p, m in ((pos, mass), (p_pin, m_pin), (p_pin, mass)):       # pageable, pinned, mixed
+        with B.TreeCode() as tc:
+            tc.set_option("device_build", 1)
+            tc.set_particles(p, m)
+            tc.build(n_leaf)
+            acc, pot = tc.forces(theta, eps)
+            out.append((acc, pot, tc.counts(), tc.stats()["n_cells"]))
+    for o in out[1:]:
+        assert np.array_equal(o[0], out[0][0]) and np.array_equal(o[1], out[0][1]) and o[3] == out[0][3]
+        assert np.array_equal(o[2][0], out[0][2][0]) and np.array_equal(o[2][1], out[0][2][1])
+    bad = torch.from_numpy(pos.copy()).pin_memory().numpy()
+    bad[7, 1] = np.inf
+    with B.TreeCode() as tc:
+        tc.set_option("device_build", 1)
+        with pytest.raises(B.TcError) as e:
+            tc.set_particles(bad, m_pin)
+        assert e.value.code == B.TC_EINVAL
+        tc.set_particles(p_pin, m_pin)                                # the context is still usable
+        tc.build(n_leaf)
+        tc.set_option("device_build", 0)                              # host build needs the host copy: fetched lazily
+        tc.build(n_leaf)
+        acc, _ = tc.forces(theta, eps)
+        assert np.abs(acc - out[0][0]).max() <= 2e-6 * np.abs(out[0][0]).max()
