@@ -216,16 +216,6 @@ int build_host_tree(const float* pos, const float* mass, int64_t n, int n_leaf, 
     if (sorted != keys) std::swap(keys, tmp_keys);
   }
   lap("sort");
-  // particles in tree (Morton) order, staged in the sort's other buffer (same 16 bytes per element): the
-  // moments and the pack below read them sequentially instead of gathering through keys[t].idx
-  static_assert(sizeof(KeyIdx) == sizeof(float4), "the sort scratch doubles as the sorted particle array");
-  float4* sp = reinterpret_cast<float4*>(tmp_keys);
-#pragma omp parallel for schedule(static)
-  for (int64_t t = 0; t < n; t++) {
-    const int64_t i = keys[t].idx;
-    sp[t] = make_float4(pos[3 * i], pos[3 * i + 1], pos[3 * i + 2], mass[i]);
-  }
-  lap("gather");
 
   // ---- O2: breadth-first split of sorted key ranges
   // cell arrays (struct of vectors), breadth-first, children contiguous
@@ -291,6 +281,52 @@ int build_host_tree(const float* pos, const float* mass, int64_t n, int n_leaf, 
   const int n_levels = (int)level_start.size() - 1;
 
   lap("split");
+  // ---- O4: groups = maximal cells with count <= N_group, or leaves, Morton order
+  std::vector<int32_t>& groups = T.scratch.groups;
+  groups.clear();
+  {
+    std::vector<int32_t> st;
+    st.push_back(0);
+    while (!st.empty()) {
+      const int32_t c = st.back(); st.pop_back();
+      if (c_count[c] <= n_group || c_nchild[c] == 0) { groups.push_back(c); continue; }
+      for (int j = c_nchild[c] - 1; j >= 0; j--) st.push_back(c_first_child[c] + j);
+    }
+  }
+  T.n_groups = (int64_t)groups.size();
+
+  // ---- pack: SoA float4 arrays in one buffer (PAPER.md:51-53; layout in tc_internal.h)
+  PackedLayout& Y = T.lay;
+  size_t off = 0;
+  Y.off_bnd = off;  off = align256(off + sizeof(float4) * (size_t)nc);
+  Y.off_xm = off;   off = align256(off + sizeof(float4) * (size_t)nc);
+  Y.off_q0 = off;   off = align256(off + sizeof(float4) * (size_t)nc);
+  Y.off_q1 = off;   off = align256(off + sizeof(float4) * (size_t)nc);
+  Y.off_part = off; off = align256(off + sizeof(float4) * (size_t)n);
+  Y.off_orig = off; off = align256(off + sizeof(int32_t) * (size_t)n);
+  Y.off_grp = off;  off = align256(off + sizeof(int4) * groups.size());
+  Y.off_gbox = off; off = align256(off + sizeof(float4) * groups.size());
+  Y.bytes = off;
+  char* base = (char*)alloc(alloc_user, Y.bytes);
+  if (!base) { msg = "build: cannot allocate the packed tree buffer"; return TC_ENOMEM; }
+  float4* bnd = (float4*)(base + Y.off_bnd);
+  float4* xm = (float4*)(base + Y.off_xm);
+  float4* q0 = (float4*)(base + Y.off_q0);
+  float4* q1 = (float4*)(base + Y.off_q1);
+  float4* part = (float4*)(base + Y.off_part);
+  int32_t* orig = (int32_t*)(base + Y.off_orig);
+  int4* grp = (int4*)(base + Y.off_grp);
+  float4* gbox = (float4*)(base + Y.off_gbox);
+  lap("groups");
+  // particles in tree (Morton) order, gathered ONCE straight into the packed buffer: the moments below and the
+  // kernels read them sequentially
+#pragma omp parallel for schedule(static)
+  for (int64_t t = 0; t < n; t++) {
+    const int64_t i = keys[t].idx;
+    part[t] = make_float4(pos[3 * i], pos[3 * i + 1], pos[3 * i + 2], mass[i]);
+    orig[t] = (int32_t)i;
+  }
+  lap("gather");
   // ---- O3: cell properties, fp64, bottom-up.  Leaves: direct sums
   // over members.  Nodes: union of the children's boxes, parallel-axis shift of the
   // children's moments to the node's centre of mass.
@@ -308,7 +344,7 @@ int build_host_tree(const float* pos, const float* mass, int64_t n, int n_leaf, 
         float mn[3] = {INFINITY, INFINITY, INFINITY}, mx[3] = {-INFINITY, -INFINITY, -INFINITY};
         const int64_t pb = c_begin[c], pe = pb + c_count[c];
         for (int64_t t = pb; t < pe; t++) {
-          const float4 b = sp[t];
+          const float4 b = part[t];
           const float xyz[3] = {b.x, b.y, b.z};
           const double m = (double)b.w;
           for (int k = 0; k < 3; k++) {
@@ -324,7 +360,7 @@ int build_host_tree(const float* pos, const float* mass, int64_t n, int n_leaf, 
           P.X[k] = (M > 0.0) ? S[k] / M : ((double)mn[k] + (double)mx[k]) / 2.0;
         double Q[6] = {0, 0, 0, 0, 0, 0};
         for (int64_t t = pb; t < pe; t++) {
-          const float4 b = sp[t];
+          const float4 b = part[t];
           const double m = (double)b.w;
           const double yx = (double)b.x - P.X[0], yy = (double)b.y - P.X[1], yz = (double)b.z - P.X[2];
           const double y2 = yx * yx + yy * yy + yz * yz;
@@ -363,43 +399,6 @@ int build_host_tree(const float* pos, const float* mass, int64_t n, int n_leaf, 
   T.n_leaves = n_leaves;
 
   lap("moments");
-  // ---- O4: groups = maximal cells with count <= N_group, or leaves, Morton order
-  std::vector<int32_t>& groups = T.scratch.groups;
-  groups.clear();
-  {
-    std::vector<int32_t> st;
-    st.push_back(0);
-    while (!st.empty()) {
-      const int32_t c = st.back(); st.pop_back();
-      if (c_count[c] <= n_group || c_nchild[c] == 0) { groups.push_back(c); continue; }
-      for (int j = c_nchild[c] - 1; j >= 0; j--) st.push_back(c_first_child[c] + j);
-    }
-  }
-  T.n_groups = (int64_t)groups.size();
-
-  lap("groups");
-  // ---- pack: SoA float4 arrays in one buffer (PAPER.md:51-53; layout in tc_internal.h)
-  PackedLayout& Y = T.lay;
-  size_t off = 0;
-  Y.off_bnd = off;  off = align256(off + sizeof(float4) * (size_t)nc);
-  Y.off_xm = off;   off = align256(off + sizeof(float4) * (size_t)nc);
-  Y.off_q0 = off;   off = align256(off + sizeof(float4) * (size_t)nc);
-  Y.off_q1 = off;   off = align256(off + sizeof(float4) * (size_t)nc);
-  Y.off_part = off; off = align256(off + sizeof(float4) * (size_t)n);
-  Y.off_orig = off; off = align256(off + sizeof(int32_t) * (size_t)n);
-  Y.off_grp = off;  off = align256(off + sizeof(int4) * groups.size());
-  Y.off_gbox = off; off = align256(off + sizeof(float4) * groups.size());
-  Y.bytes = off;
-  char* base = (char*)alloc(alloc_user, Y.bytes);
-  if (!base) { msg = "build: cannot allocate the packed tree buffer"; return TC_ENOMEM; }
-  float4* bnd = (float4*)(base + Y.off_bnd);
-  float4* xm = (float4*)(base + Y.off_xm);
-  float4* q0 = (float4*)(base + Y.off_q0);
-  float4* q1 = (float4*)(base + Y.off_q1);
-  float4* part = (float4*)(base + Y.off_part);
-  int32_t* orig = (int32_t*)(base + Y.off_orig);
-  int4* grp = (int4*)(base + Y.off_grp);
-  float4* gbox = (float4*)(base + Y.off_gbox);
   try { T.link.resize((size_t)nc * 4); T.q6.resize((size_t)nc * 6); } catch (...) { msg = "build: out of host memory"; return TC_ENOMEM; }
 
 #pragma omp parallel for schedule(static)
@@ -433,11 +432,6 @@ int build_host_tree(const float* pos, const float* mass, int64_t n, int n_leaf, 
     T.link[4 * c + 2] = c_begin[c];
     T.link[4 * c + 3] = c_count[c];
     for (int k = 0; k < 6; k++) T.q6[6 * c + k] = (float)P.Q[k];
-  }
-#pragma omp parallel for schedule(static)
-  for (int64_t t = 0; t < n; t++) {
-    part[t] = sp[t];
-    orig[t] = (int32_t)keys[t].idx;
   }
   lap("pack");
   // Schedule (grp[i].w = i-th group to run): the persistent kernel hands groups out through an
