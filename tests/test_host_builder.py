@@ -110,3 +110,13 @@ def test_deep_clusters_through_the_radix_sort_fixup():
     pos[9000:9300] = pos[9000]                                                                            # level-21 leaf
     mass = np.full(n, 1.0 / n, np.float32)
     _compare(pos, mass, 8, 32)
+
+
+def test_far_outlier_takes_the_lopsided_sort_path():
+    """One escaper stretches the root cube: every other particle shares the top digits of its key, so the bucketed
+    sort would run on one thread and the builder falls back to three global passes — same tree either way."""
+    rng = np.random.default_rng(10)
+    n = 70000
+    pos = (1e-3 * rng.standard_normal((n, 3))).astype(np.float32)
+    pos[123] = (100.0, 100.0, 100.0)
+    _compare(pos, np.full(n, 1.0 / n, np.float32), 16, 64)
