@@ -49,8 +49,14 @@ namespace {
 #endif
 constexpr int kWarpsPerCta = TC_WARPS;
 constexpr int kCellCap = TC_CELLCAP;  // un-opened cells staged per warp before evaluation
-constexpr int kLeafQCap = 128;   // opened-leaf ranges queued per warp
-constexpr int kBodyCap = 128;    // bodies staged per warp per evaluation round
+#ifndef TC_LEAFQCAP
+#define TC_LEAFQCAP 256
+#endif
+constexpr int kLeafQCap = TC_LEAFQCAP;   // opened-leaf ranges queued per warp
+#ifndef TC_BODYCAP
+#define TC_BODYCAP 384
+#endif
+constexpr int kBodyCap = TC_BODYCAP;   // bodies staged per warp per evaluation round
 constexpr int kMaxKP = TC_MAXKP; // particle PAIRS per lane (packed f32x2 arithmetic)
 // Particles of a group handled per walk.  64 * kMaxKP would fit, but splitting a larger group into
 // passes of 64 keeps the lanes fuller (96 = 64 + 32 costs 1 + 1/2 pair-slots, one pass of 96 costs 2)
