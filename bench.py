@@ -47,7 +47,7 @@ PAPER_FLOPS_PC, PAPER_FLOPS_PP = 70, 38
 N_SM, LANES = 148, 128
 L2_FLUSH_BYTES = 256 << 20        # > 126 MB L2
 # DRAM bytes of one launch of the force kernel at config 3, from the committed ncu capture (profiles/)
-DRAM_TRAFFIC_BYTES = 67684864
+DRAM_TRAFFIC_BYTES = 74562048
 
 
 def fp32_peak_tflops(mhz: float) -> float:
@@ -323,7 +323,7 @@ def run_ours(args) -> None:
                      "peak_measured_how": "tc_fp32_peak: FFMA-only microbenchmark on this device in this run",
                      "flops_per_launch": flops, "algorithmic_bytes_per_launch": int(tree_bytes + 24 * n),
                      "traffic_how": "dram__bytes_read.sum + dram__bytes_write.sum of one ncu --set full capture "
-                                    "(profiles/r01c_final.md); HBM is not the bound"},
+                                    "(profiles/r01d_final.md); HBM is not the bound"},
     }
     out["cpu_baseline"] = cpu_baseline(*inputs.make(WORKLOAD)) if world == 1 else None
     print(json.dumps(out), flush=True)
