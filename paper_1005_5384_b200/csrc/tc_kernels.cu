@@ -332,7 +332,8 @@ template <bool kAdd, bool kSelf>
 __device__ __forceinline__ void write_back(const Lanes& L, const Acc2 (&A)[kMaxKP], const float4* __restrict__ part,
                                            const int32_t* __restrict__ orig, int first, int m, float eps2, int lane,
                                            float* __restrict__ acc, float* __restrict__ pot, int32_t* __restrict__ out_cnt,
-                                           int cnt_value, int32_t* __restrict__ out_cnt2 = nullptr, int cnt2_value = 0) {
+                                           int cnt_value, int32_t* __restrict__ out_cnt2 = nullptr, int cnt2_value = 0,
+                                           bool self_met = true) {
 #pragma unroll
   for (int j = 0; j < 2 * kMaxKP; j++) {
     if (j >= 2 * L.kp) break;                        // warp-uniform
@@ -349,7 +350,7 @@ __device__ __forceinline__ void write_back(const Lanes& L, const Acc2 (&A)[kMaxK
     if (lane < L.q && tq < m) {
       const int t = first + tq;
       const int i = __ldg(orig + t);
-      if (kSelf) ph += __ldg(part + t).w * rsqrt_approx(eps2);     // the particle met itself once
+      if (kSelf && self_met) ph += __ldg(part + t).w * rsqrt_approx(eps2);     // the particle met itself once
       float* a3 = acc + 3 * (size_t)i;
       if (kAdd) { a3[0] += ax; a3[1] += ay; a3[2] += az; if (pot) pot[i] += ph; }
       else { a3[0] = ax; a3[1] = ay; a3[2] = az; if (pot) pot[i] = ph; }
@@ -427,6 +428,12 @@ forces_kernel(const float4* __restrict__ bnd, const float4* __restrict__ xm, con
       long long n_pc = 0, n_pp = 0, n_tests = 0;
       int n_spills = 0, n_lr = 0;                        // n_lr: opened-leaf ranges so far
       bool overflow = false;
+      // Did the pass's particles meet themselves in the particle-particle part?  Always, under the default
+      // rule (the boxes of the group and of its ancestors overlap, d = 0, they open).  Under the COM rule (R21)
+      // an ancestor whose centre of mass lies far outside the group's cube can stay UN-opened at large theta:
+      // the group then sees its own mass through that cell's multipole (the variant's known flaw, kept as the
+      // oracle has it) and there is no self pair to take out of the potential again.
+      bool self_met = kPlain || root_leaf;
       if (root_leaf) {
         if (lane == 0) {
           if (MODE == kFused) sm.leafq[0] = make_int2(root_a, root_n);
@@ -493,6 +500,10 @@ forces_kernel(const float4* __restrict__ bnd, const float4* __restrict__ xm, con
           }
           if (MODE == kFused) lq += __popc(m_leaf); else n_lr += __popc(m_leaf);
           n_pp += __reduce_add_sync(kFull, to_leaf ? lb : 0);
+          if (!kPlain && MODE == kFused) {                 // own leaf opened? (all or nothing per group, see above)
+            const int fb = G.y + pb;
+            self_met |= __any_sync(kFull, to_leaf && la <= fb && fb < la + lb);
+          }
         }
         if (m_stack) {                                   // opened node: walk on
           const int npush = __popc(m_stack);
@@ -536,7 +547,7 @@ forces_kernel(const float4* __restrict__ bnd, const float4* __restrict__ xm, con
       if (MODE == kFused) {
         // ---- A6: reduce the slices of every particle, write back in the caller's order
         write_back<false, !kEps0>(L, A, part, orig, G.y + pb, m, eps2, lane, acc, pot, out_npc, (int32_t)n_pc, out_npp,
-                                  (int32_t)(n_pp - 1));
+                                  (int32_t)(n_pp - 1), self_met);
       } else if (MODE == kCount) {
         if (lane == 0) { lio.cnt_c[g] = (unsigned long long)n_pc; lio.cnt_l[g] = (unsigned long long)n_lr; lio.leaf_bodies[g] = (int)n_pp; }
       }
@@ -622,14 +633,22 @@ leaf_kernel(const float4* __restrict__ part, const int32_t* __restrict__ orig, c
       const int m = min(kPass, G.z - pb);
       Lanes L; Pos2 P[kMaxKP]; Acc2 A[kMaxKP];
       setup_pass(L, P, A, part, G.y + pb, m, lane);
+      bool self_met = false;                 // is the pass's own leaf on the list? (see forces_kernel)
+      const int fb = G.y + pb;
       for (int base = 0; base < n_l; base += kLeafQCap) {
         const int cnt = min(kLeafQCap, n_l - base);
-        for (int t = lane; t < cnt; t += 32) sm.leafq[t] = __ldg(lio.leaves + b + base + t);
+        bool mine = false;
+        for (int t = lane; t < cnt; t += 32) {
+          const int2 r = __ldg(lio.leaves + b + base + t);
+          sm.leafq[t] = r;
+          mine |= (r.x <= fb && fb < r.x + r.y);
+        }
+        self_met |= __any_sync(kFull, mine);
         __syncwarp();
         eval_leaves<kEps0>(sm.u.bs, sm.leafq, cnt, part, eps2, L, P, A, lane);
         __syncwarp();
       }
-      write_back<true, !kEps0>(L, A, part, orig, G.y + pb, m, eps2, lane, acc, pot, out_npp, n_bodies - 1);
+      write_back<true, !kEps0>(L, A, part, orig, G.y + pb, m, eps2, lane, acc, pot, out_npp, n_bodies - 1, nullptr, 0, self_met);
     }
   }
 }
