@@ -39,10 +39,24 @@ inline uint64_t spread21(uint64_t v) {  // bit i -> bit 3i
   return v;
 }
 
-struct KeyIdx {
-  uint64_t key;
-  uint32_t idx;
+// Sort element: the top 3 BITS bits of the Morton key (the first BITS tree levels) above the particle index,
+// in ONE 64-bit word (half the memory traffic of a (key, idx) pair in every pass of the sort, and the arrays
+// of 2^20 particles stay in the cache).  The full keys are kept beside it, in the caller's order, for the rare
+// cells that are split below level BITS.
+struct SortPlan {
+  int bits;        // radix digit = tree levels per pass; three passes
+  int low;         // 63 - 3 bits: key bits below the sorted prefix
+  int idxb;        // 64 - 3 bits: index bits of an element
+  uint64_t imask;  // (1 << idxb) - 1
 };
+inline SortPlan sort_plan(int64_t n) {
+  // 11 bits (2048 bins: histograms and write streams stay in L1/L2) is fastest up to a few million particles; deeper
+  // trees want a longer prefix (fewer cells finished by the comparison sort), as far as the index still fits
+  const int bits = n <= (int64_t(1) << 22) ? 11 : n <= (int64_t(1) << 25) ? 13 : n <= (int64_t(1) << 28) ? 12 : 11;
+  SortPlan P;
+  P.bits = bits; P.low = 63 - 3 * bits; P.idxb = 64 - 3 * bits; P.imask = (uint64_t(1) << P.idxb) - 1;
+  return P;
+}
 
 // O1: integer grid coordinates and 63-bit Morton keys of all particles; returns the OR of all keys.
 // One body, two instantiations: baseline x86-64, and AVX2 + BMI2 (vectorised floor / min / max, bit
@@ -59,43 +73,47 @@ struct KeyIdx {
     }                                                                                               \
     /* octant o = 4 bx + 2 by + bz at every level  ->  x is the most significant of each triple */  \
     const uint64_t key = (SPREAD(g[0]) << 2) | (SPREAD(g[1]) << 1) | SPREAD(g[2]);                  \
-    keys[i].key = key; keys[i].idx = (uint32_t)i;                                                   \
+    fullkey[i] = key; elem[i] = ((key >> low) << idxb) | (uint64_t)i;                               \
     key_or |= key;                                                                                  \
   }                                                                                                 \
   return key_or;
 
-uint64_t compute_keys_base(const float* pos, int64_t n, const double* org, double scale, double gmax, KeyIdx* keys) {
+uint64_t compute_keys_base(const float* pos, int64_t n, const double* org, double scale, double gmax, uint64_t* fullkey,
+                           uint64_t* elem, int low, int idxb) {
   TC_KEYS_BODY(spread21)
 }
 #if defined(__x86_64__) && defined(__GNUC__)
 #define TC_PDEP21(x) __builtin_ia32_pdep_di((x), 0x1249249249249249ull)
 #pragma GCC push_options
 #pragma GCC target("avx2,bmi2")
-uint64_t compute_keys_v3(const float* pos, int64_t n, const double* org, double scale, double gmax, KeyIdx* keys) {
+uint64_t compute_keys_v3(const float* pos, int64_t n, const double* org, double scale, double gmax, uint64_t* fullkey,
+                         uint64_t* elem, int low, int idxb) {
   TC_KEYS_BODY(TC_PDEP21)
 }
 #pragma GCC pop_options
 #endif
-uint64_t compute_keys(const float* pos, int64_t n, const double* org, double scale, double gmax, KeyIdx* keys) {
+uint64_t compute_keys(const float* pos, int64_t n, const double* org, double scale, double gmax, uint64_t* fullkey,
+                      uint64_t* elem, int low, int idxb) {
 #if defined(__x86_64__) && defined(__GNUC__)
-  if (__builtin_cpu_supports("avx2") && __builtin_cpu_supports("bmi2")) return compute_keys_v3(pos, n, org, scale, gmax, keys);
+  if (__builtin_cpu_supports("avx2") && __builtin_cpu_supports("bmi2")) return compute_keys_v3(pos, n, org, scale, gmax, fullkey, elem, low, idxb);
 #endif
-  return compute_keys_base(pos, n, org, scale, gmax, keys);
+  return compute_keys_base(pos, n, org, scale, gmax, fullkey, elem, low, idxb);
 }
 
-// Sort of (key, idx) by key, stable (equal keys keep ascending idx).  Three LSD radix passes of BITS
-// bits order the keys by their top 3 BITS bits (BITS tree levels); a run of equal prefixes only needs
-// its low bits ordered when it is longer than `n_leaf` (it is then split below level BITS), which is
-// rare — those runs are finished with std::stable_sort.  BITS = 11 (2048 bins: histograms and write
-// streams stay in L1/L2) is fastest up to a few million particles, 13 above, where trees are deeper
-// and the fix-up of an 11-level prefix would dominate (measured: 2.5 vs 4.2 ms at N = 2^20, 40 vs 33 ms at 2^24).  Shorter runs end up inside one leaf, where the
-// order of the members is immaterial (it stays the caller's order).
+// Sort of the elements by Morton key, stable (equal keys keep ascending index).  Three LSD radix passes of BITS
+// bits order them by the key prefix they carry (BITS tree levels); a run of equal prefixes only needs its low
+// key bits ordered when it is longer than `n_leaf` (it is then split below level BITS), which is rare — those
+// runs are finished with std::stable_sort on the full keys.  Shorter runs end up inside one leaf, where the
+// order of the members is immaterial (it stays the caller's order).  (Measured with (key, idx) pairs: 11 bits
+// 2.5 vs 4.2 ms at N = 2^20, 13 bits 33 vs 40 ms at 2^24.)
 // Returns the buffer that holds the sorted array (`a` or `tmp`: no copy back after an odd number of passes).
 template <int BITS>
-KeyIdx* radix_sort_t(KeyIdx* a, KeyIdx* tmp, int64_t n, uint64_t key_or, int n_leaf) {
-  constexpr int R = 1 << BITS, LOW = 63 - 3 * BITS;
+uint64_t* radix_sort_t(uint64_t* a, uint64_t* tmp, int64_t n, uint64_t key_or, int n_leaf, const uint64_t* fullkey) {
+  constexpr int R = 1 << BITS, LOW = 63 - 3 * BITS, IDXB = 64 - 3 * BITS;
+  constexpr uint64_t IMASK = (uint64_t(1) << IDXB) - 1;
+  const auto by_full_key = [fullkey](uint64_t x, uint64_t y) { return fullkey[x & IMASK] < fullkey[y & IMASK]; };
   if (n < 8192) {   // small inputs: the histograms would cost more than the sort
-    std::stable_sort(a, a + n, [](const KeyIdx& x, const KeyIdx& y) { return x.key < y.key; });
+    std::stable_sort(a, a + n, by_full_key);
     return a;
   }
   int nthreads = 1;
@@ -104,10 +122,11 @@ KeyIdx* radix_sort_t(KeyIdx* a, KeyIdx* tmp, int64_t n, uint64_t key_or, int n_l
 #endif
   if (n < (1 << 16)) nthreads = 1;
   std::vector<int64_t> hist((size_t)nthreads * R);
-  KeyIdx* src = a;
-  KeyIdx* dst = tmp;
-  for (int shift = LOW; shift < 63; shift += BITS) {
-    if (((key_or >> shift) & (R - 1)) == 0) continue;  // digit is zero in every key
+  uint64_t* src = a;
+  uint64_t* dst = tmp;
+  for (int pass = 0; pass < 3; pass++) {
+    if (((key_or >> (LOW + pass * BITS)) & (R - 1)) == 0) continue;  // digit is zero in every key
+    const int shift = IDXB + pass * BITS;
     std::fill(hist.begin(), hist.end(), 0);
 #pragma omp parallel num_threads(nthreads)
     {
@@ -118,7 +137,7 @@ KeyIdx* radix_sort_t(KeyIdx* a, KeyIdx* tmp, int64_t n, uint64_t key_or, int n_l
 #endif
       const int64_t lo = n * t / nthreads, hi = n * (t + 1) / nthreads;
       int64_t* h = &hist[(size_t)t * R];
-      for (int64_t i = lo; i < hi; i++) h[(src[i].key >> shift) & (R - 1)]++;
+      for (int64_t i = lo; i < hi; i++) h[(src[i] >> shift) & (R - 1)]++;
 #pragma omp barrier
 #pragma omp single
       {
@@ -130,7 +149,7 @@ KeyIdx* radix_sort_t(KeyIdx* a, KeyIdx* tmp, int64_t n, uint64_t key_or, int n_l
             run += c;
           }
       }
-      for (int64_t i = lo; i < hi; i++) dst[h[(src[i].key >> shift) & (R - 1)]++] = src[i];
+      for (int64_t i = lo; i < hi; i++) dst[h[(src[i] >> shift) & (R - 1)]++] = src[i];
     }
     std::swap(src, dst);
   }
@@ -138,18 +157,22 @@ KeyIdx* radix_sort_t(KeyIdx* a, KeyIdx* tmp, int64_t n, uint64_t key_or, int n_l
   // finish the long runs (parallel over run starts; runs are disjoint)
 #pragma omp parallel for schedule(dynamic, 65536)
   for (int64_t i = 0; i < n; i++) {
-    const uint64_t pre = a[i].key >> LOW;
-    if (i > 0 && (a[i - 1].key >> LOW) == pre) continue;      // not a run start
+    const uint64_t pre = a[i] >> IDXB;
+    if (i > 0 && (a[i - 1] >> IDXB) == pre) continue;      // not a run start
     int64_t j = i + 1;
-    while (j < n && j - i <= n_leaf && (a[j].key >> LOW) == pre) j++;
+    while (j < n && j - i <= n_leaf && (a[j] >> IDXB) == pre) j++;
     if (j - i <= n_leaf) continue;
-    while (j < n && (a[j].key >> LOW) == pre) j++;
-    std::stable_sort(a + i, a + j, [](const KeyIdx& x, const KeyIdx& y) { return x.key < y.key; });
+    while (j < n && (a[j] >> IDXB) == pre) j++;
+    std::stable_sort(a + i, a + j, by_full_key);
   }
   return a;
 }
-KeyIdx* radix_sort(KeyIdx* a, KeyIdx* tmp, int64_t n, uint64_t key_or, int n_leaf) {
-  return n > (int64_t(1) << 22) ? radix_sort_t<13>(a, tmp, n, key_or, n_leaf) : radix_sort_t<11>(a, tmp, n, key_or, n_leaf);
+uint64_t* radix_sort(const SortPlan& P, uint64_t* a, uint64_t* tmp, int64_t n, uint64_t key_or, int n_leaf, const uint64_t* fullkey) {
+  switch (P.bits) {
+    case 13: return radix_sort_t<13>(a, tmp, n, key_or, n_leaf, fullkey);
+    case 12: return radix_sort_t<12>(a, tmp, n, key_or, n_leaf, fullkey);
+    default: return radix_sort_t<11>(a, tmp, n, key_or, n_leaf, fullkey);
+  }
 }
 
 struct CellProp {   // fp64 moments, fp32-exact bounding box
@@ -206,15 +229,13 @@ int build_host_tree(const float* pos, const float* mass, int64_t n, int n_leaf, 
 
   // key buffers: plain arrays (no zero fill; every element is written below)
   // (from the context's grow-only scratch: a rebuild touches no fresh pages)
-  KeyIdx* keys = static_cast<KeyIdx*>(T.scratch.get(0, sizeof(KeyIdx) * (size_t)n));
-  KeyIdx* tmp_keys = static_cast<KeyIdx*>(T.scratch.get(1, sizeof(KeyIdx) * (size_t)n));
-  if (!keys || !tmp_keys) { msg = "build: out of host memory"; return TC_ENOMEM; }
-  const uint64_t key_or = compute_keys(pos, n, org, scale, gmax, keys);
+  const SortPlan SP = sort_plan(n);
+  uint64_t* const fullkey = static_cast<uint64_t*>(T.scratch.get(0, sizeof(uint64_t) * (size_t)n));   // caller's order
+  uint64_t* keys = static_cast<uint64_t*>(T.scratch.get(1, sizeof(uint64_t) * 2 * (size_t)n));        // elements, and their twin
+  if (!fullkey || !keys) { msg = "build: out of host memory"; return TC_ENOMEM; }
+  const uint64_t key_or = compute_keys(pos, n, org, scale, gmax, fullkey, keys, SP.low, SP.idxb);
   lap("keys");
-  {
-    KeyIdx* const sorted = radix_sort(keys, tmp_keys, n, key_or, n_leaf);
-    if (sorted != keys) std::swap(keys, tmp_keys);
-  }
+  keys = radix_sort(SP, keys, keys + n, n, key_or, n_leaf, fullkey);
   lap("sort");
 
   // ---- O2: breadth-first split of sorted key ranges
@@ -232,6 +253,11 @@ int build_host_tree(const float* pos, const float* mass, int64_t n, int n_leaf, 
     level_start.push_back(lvl_e);
     if (level == kMaxLevel) break;
     const int shift = 3 * (kMaxLevel - 1 - level);
+    // the octant digit of this level: inside the element's prefix for the first `bits` levels, from the full key below
+    const bool in_prefix = level < SP.bits;
+    const int pshift = SP.idxb + 3 * (SP.bits - 1 - level);
+    const uint64_t imask = SP.imask;
+    const auto octant = [=](uint64_t q) -> uint64_t { return in_prefix ? (q >> pshift) & 7 : (fullkey[q & imask] >> shift) & 7; };
     const int64_t nl = lvl_e - lvl_b;
     nch.assign((size_t)nl + 1, 0);
     // pass 1: the non-empty octants of every node of this level; their starts are kept for pass 2
@@ -241,16 +267,16 @@ int build_host_tree(const float* pos, const float* mass, int64_t n, int n_leaf, 
 #pragma omp parallel for schedule(dynamic, 256)
     for (int64_t c = lvl_b; c < lvl_e; c++) {
       if (c_count[c] <= n_leaf) continue;  // leaf (R4: <=)
-      const KeyIdx* kb = keys + c_begin[c];
-      const KeyIdx* ke = kb + c_count[c];
+      const uint64_t* kb = keys + c_begin[c];
+      const uint64_t* ke = kb + c_count[c];
       int32_t* bd = bnds + 9 * (size_t)(c - lvl_b);
       int cnt = 0;
-      const KeyIdx* p = kb;
+      const uint64_t* p = kb;
       while (p < ke) {
-        const uint64_t o = (p->key >> shift) & 7;
+        const uint64_t o = octant(*p);
         bd[cnt++] = (int32_t)(p - keys);
         // first key of this cell with octant > o
-        p = std::partition_point(p, ke, [&](const KeyIdx& q) { return ((q.key >> shift) & 7) <= o; });
+        p = std::partition_point(p, ke, [&](uint64_t q) { return octant(q) <= o; });
       }
       bd[cnt] = (int32_t)(ke - keys);
       nch[(size_t)(c - lvl_b)] = cnt;
@@ -322,7 +348,7 @@ int build_host_tree(const float* pos, const float* mass, int64_t n, int n_leaf, 
   // kernels read them sequentially
 #pragma omp parallel for schedule(static)
   for (int64_t t = 0; t < n; t++) {
-    const int64_t i = keys[t].idx;
+    const int64_t i = (int64_t)(keys[t] & SP.imask);
     part[t] = make_float4(pos[3 * i], pos[3 * i + 1], pos[3 * i + 2], mass[i]);
     orig[t] = (int32_t)i;
   }
