@@ -44,14 +44,14 @@ inline uint64_t spread21(uint64_t v) {  // bit i -> bit 3i
 // of 2^20 particles stay in the cache).  The full keys are kept beside it, in the caller's order, for the rare
 // cells that are split below level BITS.
 struct SortPlan {
-  int bits;        // radix digit = tree levels per pass; three passes
+  int bits;        // tree levels covered by the sorted prefix (3 bits each)
   int low;         // 63 - 3 bits: key bits below the sorted prefix
   int idxb;        // 64 - 3 bits: index bits of an element
   uint64_t imask;  // (1 << idxb) - 1
 };
 inline SortPlan sort_plan(int64_t n) {
-  // 11 bits (2048 bins: histograms and write streams stay in L1/L2) is fastest up to a few million particles; deeper
-  // trees want a longer prefix (fewer cells finished by the comparison sort), as far as the index still fits
+  // a prefix of 11 levels is enough up to a few million particles; deeper trees want a longer one (fewer cells
+  // finished by the comparison sort: 33 vs 40 ms at N = 2^24), as far as the index still fits beside it
   const int bits = n <= (int64_t(1) << 22) ? 11 : n <= (int64_t(1) << 25) ? 13 : n <= (int64_t(1) << 28) ? 12 : 11;
   SortPlan P;
   P.bits = bits; P.low = 63 - 3 * bits; P.idxb = 64 - 3 * bits; P.imask = (uint64_t(1) << P.idxb) - 1;
@@ -100,16 +100,18 @@ uint64_t compute_keys(const float* pos, int64_t n, const double* org, double sca
   return compute_keys_base(pos, n, org, scale, gmax, fullkey, elem, low, idxb);
 }
 
-// Sort of the elements by Morton key, stable (equal keys keep ascending index).  Three LSD radix passes of BITS
-// bits order them by the key prefix they carry (BITS tree levels); a run of equal prefixes only needs its low
+// Sort of the elements by Morton key, stable (equal keys keep ascending index).  NP LSD radix passes
+// order them by the 3 BITS-bit key prefix they carry (BITS tree levels); a run of equal prefixes only needs its low
 // key bits ordered when it is longer than `n_leaf` (it is then split below level BITS), which is rare — those
 // runs are finished with std::stable_sort on the full keys.  Shorter runs end up inside one leaf, where the
 // order of the members is immaterial (it stays the caller's order).  (Measured with (key, idx) pairs: 11 bits
 // 2.5 vs 4.2 ms at N = 2^20, 13 bits 33 vs 40 ms at 2^24.)
 // Returns the buffer that holds the sorted array (`a` or `tmp`: no copy back after an odd number of passes).
-template <int BITS>
+template <int BITS, int NP>
 uint64_t* radix_sort_t(uint64_t* a, uint64_t* tmp, int64_t n, uint64_t key_or, int n_leaf, const uint64_t* fullkey) {
-  constexpr int R = 1 << BITS, LOW = 63 - 3 * BITS, IDXB = 64 - 3 * BITS;
+  // the 3 BITS prefix bits are sorted in NP passes; the first (3 BITS) % NP passes take one bit more
+  constexpr int WB = (3 * BITS) / NP, WREM = (3 * BITS) % NP;
+  constexpr int R = 1 << (WB + (WREM ? 1 : 0)), LOW = 63 - 3 * BITS, IDXB = 64 - 3 * BITS;
   constexpr uint64_t IMASK = (uint64_t(1) << IDXB) - 1;
   const auto by_full_key = [fullkey](uint64_t x, uint64_t y) { return fullkey[x & IMASK] < fullkey[y & IMASK]; };
   if (n < 8192) {   // small inputs: the histograms would cost more than the sort
@@ -124,9 +126,13 @@ uint64_t* radix_sort_t(uint64_t* a, uint64_t* tmp, int64_t n, uint64_t key_or, i
   std::vector<int64_t> hist((size_t)nthreads * R);
   uint64_t* src = a;
   uint64_t* dst = tmp;
-  for (int pass = 0; pass < 3; pass++) {
-    if (((key_or >> (LOW + pass * BITS)) & (R - 1)) == 0) continue;  // digit is zero in every key
-    const int shift = IDXB + pass * BITS;
+  int done = 0;                                                       // prefix bits already sorted
+  for (int pass = 0; pass < NP; pass++) {
+    const int w = WB + (pass < WREM ? 1 : 0);
+    const uint64_t dmask = (uint64_t(1) << w) - 1;
+    const int shift = IDXB + done;
+    done += w;
+    if (((key_or >> (shift - IDXB + LOW)) & dmask) == 0) continue;    // digit is zero in every key
     std::fill(hist.begin(), hist.end(), 0);
 #pragma omp parallel num_threads(nthreads)
     {
@@ -137,7 +143,7 @@ uint64_t* radix_sort_t(uint64_t* a, uint64_t* tmp, int64_t n, uint64_t key_or, i
 #endif
       const int64_t lo = n * t / nthreads, hi = n * (t + 1) / nthreads;
       int64_t* h = &hist[(size_t)t * R];
-      for (int64_t i = lo; i < hi; i++) h[(src[i] >> shift) & (R - 1)]++;
+      for (int64_t i = lo; i < hi; i++) h[(src[i] >> shift) & dmask]++;
 #pragma omp barrier
 #pragma omp single
       {
@@ -149,7 +155,7 @@ uint64_t* radix_sort_t(uint64_t* a, uint64_t* tmp, int64_t n, uint64_t key_or, i
             run += c;
           }
       }
-      for (int64_t i = lo; i < hi; i++) dst[h[(src[i] >> shift) & (R - 1)]++] = src[i];
+      for (int64_t i = lo; i < hi; i++) dst[h[(src[i] >> shift) & dmask]++] = src[i];
     }
     std::swap(src, dst);
   }
@@ -168,10 +174,12 @@ uint64_t* radix_sort_t(uint64_t* a, uint64_t* tmp, int64_t n, uint64_t key_or, i
   return a;
 }
 uint64_t* radix_sort(const SortPlan& P, uint64_t* a, uint64_t* tmp, int64_t n, uint64_t key_or, int n_leaf, const uint64_t* fullkey) {
+  // passes: 4 x 8-9 bits for the 33-bit prefix (256-512 write streams per thread stay in L1: 1.8 vs 2.1 ms at N = 2^20,
+  // 5 passes 2.6 ms); the longer prefixes of large N are memory-bound per pass, so 3 passes (23 vs 31 ms at 2^24)
   switch (P.bits) {
-    case 13: return radix_sort_t<13>(a, tmp, n, key_or, n_leaf, fullkey);
-    case 12: return radix_sort_t<12>(a, tmp, n, key_or, n_leaf, fullkey);
-    default: return radix_sort_t<11>(a, tmp, n, key_or, n_leaf, fullkey);
+    case 13: return radix_sort_t<13, 3>(a, tmp, n, key_or, n_leaf, fullkey);
+    case 12: return radix_sort_t<12, 3>(a, tmp, n, key_or, n_leaf, fullkey);
+    default: return radix_sort_t<11, 4>(a, tmp, n, key_or, n_leaf, fullkey);
   }
 }
 

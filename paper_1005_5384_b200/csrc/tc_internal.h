@@ -59,7 +59,7 @@ struct HostTree {
   void* packed = nullptr;  // lay.bytes, owned by the ctx (pinned or malloc)
   size_t packed_cap = 0;
   bool packed_pinned = false;
-  HostScratch scratch;     // sort keys (2x) and per-cell moments of build_host_tree
+  HostScratch scratch;     // Morton keys, sort elements (2x) and per-cell moments of build_host_tree
 };
 
 // Host builder (tc_build.cpp).  pos [n,3], mass [n] host fp32.  Allocates/reuses
