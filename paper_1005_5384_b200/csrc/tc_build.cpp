@@ -52,7 +52,7 @@ struct SortPlan {
 inline SortPlan sort_plan(int64_t n) {
   // a prefix of 11 levels is enough up to a few million particles; deeper trees want a longer one (fewer cells
   // finished by the comparison sort: 33 vs 40 ms at N = 2^24), as far as the index still fits beside it
-  const int bits = n <= (int64_t(1) << 22) ? 11 : n <= (int64_t(1) << 25) ? 13 : n <= (int64_t(1) << 28) ? 12 : 11;
+  const int bits = (n > (int64_t(1) << 22) && n <= (int64_t(1) << 25)) ? 13 : 11;   // 13 levels leave 25 index bits
   SortPlan P;
   P.bits = bits; P.low = 63 - 3 * bits; P.idxb = 64 - 3 * bits; P.imask = (uint64_t(1) << P.idxb) - 1;
   return P;
@@ -178,7 +178,6 @@ uint64_t* radix_sort(const SortPlan& P, uint64_t* a, uint64_t* tmp, int64_t n, u
   // 5 passes 2.6 ms); the longer prefixes of large N are memory-bound per pass, so 3 passes (23 vs 31 ms at 2^24)
   switch (P.bits) {
     case 13: return radix_sort_t<13, 3>(a, tmp, n, key_or, n_leaf, fullkey);
-    case 12: return radix_sort_t<12, 3>(a, tmp, n, key_or, n_leaf, fullkey);
     default: return radix_sort_t<11, 4>(a, tmp, n, key_or, n_leaf, fullkey);
   }
 }

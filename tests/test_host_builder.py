@@ -120,3 +120,34 @@ def test_far_outlier_takes_the_lopsided_sort_path():
     pos = (1e-3 * rng.standard_normal((n, 3))).astype(np.float32)
     pos[123] = (100.0, 100.0, 100.0)
     _compare(pos, np.full(n, 1.0 / n, np.float32), 16, 64)
+
+
+def test_sort_with_the_13_level_prefix_above_4m_particles():
+    """N just above 2^22 takes the sort plan of the large runs (13-level prefix, 25 index bits, 3 passes;
+    csrc/tc_build.cpp::sort_plan).  Checked against the oracle's tree without the per-cell Python loops of
+    `_compare`: same cell / leaf / group counts and depth, and the same leaves — (first, count) of every leaf
+    in Morton order and, leaf by leaf, the same member set."""
+    n = (1 << 22) + 1237
+    pos, mass = inputs.plummer(n, 77)
+    with B.TreeCode(host_only=True, n_group=64) as tc:
+        tc.set_particles(pos, mass)
+        tc.build(16)
+        s, tr = tc.stats(), tc.tree()
+    o = Oracle(pos, mass, 16, 64)
+    assert (s["n_cells"], s["n_leaves"], s["n_groups"], s["depth"]) == (o.n_cells, o.n_leaves, o.n_groups, o.depth)
+    oc = o.cells()
+
+    def leaves(begin, count, perm):
+        order = np.argsort(begin, kind="stable")
+        b, c = begin[order].astype(np.int64), count[order].astype(np.int64)
+        assert np.array_equal(np.concatenate([[0], np.cumsum(c)[:-1]]), b) and c.sum() == n   # a partition of [0, n)
+        leaf_id = np.repeat(np.arange(len(b)), c)
+        return b, c, perm[np.lexsort((perm, leaf_id))]          # members sorted inside every leaf
+
+    link = tr["link"]
+    is_leaf = link[:, 1] == 0
+    lb, lc, lp = leaves(link[is_leaf, 2], link[is_leaf, 3], np.asarray(tr["perm"]).astype(np.int64))
+    m = oc["n_child"] == 0
+    ob, on, op = leaves(oc["begin"][m], oc["count"][m], np.asarray(o.perm()).astype(np.int64))
+    assert np.array_equal(lb, ob) and np.array_equal(lc, on)
+    assert np.array_equal(lp, op)
