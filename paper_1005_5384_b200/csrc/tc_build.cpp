@@ -248,10 +248,17 @@ int build_host_tree(const float* pos, const float* mass, int64_t n, int n_leaf, 
   // ---- O2: breadth-first split of sorted key ranges
   // cell arrays (struct of vectors), breadth-first, children contiguous
   std::vector<int32_t>&c_begin = T.scratch.c_begin, &c_count = T.scratch.c_count, &c_first_child = T.scratch.c_first_child,
-                      &c_nchild = T.scratch.c_nchild;   // capacity survives between builds
-  c_begin.clear(); c_count.clear(); c_first_child.clear(); c_nchild.clear();
+                      &c_nchild = T.scratch.c_nchild;
+  // their SIZE is a high-water mark that survives between builds (a rebuild of the same problem fills nothing in again);
+  // the cells of this build are [0, lvl_e), and every one of them is written below
+  const auto grow_cells = [&](size_t need) {
+    if (c_begin.size() >= need) return;
+    const size_t to = std::max(need, c_begin.size() + c_begin.size() / 2);
+    c_begin.resize(to); c_count.resize(to); c_first_child.resize(to); c_nchild.resize(to);
+  };
+  grow_cells(1);
   std::vector<int64_t> level_start;  // first cell id of every level (+ end sentinel)
-  c_begin.push_back(0); c_count.push_back((int32_t)n); c_first_child.push_back(-1); c_nchild.push_back(0);
+  c_begin[0] = 0; c_count[0] = (int32_t)n; c_first_child[0] = -1; c_nchild[0] = 0;
   level_start.push_back(0);
   int64_t lvl_b = 0, lvl_e = 1;
   int level = 0;
@@ -294,13 +301,12 @@ int build_host_tree(const float* pos, const float* mass, int64_t n, int n_leaf, 
     if (total == 0) break;
     if (lvl_e + total > (int64_t)0x0fffffff) { msg = "build: more than 2^28 cells"; return TC_EINVAL; }
     const int64_t new_e = lvl_e + total;
-    c_begin.resize((size_t)new_e); c_count.resize((size_t)new_e);
-    c_first_child.resize((size_t)new_e, -1); c_nchild.resize((size_t)new_e, 0);
+    grow_cells((size_t)new_e);
     // pass 2: create the children
 #pragma omp parallel for schedule(dynamic, 256)
     for (int64_t c = lvl_b; c < lvl_e; c++) {
       const int32_t k = nch[(size_t)(c - lvl_b) + 1] - nch[(size_t)(c - lvl_b)];
-      if (k == 0) continue;
+      if (k == 0) { c_first_child[c] = -1; c_nchild[c] = 0; continue; }   // leaf
       const int64_t first = lvl_e + nch[(size_t)(c - lvl_b)];
       c_first_child[c] = (int32_t)first; c_nchild[c] = k;
       const int32_t* bd = bnds + 9 * (size_t)(c - lvl_b);
@@ -308,7 +314,9 @@ int build_host_tree(const float* pos, const float* mass, int64_t n, int n_leaf, 
     }
     lvl_b = lvl_e; lvl_e = new_e; level++;
   }
-  const int64_t nc = (int64_t)c_begin.size();
+  // the last level was not expanded: all of its cells are leaves
+  for (int64_t c = lvl_b; c < lvl_e; c++) { c_first_child[c] = -1; c_nchild[c] = 0; }
+  const int64_t nc = lvl_e;
   T.n_cells = nc;
   T.depth = (int32_t)level_start.size() - 2;
   const int n_levels = (int)level_start.size() - 1;

@@ -151,3 +151,27 @@ def test_sort_with_the_13_level_prefix_above_4m_particles():
     ob, on, op = leaves(oc["begin"][m], oc["count"][m], np.asarray(o.perm()).astype(np.int64))
     assert np.array_equal(lb, ob) and np.array_equal(lc, on)
     assert np.array_equal(lp, op)
+
+
+def test_rebuilds_in_one_context_equal_fresh_contexts():
+    """The builder's per-cell arrays and sort buffers live in the context between builds and are not cleared
+    (csrc/tc_build.cpp): a big problem, then smaller and differently shaped ones in the SAME context must give,
+    array for array, the tree a fresh context builds."""
+    cases = [(inputs.plummer(40000, 51), 16, 64), (inputs.uniform_cube(3000, 52), 4, 16), (inputs.plummer(700, 53), 1, 1),
+             (inputs.plummer(25000, 54), 8, 96), (inputs.uniform_cube(9000, 55), 16, 64)]
+    with B.TreeCode(host_only=True) as reused:
+        for (pos, mass), n_leaf, n_group in cases:
+            reused.set_option("n_group", n_group)
+            reused.set_particles(pos, mass)
+            reused.build(n_leaf)
+            s1, t1, g1 = reused.stats(), reused.tree(), B.tc_get_group_boxes(reused.ctx)
+            with B.TreeCode(host_only=True, n_group=n_group) as fresh:
+                fresh.set_particles(pos, mass)
+                fresh.build(n_leaf)
+                s2, t2, g2 = fresh.stats(), fresh.tree(), B.tc_get_group_boxes(fresh.ctx)
+            for k in ("n_cells", "n_leaves", "n_groups", "depth"):
+                assert s1[k] == s2[k]
+            assert t1.keys() == t2.keys()
+            for k in t1:
+                assert np.array_equal(np.asarray(t1[k]), np.asarray(t2[k])), k
+            assert np.array_equal(g1, g2)
