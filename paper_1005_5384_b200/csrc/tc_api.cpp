@@ -32,7 +32,8 @@ struct tc_ctx {
   tc::TwoPassScratch tps;
   bool last_two_pass = false;
   // particles (host copy, caller order)
-  std::vector<float> pos, mass;
+  std::vector<float4> xyzm;                 // the context's host copy of the particles: (x, y, z, m), caller's order
+  std::vector<float> pos, mass;             // staging of DEVICE inputs on their way into xyzm
   int64_t n = 0;
   // tree
   tc::HostTree tree;
@@ -134,15 +135,9 @@ int ensure_host_particles(tc_ctx* c) {
   if (c->host_particles_valid) return TC_OK;
   if (!c->src_valid) return fail(c, TC_ESTATE, "no particles");
   const int64_t n = c->n;
-  std::vector<float4> h;
-  try { h.resize((size_t)n); c->pos.resize((size_t)n * 3); c->mass.resize((size_t)n); } catch (...) { return fail(c, TC_ENOMEM, "out of host memory"); }
-  TC_CUDA(c, cudaMemcpyAsync(h.data(), c->d_src, sizeof(float4) * (size_t)n, cudaMemcpyDeviceToHost, c->stream));
+  try { c->xyzm.resize((size_t)n); } catch (...) { return fail(c, TC_ENOMEM, "out of host memory"); }
+  TC_CUDA(c, cudaMemcpyAsync(c->xyzm.data(), c->d_src, sizeof(float4) * (size_t)n, cudaMemcpyDeviceToHost, c->stream));
   TC_CUDA(c, cudaStreamSynchronize(c->stream));
-#pragma omp parallel for schedule(static)
-  for (int64_t i = 0; i < n; i++) {
-    c->pos[3 * (size_t)i] = h[(size_t)i].x; c->pos[3 * (size_t)i + 1] = h[(size_t)i].y; c->pos[3 * (size_t)i + 2] = h[(size_t)i].z;
-    c->mass[(size_t)i] = h[(size_t)i].w;
-  }
   c->host_particles_valid = true;
   return TC_OK;
 }
@@ -157,12 +152,7 @@ int ensure_src(tc_ctx* c) {
     TC_CUDA(c, cudaMalloc((void**)&c->d_src, sizeof(float4) * (size_t)n));
     c->src_cap = n;
   }
-  std::vector<float4> h;
-  try { h.resize((size_t)n); } catch (...) { return fail(c, TC_ENOMEM, "out of host memory"); }
-  const float* P = c->pos.data(); const float* M = c->mass.data();
-#pragma omp parallel for schedule(static)
-  for (int64_t i = 0; i < n; i++) h[(size_t)i] = make_float4(P[3 * i], P[3 * i + 1], P[3 * i + 2], M[i]);
-  TC_CUDA(c, cudaMemcpyAsync(c->d_src, h.data(), sizeof(float4) * (size_t)n, cudaMemcpyHostToDevice, c->stream));
+  TC_CUDA(c, cudaMemcpyAsync(c->d_src, c->xyzm.data(), sizeof(float4) * (size_t)n, cudaMemcpyHostToDevice, c->stream));
   TC_CUDA(c, cudaStreamSynchronize(c->stream));
   c->src_valid = true;
   return TC_OK;
@@ -330,7 +320,11 @@ int tc_set_particles(tc_ctx* c, const float* pos, const float* mass, int64_t n) 
     c->n = n;
     return TC_OK;
   }
-  try { c->pos.resize((size_t)n * 3); c->mass.resize((size_t)n); } catch (...) { return fail(c, TC_ENOMEM, "tc_set_particles: out of host memory"); }
+  try {
+    c->xyzm.resize((size_t)n);
+    if (pos_dev) c->pos.resize((size_t)n * 3);
+    if (mass_dev) c->mass.resize((size_t)n);
+  } catch (...) { return fail(c, TC_ENOMEM, "tc_set_particles: out of host memory"); }
   const float* P = pos; const float* M = mass;      // where the validation pass reads from
   if (pos_dev) { TC_CUDA(c, cudaMemcpyAsync(c->pos.data(), pos, sizeof(float) * 3 * (size_t)n, cudaMemcpyDeviceToHost, c->stream)); P = c->pos.data(); }
   if (mass_dev) { TC_CUDA(c, cudaMemcpyAsync(c->mass.data(), mass, sizeof(float) * (size_t)n, cudaMemcpyDeviceToHost, c->stream)); M = c->mass.data(); }
@@ -343,12 +337,12 @@ int tc_set_particles(tc_ctx* c, const float* pos, const float* mass, int64_t n) 
   }
   // one pass: copy into the context, validate, and (device build) stage (x,y,z,m) in pinned memory
   bool bad_pos = false, bad_mass = false;
-  float* CP = c->pos.data(); float* CM = c->mass.data();
+  float4* X4 = c->xyzm.data();
   float4* H = dev_mode ? c->h_src : nullptr;
 #pragma omp parallel for schedule(static) reduction(| : bad_pos, bad_mass)
   for (int64_t i = 0; i < n; i++) {
     const float x = P[3 * i], y = P[3 * i + 1], z = P[3 * i + 2], m = M[i];
-    CP[3 * i] = x; CP[3 * i + 1] = y; CP[3 * i + 2] = z; CM[i] = m;
+    X4[i] = make_float4(x, y, z, m);
     if (H) H[i] = make_float4(x, y, z, m);
     bad_pos |= !(std::isfinite(x) && std::isfinite(y) && std::isfinite(z));
     bad_mass |= !(std::isfinite(m) && m >= 0.f);
@@ -389,7 +383,7 @@ int tc_build(tc_ctx* c, int n_leaf) {
   { const int rc0 = ensure_host_particles(c); if (rc0 != TC_OK) return rc0; }
   const double t0 = now_ms();
   std::string msg;
-  const int rc = tc::build_host_tree(c->pos.data(), c->mass.data(), c->n, n_leaf, c->n_group, c->tree, packed_alloc, c, msg);
+  const int rc = tc::build_host_tree(c->xyzm.data(), c->n, n_leaf, c->n_group, c->tree, packed_alloc, c, msg);
   if (rc != TC_OK) return fail(c, rc, msg);
   const double t1 = now_ms();
   const tc::HostTree& T = c->tree;

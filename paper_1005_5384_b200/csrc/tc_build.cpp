@@ -67,7 +67,7 @@ inline SortPlan sort_plan(int64_t n) {
   for (int64_t i = 0; i < n; i++) {                                                                 \
     uint64_t g[3];                                                                                  \
     for (int k = 0; k < 3; k++) {                                                                   \
-      double v = std::floor(((double)pos[3 * i + k] - org[k]) * scale);                             \
+      double v = std::floor(((double)pos[4 * i + k] - org[k]) * scale);                             \
       v = std::min(std::max(v, 0.0), gmax);                                                         \
       g[k] = (uint64_t)v;                                                                           \
     }                                                                                               \
@@ -78,7 +78,7 @@ inline SortPlan sort_plan(int64_t n) {
   }                                                                                                 \
   return key_or;
 
-uint64_t compute_keys_base(const float* pos, int64_t n, const double* org, double scale, double gmax, uint64_t* fullkey,
+uint64_t compute_keys_base(const float* pos /* (x,y,z,m) per particle */, int64_t n, const double* org, double scale, double gmax, uint64_t* fullkey,
                            uint64_t* elem, int low, int idxb) {
   TC_KEYS_BODY(spread21)
 }
@@ -202,7 +202,7 @@ void* HostScratch::get(int k, size_t bytes) {
 }
 HostScratch::~HostScratch() { for (void* p : buf) std::free(p); }
 
-int build_host_tree(const float* pos, const float* mass, int64_t n, int n_leaf, int n_group,
+int build_host_tree(const float4* xyzm, int64_t n, int n_leaf, int n_group,
                     HostTree& T, PackedAlloc alloc, void* alloc_user, std::string& msg) {
   if (n < 1 || n_leaf < 1 || n_group < 1) { msg = "build: n, n_leaf, n_group must be >= 1"; return TC_EINVAL; }
   T.n = n; T.n_leaf = n_leaf; T.n_group = n_group;
@@ -217,7 +217,7 @@ int build_host_tree(const float* pos, const float* mass, int64_t n, int n_leaf, 
     double l0 = lo[0], l1 = lo[1], l2 = lo[2], h0 = hi[0], h1 = hi[1], h2 = hi[2];
 #pragma omp parallel for schedule(static) reduction(min : l0, l1, l2) reduction(max : h0, h1, h2)
     for (int64_t i = 0; i < n; i++) {
-      const double x = (double)pos[3 * i], y = (double)pos[3 * i + 1], z = (double)pos[3 * i + 2];
+      const double x = (double)xyzm[i].x, y = (double)xyzm[i].y, z = (double)xyzm[i].z;
       l0 = std::min(l0, x); h0 = std::max(h0, x);
       l1 = std::min(l1, y); h1 = std::max(h1, y);
       l2 = std::min(l2, z); h2 = std::max(h2, z);
@@ -240,7 +240,7 @@ int build_host_tree(const float* pos, const float* mass, int64_t n, int n_leaf, 
   uint64_t* const fullkey = static_cast<uint64_t*>(T.scratch.get(0, sizeof(uint64_t) * (size_t)n));   // caller's order
   uint64_t* keys = static_cast<uint64_t*>(T.scratch.get(1, sizeof(uint64_t) * 2 * (size_t)n));        // elements, and their twin
   if (!fullkey || !keys) { msg = "build: out of host memory"; return TC_ENOMEM; }
-  const uint64_t key_or = compute_keys(pos, n, org, scale, gmax, fullkey, keys, SP.low, SP.idxb);
+  const uint64_t key_or = compute_keys(reinterpret_cast<const float*>(xyzm), n, org, scale, gmax, fullkey, keys, SP.low, SP.idxb);
   lap("keys");
   keys = radix_sort(SP, keys, keys + n, n, key_or, n_leaf, fullkey);
   lap("sort");
@@ -364,7 +364,7 @@ int build_host_tree(const float* pos, const float* mass, int64_t n, int n_leaf, 
 #pragma omp parallel for schedule(static)
   for (int64_t t = 0; t < n; t++) {
     const int64_t i = (int64_t)(keys[t] & SP.imask);
-    part[t] = make_float4(pos[3 * i], pos[3 * i + 1], pos[3 * i + 2], mass[i]);
+    part[t] = xyzm[i];                       // one aligned 16-byte read per particle
     orig[t] = (int32_t)i;
   }
   lap("gather");

@@ -62,11 +62,11 @@ struct HostTree {
   HostScratch scratch;     // Morton keys, sort elements (2x) and per-cell moments of build_host_tree
 };
 
-// Host builder (tc_build.cpp).  pos [n,3], mass [n] host fp32.  Allocates/reuses
+// Host builder (tc_build.cpp).  xyzm [n] = (x, y, z, m) host fp32, caller's order.  Allocates/reuses
 // T.packed through alloc(bytes) (returns nullptr on failure).  Returns TC_OK or an
 // error code with msg set.
 typedef void* (*PackedAlloc)(void* user, size_t bytes);
-int build_host_tree(const float* pos, const float* mass, int64_t n, int n_leaf, int n_group,
+int build_host_tree(const float4* xyzm, int64_t n, int n_leaf, int n_group,
                     HostTree& T, PackedAlloc alloc, void* alloc_user, std::string& msg);
 
 // Device-side view handed to the kernels (tc_kernels.cu).
