@@ -33,6 +33,8 @@ struct tc_ctx {
   bool last_two_pass = false;
   // particles (host copy, caller order)
   std::vector<float4> xyzm;                 // the context's host copy of the particles: (x, y, z, m), caller's order
+  bool bbox_valid = false;                  // bbox[] = per-axis min (0-2) and max (3-5) of xyzm, taken by the pass that copied it in
+  float bbox[6] = {0, 0, 0, 0, 0, 0};
   std::vector<float> pos, mass;             // staging of DEVICE inputs on their way into xyzm
   int64_t n = 0;
   // tree
@@ -49,7 +51,7 @@ struct tc_ctx {
   bool forces_done = false, timing_pending = false;
   tc::DeviceBuildScratch dscr;
   bool tree_host_valid = false;       // the host copy of the packed tree (tc_get_tree) is current
-  bool host_particles_valid = false;  // pos/mass below hold the current particles (else only d_src does)
+  bool host_particles_valid = false;  // xyzm holds the current particles (else only d_src does)
   float4* h_src = nullptr; int64_t h_src_cap = 0;     // pinned staging of (x,y,z,m) for the device build
   float* d_raw = nullptr; int64_t raw_cap = 0;        // device landing area of PINNED host inputs (pos [3n] | mass [n])
   unsigned int* d_flags = nullptr;
@@ -279,7 +281,7 @@ int tc_set_particles(tc_ctx* c, const float* pos, const float* mass, int64_t n) 
   if (!c) return TC_EINVAL;
   if (!pos || !mass) return fail(c, TC_EINVAL, "tc_set_particles: null pointer");
   if (n < 1 || n > 2147483647LL) return fail(c, TC_EINVAL, "tc_set_particles: n must be in [1, 2^31-1]");
-  c->built = false; c->forces_done = false; c->src_valid = false; c->host_particles_valid = false;
+  c->built = false; c->forces_done = false; c->src_valid = false; c->host_particles_valid = false; c->bbox_valid = false;
   c->n = 0;
   const bool pos_dev = is_device_ptr(c, pos), mass_dev = is_device_ptr(c, mass);
   const bool dev_mode = c->device_build && !c->host_only;
@@ -339,10 +341,13 @@ int tc_set_particles(tc_ctx* c, const float* pos, const float* mass, int64_t n) 
   bool bad_pos = false, bad_mass = false;
   float4* X4 = c->xyzm.data();
   float4* H = dev_mode ? c->h_src : nullptr;
-#pragma omp parallel for schedule(static) reduction(| : bad_pos, bad_mass)
+  // (the per-axis extremes are the first thing tc_build needs: taken here, while the data passes by)
+  float l0 = INFINITY, l1 = INFINITY, l2 = INFINITY, h0 = -INFINITY, h1 = -INFINITY, h2 = -INFINITY;
+#pragma omp parallel for schedule(static) reduction(| : bad_pos, bad_mass) reduction(min : l0, l1, l2) reduction(max : h0, h1, h2)
   for (int64_t i = 0; i < n; i++) {
     const float x = P[3 * i], y = P[3 * i + 1], z = P[3 * i + 2], m = M[i];
     X4[i] = make_float4(x, y, z, m);
+    l0 = std::min(l0, x); h0 = std::max(h0, x); l1 = std::min(l1, y); h1 = std::max(h1, y); l2 = std::min(l2, z); h2 = std::max(h2, z);
     if (H) H[i] = make_float4(x, y, z, m);
     bad_pos |= !(std::isfinite(x) && std::isfinite(y) && std::isfinite(z));
     bad_mass |= !(std::isfinite(m) && m >= 0.f);
@@ -350,6 +355,8 @@ int tc_set_particles(tc_ctx* c, const float* pos, const float* mass, int64_t n) 
   if (bad_pos) return fail(c, TC_EINVAL, "tc_set_particles: non-finite position");
   if (bad_mass) return fail(c, TC_EINVAL, "tc_set_particles: negative or non-finite mass");
   c->host_particles_valid = true;
+  c->bbox[0] = l0; c->bbox[1] = l1; c->bbox[2] = l2; c->bbox[3] = h0; c->bbox[4] = h1; c->bbox[5] = h2;
+  c->bbox_valid = true;
   if (dev_mode) {     // stream-ordered: tc_build runs on the same stream
     TC_CUDA(c, cudaMemcpyAsync(c->d_src, c->h_src, sizeof(float4) * (size_t)n, cudaMemcpyHostToDevice, c->stream));
     c->src_valid = true;
@@ -383,7 +390,8 @@ int tc_build(tc_ctx* c, int n_leaf) {
   { const int rc0 = ensure_host_particles(c); if (rc0 != TC_OK) return rc0; }
   const double t0 = now_ms();
   std::string msg;
-  const int rc = tc::build_host_tree(c->xyzm.data(), c->n, n_leaf, c->n_group, c->tree, packed_alloc, c, msg);
+  const int rc = tc::build_host_tree(c->xyzm.data(), c->n, n_leaf, c->n_group, c->tree, packed_alloc, c, msg,
+                                     c->bbox_valid ? c->bbox : nullptr);
   if (rc != TC_OK) return fail(c, rc, msg);
   const double t1 = now_ms();
   const tc::HostTree& T = c->tree;

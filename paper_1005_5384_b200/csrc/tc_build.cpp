@@ -203,7 +203,7 @@ void* HostScratch::get(int k, size_t bytes) {
 HostScratch::~HostScratch() { for (void* p : buf) std::free(p); }
 
 int build_host_tree(const float4* xyzm, int64_t n, int n_leaf, int n_group,
-                    HostTree& T, PackedAlloc alloc, void* alloc_user, std::string& msg) {
+                    HostTree& T, PackedAlloc alloc, void* alloc_user, std::string& msg, const float* bbox6) {
   if (n < 1 || n_leaf < 1 || n_group < 1) { msg = "build: n, n_leaf, n_group must be >= 1"; return TC_EINVAL; }
   T.n = n; T.n_leaf = n_leaf; T.n_group = n_group;
   const bool timing = std::getenv("TC_BUILD_TIMING") != nullptr;
@@ -213,7 +213,9 @@ int build_host_tree(const float4* xyzm, int64_t n, int n_leaf, int n_group,
   // ---- O1: root cube and integer grid ("a cube containing all particles")
   double lo[3], hi[3];
   for (int k = 0; k < 3; k++) { lo[k] = std::numeric_limits<double>::infinity(); hi[k] = -lo[k]; }
-  {
+  if (bbox6) {
+    for (int k = 0; k < 3; k++) { lo[k] = (double)bbox6[k]; hi[k] = (double)bbox6[3 + k]; }
+  } else {
     double l0 = lo[0], l1 = lo[1], l2 = lo[2], h0 = hi[0], h1 = hi[1], h2 = hi[2];
 #pragma omp parallel for schedule(static) reduction(min : l0, l1, l2) reduction(max : h0, h1, h2)
     for (int64_t i = 0; i < n; i++) {

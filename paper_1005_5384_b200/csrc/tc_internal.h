@@ -67,7 +67,8 @@ struct HostTree {
 // error code with msg set.
 typedef void* (*PackedAlloc)(void* user, size_t bytes);
 int build_host_tree(const float4* xyzm, int64_t n, int n_leaf, int n_group,
-                    HostTree& T, PackedAlloc alloc, void* alloc_user, std::string& msg);
+                    HostTree& T, PackedAlloc alloc, void* alloc_user, std::string& msg,
+                    const float* bbox6 = nullptr /* per-axis min (0-2), max (3-5) of xyzm if the caller has them */);
 
 // Device-side view handed to the kernels (tc_kernels.cu).
 struct DeviceTree {
