@@ -58,7 +58,8 @@ typedef struct tc_stats {
   int64_t n_pc_total;     /* sum over particles of particle-cell interactions of
                              the last tc_forces                                   */
   int64_t n_pp_total;     /* same, particle-particle (self excluded)              */
-  int64_t n_tests_total;  /* opening tests of the last tc_forces (sum over groups)*/
+  int64_t n_tests_total;  /* opening tests EXECUTED by the last tc_forces: one walk per group; only a group of more
+                             than 128 particles (N_group > 128, or a level-21 leaf of coincident particles) is walked once per 128 */
   int64_t n_spills;       /* walk-stack spills to global memory (last tc_forces)  */
   double t_host_ms;       /* last tc_build: host tree + moments + pack            */
   double t_copy_ms;       /* last tc_build: bulk host->device copy (wall)         */

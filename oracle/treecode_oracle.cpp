@@ -20,6 +20,10 @@
 //    tree        : brute-force cell enumeration from the definition; invariants
 //    moments     : parallel-axis merge of children; tracelessness; COM in bbox
 //    quadrupole  : closed form, two masses at +-s (tests/golden/quadrupole_two_mass.txt)
+//    softened quadrupole (R11, sigma^2 = r^2 + eps^2 in the s^-5 and s^-7 terms too): hand-evaluated values at
+//                  eps = 0.375, 0.5 and 0.1 with Q != 0, on and off axis
+//                  (tests/golden/quadrupole_two_mass_softened.txt), and a = -grad(phi) of the same cell term by
+//                  central differences at eps = 0, 0.1, 0.5
 //    walk        : coverage invariant; theta = 0; brute force over all (group, cell) pairs
 //    evaluation  : N = 2 closed form; theta = 0 == direct sum; theta -> 0 convergence;
 //                  momentum invariant; Plummer analytic field

@@ -13,7 +13,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libtc_b200.so")
 SOURCES = ["tc_api.cpp", "tc_build.cpp", "tc_kernels.cu", "tc_build_gpu.cu"]
-HEADERS = ["tc_internal.h", os.path.join("..", "..", "include", "tc.h")]
+HEADERS = ["tc_internal.h", "tc_lanes.h", os.path.join("..", "..", "include", "tc.h")]
 
 NVCC_FLAGS = [
     "-std=c++17", "-O3", "-lineinfo",

@@ -25,6 +25,7 @@
 #endif
 
 #include "tc_internal.h"
+#include "tc_lanes.h"
 
 namespace tc {
 namespace {
@@ -479,30 +480,18 @@ int build_host_tree(const float4* xyzm, int64_t n, int n_leaf, int n_group,
   lap("pack");
   // Schedule (grp[i].w = i-th group to run): the persistent kernel hands groups out through an
   // atomic counter, so costly groups go first and the tail of the launch is made of cheap ones.
-  // Cost model = issue slots per list entry of the kernel's lane mapping (tc_kernels.cu): a pass
-  // over m <= 64 particles costs min_S ceil(m / (2 floor(32/S))) / S (particle pairs per lane / slices).  Stable: Morton order inside a
-  // cost class keeps neighbouring groups together.
+  // Cost model = issue slots per list entry of the kernel's lane mapping: tc_lanes.h, the table the kernel
+  // itself reads.  Stable: Morton order inside a cost class keeps neighbouring groups together.
   {
-    constexpr int kPass = 64, kMaxKP = 3;        // mirror of tc_kernels.cu
-    double pass_cost[kPass + 1];
-    for (int m = 0; m <= kPass; m++) {
-      double best = 1e30;
-      for (int sl = 1; sl <= 32; sl++) {
-        const int q = 32 / sl, kp = (m + 2 * q - 1) / (2 * q);                     // pairs of particles per lane
-        if (kp >= 1 && kp <= kMaxKP) best = std::min(best, (double)kp / sl);
-      }
-      pass_cost[m] = (m == 0) ? 0.0 : best;
-    }
-    // counting sort by cost class (cost in 1/960 units: every kp / S with S <= 32 is a multiple of it
-    // up to rounding), descending; stable, so Morton order survives inside a class
+    static constexpr LaneTable lanes = LaneTable();
+    // counting sort by cost class, descending; stable, so Morton order survives inside a class
     const size_t ng = groups.size();
     std::vector<int32_t> cls(ng);
     int32_t cmax = 0;
 #pragma omp parallel for schedule(static) reduction(max : cmax)
     for (size_t g = 0; g < ng; g++) {
       const int64_t cnt = c_count[groups[g]];
-      const double cost = (double)(cnt / kPass) * pass_cost[kPass] + pass_cost[cnt % kPass];
-      cls[g] = (int32_t)std::min(cost * 960.0 + 0.5, 1.0e6);
+      cls[g] = group_cost_class(lanes, cnt);
       cmax = std::max(cmax, cls[g]);
     }
     std::vector<int32_t> start((size_t)cmax + 2, 0);

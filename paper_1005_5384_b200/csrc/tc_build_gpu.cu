@@ -29,6 +29,7 @@
 #include <vector>
 
 #include "tc_internal.h"
+#include "tc_lanes.h"
 
 namespace tc {
 namespace {
@@ -269,17 +270,15 @@ __global__ void k_pack_particles(const float4* __restrict__ src, const unsigned 
 }
 
 // group records: key for the Morton order = first body; cost class for the schedule
+__constant__ LaneTable c_lanes_build = LaneTable();   // the kernel's lane mapping (tc_lanes.h): cost model of the schedule
 __global__ void k_group_keys(const int* __restrict__ gcell, int ng, const int* __restrict__ c_begin, const int* __restrict__ c_count,
-                             unsigned int* __restrict__ first_body, unsigned int* __restrict__ cls_key,
-                             const float* __restrict__ pass_cost, int k_pass) {
+                             unsigned int* __restrict__ first_body, unsigned int* __restrict__ cls_key) {
   const int g = blockIdx.x * blockDim.x + threadIdx.x;
   if (g >= ng) return;
   const int c = gcell[g];
   first_body[g] = (unsigned int)c_begin[c];
   const int cnt = c_count[c];
-  const double cost = (double)(cnt / k_pass) * (double)pass_cost[k_pass] + (double)pass_cost[cnt % k_pass];
-  const unsigned int cls = (unsigned int)fmin(cost * 960.0 + 0.5, 1.0e6);
-  cls_key[g] = 1000000u - cls;        // ascending key = descending cost
+  cls_key[g] = (unsigned int)(kMaxCostClass - group_cost_class(c_lanes_build, cnt));   // ascending key = descending cost
 }
 
 __global__ void k_iota(unsigned int* a, int n) {
@@ -345,7 +344,7 @@ static int grow(T*& p, size_t& cap, size_t need, bool keep, cudaStream_t st, std
 
 void DeviceBuildScratch::release() {
   void* ptrs[] = {keys, keys_alt, idx, idx_alt, cub_tmp, c_begin, c_count, c_first, c_nchild, c_parent, nch, off, mom,
-                  is_group, gcell, gcell_sorted, gkey, gkey_alt, gval, gval_alt, boxes, small, link, q6, pass_cost, bounds};
+                  is_group, gcell, gcell_sorted, gkey, gkey_alt, gval, gval_alt, boxes, small, link, q6, bounds};
   for (void* p : ptrs) cudaFree(p);
   *this = DeviceBuildScratch();
 }
@@ -477,23 +476,9 @@ int build_device_tree(const float4* src, int64_t n, int n_leaf, int n_group, Dev
   TCG_GROW(S.gkey, S.cap_gkey, ng, false); TCG_GROW(S.gkey_alt, S.cap_gkeya, ng, false);
   TCG_GROW(S.gval, S.cap_gval, ng, false); TCG_GROW(S.gval_alt, S.cap_gvala, ng, false);
   TCG_GROW(S.gcell_sorted, S.cap_gcells, ng, false);
-  // cost model of the kernel's lane mapping: mirror of tc_build.cpp / tc_kernels.cu
-  constexpr int kPass = 64, kMaxKP = 3;
-  float pass_cost[kPass + 1];
-  for (int m = 0; m <= kPass; m++) {
-    double best = 1e30;
-    for (int sl = 1; sl <= 32; sl++) {
-      const int q = 32 / sl, kp = (m + 2 * q - 1) / (2 * q);
-      if (kp >= 1 && kp <= kMaxKP) best = std::min(best, (double)kp / sl);
-    }
-    pass_cost[m] = (m == 0) ? 0.f : (float)best;
-  }
-  TCG_GROW(S.pass_cost, S.cap_pc, kPass + 1, false);
-  TCG_CUDA(cudaMemcpyAsync(S.pass_cost, pass_cost, sizeof(pass_cost), cudaMemcpyHostToDevice, st));
-  TCG_CUDA(cudaStreamSynchronize(st));       // pass_cost is a stack array
   {
     // (1) sort the group cells by first body: keys = first body, values = cell id
-    k_group_keys<<<blocks(ng), 256, 0, st>>>(S.gcell, (int)ng, S.c_begin, S.c_count, S.gkey, S.gval, S.pass_cost, kPass);
+    k_group_keys<<<blocks(ng), 256, 0, st>>>(S.gcell, (int)ng, S.c_begin, S.c_count, S.gkey, S.gval);
     cub::DoubleBuffer<unsigned int> kb(S.gkey, S.gkey_alt);
     cub::DoubleBuffer<int> vb(S.gcell, S.gcell_sorted);
     size_t need = 0;
@@ -503,7 +488,7 @@ int build_device_tree(const float4* src, int64_t n, int n_leaf, int n_group, Dev
     if (vb.Current() != S.gcell_sorted) { std::swap(S.gcell, S.gcell_sorted); std::swap(S.cap_gcell, S.cap_gcells); }
     if (kb.Current() != S.gkey) { std::swap(S.gkey, S.gkey_alt); std::swap(S.cap_gkey, S.cap_gkeya); }
     // (2) schedule: stable sort of the Morton-ordered group indices by descending cost class
-    k_group_keys<<<blocks(ng), 256, 0, st>>>(S.gcell_sorted, (int)ng, S.c_begin, S.c_count, S.gkey_alt, S.gkey, S.pass_cost, kPass);
+    k_group_keys<<<blocks(ng), 256, 0, st>>>(S.gcell_sorted, (int)ng, S.c_begin, S.c_count, S.gkey_alt, S.gkey);
     k_iota<<<blocks(ng), 256, 0, st>>>(S.gval, (int)ng);
     cub::DoubleBuffer<unsigned int> kb2(S.gkey, S.gkey_alt);
     cub::DoubleBuffer<unsigned int> vb2(S.gval, S.gval_alt);

@@ -148,7 +148,6 @@ struct DeviceBuildScratch {
   unsigned int* small = nullptr;                             size_t cap_small = 0;   // counters
   int4* link = nullptr;                                      size_t cap_link = 0;    // tc_get_tree
   float* q6 = nullptr;                                       size_t cap_q6 = 0;      // tc_get_tree
-  float* pass_cost = nullptr;                                size_t cap_pc = 0;
   void release();
 };
 

@@ -15,13 +15,14 @@
 //   * a chunk is evaluated as soon as it fills (FP32 FMA + one rsqrt.approx per
 //     interaction), so no interaction list ever reaches global memory and there is
 //     no count pass, no host scan, no second walk;
-//   * lanes map to (list slice s, particle column p): a pass over m <= 64 particles
-//     picks S slices of q = floor(32/S) columns and kp = ceil(m / 2q) <= 3 particle
-//     PAIRS per lane so that kp/S is minimal; every list record is loaded from shared
-//     memory once per lane and applied to the lane's pairs with packed FP32
-//     instructions (FFMA2/FMUL2/FADD2: two particles per instruction), slices are
-//     reduced with shuffles at the end — the fix for the paper's 30 % thread
-//     utilisation.
+//   * lanes map to (list slice s, particle column p): a pass over m <= kPassCap particles
+//     (ONE walk per group) picks S slices of q = floor(32/S) columns and
+//     K = ceil(m / q) <= kMaxK particles per lane so that the issue slots per list entry
+//     are minimal (tc_lanes.h); every list record is loaded from shared memory once per
+//     lane and applied to the lane's particles: floor(K/2) PAIRS with packed FP32
+//     instructions (FFMA2/FMUL2/FADD2: two particles per instruction) and, when K is
+//     odd, one more particle with scalar instructions; slices are reduced with shuffles
+//     at the end — the fix for the paper's 30 % thread utilisation.
 // No tensor cores: this is not a dense contraction.
 #include <cuda_runtime.h>
 
@@ -31,18 +32,23 @@
 #include <cstdint>
 
 #include "tc_internal.h"
+#include "tc_lanes.h"
 
 namespace tc {
 namespace {
 
-#ifndef TC_MAXKP
-#define TC_MAXKP 3
-#endif
 #ifndef TC_MINB
 #define TC_MINB 4
 #endif
+#ifndef TC_WALKB
+#define TC_WALKB 2
+#endif
+constexpr int kWalkB = TC_WALKB;   // batches of 4 nodes (32 child tests) per walk iteration
+#ifndef TC_UNROLL2_MAXK
+#define TC_UNROLL2_MAXK 2   // particle-cell loop: two records in flight up to this many particles per lane
+#endif
 #ifndef TC_CELLCAP
-#define TC_CELLCAP 192
+#define TC_CELLCAP 224
 #endif
 #ifndef TC_WARPS
 #define TC_WARPS 4
@@ -57,11 +63,7 @@ constexpr int kLeafQCap = TC_LEAFQCAP;   // opened-leaf ranges queued per warp
 #define TC_BODYCAP 384
 #endif
 constexpr int kBodyCap = TC_BODYCAP;   // bodies staged per warp per evaluation round
-constexpr int kMaxKP = TC_MAXKP; // particle PAIRS per lane (packed f32x2 arithmetic)
-// Particles of a group handled per walk.  64 * kMaxKP would fit, but splitting a larger group into
-// passes of 64 keeps the lanes fuller (96 = 64 + 32 costs 1 + 1/2 pair-slots, one pass of 96 costs 2)
-// and measured faster although the tree is walked once per pass.
-constexpr int kPass = 64;
+constexpr int kMaxKP = kMaxK / 2;  // particle PAIRS per lane (packed f32x2 arithmetic); an odd K adds one scalar particle
 constexpr unsigned kFull = 0xffffffffu;
 
 struct __align__(16) CellRec {   // one un-opened cell: 48 bytes
@@ -86,24 +88,8 @@ struct __align__(16) WarpSmem {
   uint32_t stack[STK];           // nodes to expand: first_child << 3 | (n_child - 1)
 };
 
-// Lane mapping table: for m particles in a pass the slice count S that minimises
-// kp / S with kp = ceil(m / (2 floor(32 / S))) <= kMaxKP particle pairs per lane (ties: fewer pairs).
-struct SliceTable {
-  unsigned char S[kPass + 1];
-  constexpr SliceTable() : S{} {
-    for (int m = 0; m <= kPass; m++) {
-      int bestS = 1, bestK = 64;
-      for (int s = 1; s <= 32; s++) {
-        const int q = 32 / s;
-        const int k = (m + 2 * q - 1) / (2 * q);
-        if (k < 1 || k > kMaxKP) continue;
-        if (k * bestS < bestK * s) { bestS = s; bestK = k; }   // k/s < bestK/bestS
-      }
-      S[m] = (unsigned char)bestS;
-    }
-  }
-};
-__constant__ SliceTable c_slices = SliceTable();
+// Lane mapping of a pass over m particles (tc_lanes.h): S slices x q columns, K particles per lane
+__constant__ LaneTable c_lanes = LaneTable();
 
 __device__ __forceinline__ float rsqrt_approx(float x) {
   float y;
@@ -114,21 +100,39 @@ __device__ __forceinline__ float rsqrt_approx(float x) {
 // ---- packed FP32 pairs (sm_100a FFMA2 / FMUL2 / FADD2): one instruction does the arithmetic of
 // the lane's TWO particles (lo = even, hi = odd) at half the issue cost of two scalar instructions.
 // A scalar operand (a field of the list record) is broadcast by the hardware (`R.F32` operand form).
+#ifdef TC_VOLATILE_MATH
+#define TC_ASMV volatile
+#else
+#define TC_ASMV
+#endif
 typedef unsigned long long f2;
 __device__ __forceinline__ f2 pk(float lo, float hi) { f2 r; asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(lo), "f"(hi)); return r; }
 __device__ __forceinline__ f2 bc(float x) { return pk(x, x); }
 __device__ __forceinline__ float lo(f2 v) { float a; asm("{ .reg .b32 t; mov.b64 {%0, t}, %1; }" : "=f"(a) : "l"(v)); return a; }
 __device__ __forceinline__ float hi(f2 v) { float b; asm("{ .reg .b32 t; mov.b64 {t, %0}, %1; }" : "=f"(b) : "l"(v)); return b; }
-__device__ __forceinline__ f2 add2(f2 a, f2 b) { f2 d; asm("add.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b)); return d; }
-__device__ __forceinline__ f2 sub2(f2 a, f2 b) { f2 d; asm("sub.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b)); return d; }
-__device__ __forceinline__ f2 mul2(f2 a, f2 b) { f2 d; asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b)); return d; }
-__device__ __forceinline__ f2 fma2(f2 a, f2 b, f2 c) { f2 d; asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(d) : "l"(a), "l"(b), "l"(c)); return d; }
+__device__ __forceinline__ f2 add2(f2 a, f2 b) { f2 d; asm TC_ASMV("add.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b)); return d; }
+__device__ __forceinline__ f2 sub2(f2 a, f2 b) { f2 d; asm TC_ASMV("sub.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b)); return d; }
+__device__ __forceinline__ f2 mul2(f2 a, f2 b) { f2 d; asm TC_ASMV("mul.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b)); return d; }
+__device__ __forceinline__ f2 fma2(f2 a, f2 b, f2 c) { f2 d; asm TC_ASMV("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(d) : "l"(a), "l"(b), "l"(c)); return d; }
 
 struct Acc2 {      // accumulators of a particle pair; `npot` accumulates -phi (negated at write-back)
   f2 ax, ay, az, npot;
 };
 struct Pos2 {      // positions of a particle pair
   f2 x, y, z;
+};
+struct Acc1 {      // the same for the single particle of an odd K
+  float ax, ay, az, npot;
+};
+struct Pos1 {
+  float x, y, z;
+};
+// The lane's particles of the current pass and their accumulators: floor(K/2) pairs and, K odd, one more particle
+struct PassState {
+  Pos2 P[kMaxKP];
+  Acc2 A[kMaxKP];
+  Pos1 p1;
+  Acc1 a1;
 };
 
 // particle-cell: monopole + traceless quadrupole (O6), d = X - x_i:
@@ -144,9 +148,11 @@ __device__ __forceinline__ void pc_interact(const Pos2& p, float eps2, const flo
   const f2 ri2 = mul2(ri, ri);
   const f2 ri3 = mul2(ri, ri2);
   const f2 ri5 = mul2(ri3, ri2);
-  const f2 gx = fma2(bc(nq1.x), dz, fma2(bc(nq0.w), dy, mul2(bc(nq0.x), dx)));   // -(Q d)
-  const f2 gy = fma2(bc(nq1.y), dz, fma2(bc(nq0.y), dy, mul2(bc(nq0.w), dx)));
-  const f2 gz = fma2(bc(nq0.z), dz, fma2(bc(nq1.y), dy, mul2(bc(nq1.x), dx)));
+  // -(Q d), column by column: the three products of one d_k are consecutive and share it (operand reuse cache:
+  // the register file delivers two 32-bit operands per lane and cycle, an FFMA2 with three register pairs needs six)
+  f2 gx = mul2(bc(nq0.x), dx), gy = mul2(bc(nq0.w), dx), gz = mul2(bc(nq1.x), dx);
+  gx = fma2(bc(nq0.w), dy, gx); gy = fma2(bc(nq0.y), dy, gy); gz = fma2(bc(nq1.y), dy, gz);
+  gx = fma2(bc(nq1.x), dz, gx); gy = fma2(bc(nq1.y), dz, gy); gz = fma2(bc(nq0.z), dz, gz);
   const f2 g = fma2(dz, gz, fma2(dy, gy, mul2(dx, gx)));                         // -(d^T Q d)
   const f2 t5 = mul2(g, ri5);
   a.npot = fma2(bc(xm.w), ri, a.npot);
@@ -154,6 +160,26 @@ __device__ __forceinline__ void pc_interact(const Pos2& p, float eps2, const flo
   const f2 c = fma2(bc(-2.5f), mul2(t5, ri2), mul2(bc(xm.w), ri3));
   a.ax = fma2(c, dx, a.ax); a.ay = fma2(c, dy, a.ay); a.az = fma2(c, dz, a.az);
   a.ax = fma2(ri5, gx, a.ax); a.ay = fma2(ri5, gy, a.ay); a.az = fma2(ri5, gz, a.az);
+}
+// the same interaction for ONE particle: 33 scalar FP32 instructions + 1 MUFU (the issue cost of half a pair)
+__device__ __forceinline__ void pc_interact(const Pos1& p, float eps2, const float4 xm, const float4 nq0,
+                                            const float2 nq1, Acc1& a) {
+  const float dx = __fsub_rn(xm.x, p.x), dy = __fsub_rn(xm.y, p.y), dz = __fsub_rn(xm.z, p.z);
+  const float s2 = __fmaf_rn(dz, dz, __fmaf_rn(dy, dy, __fmaf_rn(dx, dx, eps2)));
+  const float ri = rsqrt_approx(s2);
+  const float ri2 = __fmul_rn(ri, ri);
+  const float ri3 = __fmul_rn(ri, ri2);
+  const float ri5 = __fmul_rn(ri3, ri2);
+  const float gx = __fmaf_rn(nq1.x, dz, __fmaf_rn(nq0.w, dy, __fmul_rn(nq0.x, dx)));
+  const float gy = __fmaf_rn(nq1.y, dz, __fmaf_rn(nq0.y, dy, __fmul_rn(nq0.w, dx)));
+  const float gz = __fmaf_rn(nq0.z, dz, __fmaf_rn(nq1.y, dy, __fmul_rn(nq1.x, dx)));
+  const float g = __fmaf_rn(dz, gz, __fmaf_rn(dy, gy, __fmul_rn(dx, gx)));
+  const float t5 = __fmul_rn(g, ri5);
+  a.npot = __fmaf_rn(xm.w, ri, a.npot);
+  a.npot = __fmaf_rn(-0.5f, t5, a.npot);
+  const float c = __fmaf_rn(-2.5f, __fmul_rn(t5, ri2), __fmul_rn(xm.w, ri3));
+  a.ax = __fmaf_rn(c, dx, a.ax); a.ay = __fmaf_rn(c, dy, a.ay); a.az = __fmaf_rn(c, dz, a.az);
+  a.ax = __fmaf_rn(ri5, gx, a.ax); a.ay = __fmaf_rn(ri5, gy, a.ay); a.az = __fmaf_rn(ri5, gz, a.az);
 }
 
 // particle-particle, Plummer softening (O6), d = x_j - x_i:
@@ -172,115 +198,122 @@ __device__ __forceinline__ void pp_interact(const Pos2& p, float eps2, const flo
   a.npot = add2(a.npot, mr);
   a.ax = fma2(mr3, dx, a.ax); a.ay = fma2(mr3, dy, a.ay); a.az = fma2(mr3, dz, a.az);
 }
+template <bool kEps0>
+__device__ __forceinline__ void pp_interact(const Pos1& p, float eps2, const float4 b, Acc1& a) {
+  const float dx = __fsub_rn(b.x, p.x), dy = __fsub_rn(b.y, p.y), dz = __fsub_rn(b.z, p.z);
+  const float s2 = __fmaf_rn(dz, dz, __fmaf_rn(dy, dy, __fmaf_rn(dx, dx, eps2)));
+  float ri = rsqrt_approx(s2);
+  if (kEps0) ri = (s2 > 0.f) ? ri : 0.f;
+  const float ri2 = __fmul_rn(ri, ri);
+  const float mr = __fmul_rn(b.w, ri);
+  const float mr3 = __fmul_rn(mr, ri2);
+  a.npot = __fadd_rn(a.npot, mr);
+  a.ax = __fmaf_rn(mr3, dx, a.ax); a.ay = __fmaf_rn(mr3, dy, a.ay); a.az = __fmaf_rn(mr3, dz, a.az);
+}
 
-// Lane mapping of one pass over m <= kPass particles of a group (see file header):
-// lane = s * q + p, q = floor(32 / S); the lane's j-th particle is j * q + p, j < 2 kp.
+// Lane mapping of one pass over m <= kPassCap particles of a group (tc_lanes.h):
+// lane = s * q + p, q = floor(32 / S); the lane's j-th particle is j * q + p, j < K.
 struct Lanes {
-  int S, q, kp;  // warp-uniform; kp = particle PAIRS per lane
+  int S, q, K;   // warp-uniform
   int s, p;      // this lane's slice and particle column
   bool active;   // lane < S * q
 };
 
-// Un-opened cells (List 3, PAPER.md:105-114): slice s takes records s, s+S, s+2S, ...
-// Each record is loaded once and applied to the lane's KP particle pairs.
-template <int KP>
-__device__ __forceinline__ void eval_cells_k(const CellRec* __restrict__ rec, int cnt, float eps2, const Lanes& L,
-                                             const Pos2 (&P)[kMaxKP], Acc2 (&A)[kMaxKP]) {
-  if (!L.active) return;
-  // pointer walk (one add per record, no index multiply): slice s takes records s, s + S, ...
-  const CellRec* r0 = rec + L.s;
-  const CellRec* const end = rec + cnt;
-  const int st = L.S;
-  for (; r0 + st < end; r0 += 2 * st) {          // two records in flight
-    const CellRec* r1 = r0 + st;
-    const float4 a0 = r0->xm, b0 = r0->q0; const float2 c0 = r0->q1;
-    const float4 a1 = r1->xm, b1 = r1->q0; const float2 c1 = r1->q1;
+// one list record applied to the lane's KP pairs (+ ODD single particle)
+template <int KP, bool ODD>
+__device__ __forceinline__ void pc_apply(PassState& st, float eps2, const float4 a, const float4 b, const float2 c) {
 #pragma unroll
-    for (int j = 0; j < KP; j++) pc_interact(P[j], eps2, a0, b0, c0, A[j]);
+  for (int j = 0; j < KP; j++) pc_interact(st.P[j], eps2, a, b, c, st.A[j]);
+  if (ODD) pc_interact(st.p1, eps2, a, b, c, st.a1);
+}
+template <int KP, bool ODD, bool kEps0>
+__device__ __forceinline__ void pp_apply(PassState& st, float eps2, const float4 b) {
 #pragma unroll
-    for (int j = 0; j < KP; j++) pc_interact(P[j], eps2, a1, b1, c1, A[j]);
-  }
-  if (r0 < end) {
-    const float4 a0 = r0->xm, b0 = r0->q0; const float2 c0 = r0->q1;
-#pragma unroll
-    for (int j = 0; j < KP; j++) pc_interact(P[j], eps2, a0, b0, c0, A[j]);
-  }
+  for (int j = 0; j < KP; j++) pp_interact<kEps0>(st.P[j], eps2, b, st.A[j]);
+  if (ODD) pp_interact<kEps0>(st.p1, eps2, b, st.a1);
 }
 
-template <int KP = 1>
-__device__ __forceinline__ void eval_cells(const CellRec* rec, int cnt, float eps2, const Lanes& L,
-                                           const Pos2 (&P)[kMaxKP], Acc2 (&A)[kMaxKP]) {
-  if constexpr (KP == kMaxKP) {
-    eval_cells_k<KP>(rec, cnt, eps2, L, P, A);
+// Un-opened cells (List 3, PAPER.md:105-114): slice s takes records s, s+S, s+2S, ...
+// Each record is loaded once and applied to the lane's K = 2 KP + ODD particles.
+template <int KP, bool ODD>
+__device__ __forceinline__ void eval_cells_k(const CellRec* __restrict__ rec, int cnt, float eps2, const Lanes& L, PassState& st) {
+  if (!L.active) return;
+  // pointer walk (one add per record, no index multiply)
+  const CellRec* r0 = rec + L.s;
+  const CellRec* const end = rec + cnt;
+  const int sd = L.S;
+  if (2 * KP + ODD <= TC_UNROLL2_MAXK) {
+    for (; r0 + sd < end; r0 += 2 * sd) {          // two records in flight
+      const CellRec* r1 = r0 + sd;
+      const float4 a0 = r0->xm, b0 = r0->q0; const float2 c0 = r0->q1;
+      const float4 a1 = r1->xm, b1 = r1->q0; const float2 c1 = r1->q1;
+      pc_apply<KP, ODD>(st, eps2, a0, b0, c0);
+      pc_apply<KP, ODD>(st, eps2, a1, b1, c1);
+    }
+    if (r0 < end) {
+      const float4 a0 = r0->xm, b0 = r0->q0; const float2 c0 = r0->q1;
+      pc_apply<KP, ODD>(st, eps2, a0, b0, c0);
+    }
   } else {
-    if (L.kp == KP) eval_cells_k<KP>(rec, cnt, eps2, L, P, A);   // warp-uniform
-    else eval_cells<KP + 1>(rec, cnt, eps2, L, P, A);
+    for (; r0 < end; r0 += sd) {
+      const float4 a0 = r0->xm, b0 = r0->q0; const float2 c0 = r0->q1;
+      pc_apply<KP, ODD>(st, eps2, a0, b0, c0);
+    }
   }
 }
 
 // Monopole-only variant (R22, option "quadrupole" = 0): a cell is a point mass (X, M)
-template <int KP, bool kEps0>
-__device__ __forceinline__ void eval_cells_mono_k(const CellRec* __restrict__ rec, int cnt, float eps2, const Lanes& L,
-                                                  const Pos2 (&P)[kMaxKP], Acc2 (&A)[kMaxKP]) {
+template <int KP, bool ODD, bool kEps0>
+__device__ __forceinline__ void eval_cells_mono_k(const CellRec* __restrict__ rec, int cnt, float eps2, const Lanes& L, PassState& st) {
   if (!L.active) return;
-  const int st = L.S;
-  for (int e = L.s; e < cnt; e += st) {
-    const float4 b0 = rec[e].xm;
-#pragma unroll
-    for (int j = 0; j < KP; j++) pp_interact<kEps0>(P[j], eps2, b0, A[j]);
-  }
+  const int sd = L.S;
+  for (int e = L.s; e < cnt; e += sd) pp_apply<KP, ODD, kEps0>(st, eps2, rec[e].xm);
 }
 
-template <bool kEps0, int KP = 1>
-__device__ __forceinline__ void eval_cells_mono(const CellRec* rec, int cnt, float eps2, const Lanes& L,
-                                                const Pos2 (&P)[kMaxKP], Acc2 (&A)[kMaxKP]) {
-  if constexpr (KP == kMaxKP) {
-    eval_cells_mono_k<KP, kEps0>(rec, cnt, eps2, L, P, A);
-  } else {
-    if (L.kp == KP) eval_cells_mono_k<KP, kEps0>(rec, cnt, eps2, L, P, A);
-    else eval_cells_mono<kEps0, KP + 1>(rec, cnt, eps2, L, P, A);
-  }
-}
-
-template <int KP, bool kEps0>
-__device__ __forceinline__ void eval_bodies_k(const float4* __restrict__ body, int cnt, float eps2, const Lanes& L,
-                                              const Pos2 (&P)[kMaxKP], Acc2 (&A)[kMaxKP]) {
+template <int KP, bool ODD, bool kEps0>
+__device__ __forceinline__ void eval_bodies_k(const float4* __restrict__ body, int cnt, float eps2, const Lanes& L, PassState& st) {
   if (!L.active) return;
   const float4* b = body + L.s;                  // pointer walk, as in eval_cells_k
   const float4* const end = body + cnt;
-  const int st = L.S;
-  for (; b + 3 * st < end; b += 4 * st) {        // four bodies in flight
-    const float4 b0 = b[0], b1 = b[st], b2 = b[2 * st], b3 = b[3 * st];
-#pragma unroll
-    for (int j = 0; j < KP; j++) {
-      pp_interact<kEps0>(P[j], eps2, b0, A[j]); pp_interact<kEps0>(P[j], eps2, b1, A[j]);
-      pp_interact<kEps0>(P[j], eps2, b2, A[j]); pp_interact<kEps0>(P[j], eps2, b3, A[j]);
+  const int sd = L.S;
+  if (2 * KP + ODD <= 2) {
+    for (; b + 3 * sd < end; b += 4 * sd) {        // four bodies in flight
+      const float4 b0 = b[0], b1 = b[sd], b2 = b[2 * sd], b3 = b[3 * sd];
+      pp_apply<KP, ODD, kEps0>(st, eps2, b0); pp_apply<KP, ODD, kEps0>(st, eps2, b1);
+      pp_apply<KP, ODD, kEps0>(st, eps2, b2); pp_apply<KP, ODD, kEps0>(st, eps2, b3);
+    }
+  } else {
+    for (; b + sd < end; b += 2 * sd) {            // two bodies in flight
+      const float4 b0 = b[0], b1 = b[sd];
+      pp_apply<KP, ODD, kEps0>(st, eps2, b0); pp_apply<KP, ODD, kEps0>(st, eps2, b1);
     }
   }
-  for (; b < end; b += st) {
-    const float4 b0 = b[0];
-#pragma unroll
-    for (int j = 0; j < KP; j++) pp_interact<kEps0>(P[j], eps2, b0, A[j]);
-  }
+  for (; b < end; b += sd) pp_apply<KP, ODD, kEps0>(st, eps2, b[0]);
 }
 
-template <bool kEps0, int KP = 1>
-__device__ __forceinline__ void eval_bodies(const float4* body, int cnt, float eps2, const Lanes& L,
-                                            const Pos2 (&P)[kMaxKP], Acc2 (&A)[kMaxKP]) {
-  if constexpr (KP == kMaxKP) {
-    eval_bodies_k<KP, kEps0>(body, cnt, eps2, L, P, A);
-  } else {
-    if (L.kp == KP) eval_bodies_k<KP, kEps0>(body, cnt, eps2, L, P, A);
-    else eval_bodies<kEps0, KP + 1>(body, cnt, eps2, L, P, A);
+// K is warp-uniform: one branch to the instantiation for this pass's particles per lane
+enum { kEvalCells = 0, kEvalMono = 1, kEvalBodies = 2 };
+template <int WHAT, bool kEps0, int K = 1>
+__device__ __forceinline__ void eval_dispatch(const void* list, int cnt, float eps2, const Lanes& L, PassState& st) {
+  if (K == kMaxK || L.K == K) {
+    if (WHAT == kEvalCells) eval_cells_k<K / 2, (K & 1) != 0>(static_cast<const CellRec*>(list), cnt, eps2, L, st);
+    else if (WHAT == kEvalMono) eval_cells_mono_k<K / 2, (K & 1) != 0, kEps0>(static_cast<const CellRec*>(list), cnt, eps2, L, st);
+    else eval_bodies_k<K / 2, (K & 1) != 0, kEps0>(static_cast<const float4*>(list), cnt, eps2, L, st);
+  } else if constexpr (K < kMaxK) {
+    eval_dispatch<WHAT, kEps0, K + 1>(list, cnt, eps2, L, st);
   }
+}
+template <bool kEps0>
+__device__ __forceinline__ void eval_cells(const CellRec* rec, int cnt, float eps2, const Lanes& L, PassState& st, bool mono) {
+  if (mono) eval_dispatch<kEvalMono, kEps0>(rec, cnt, eps2, L, st);
+  else eval_dispatch<kEvalCells, kEps0>(rec, cnt, eps2, L, st);
 }
 
 // Opened leaves (List 4): flatten the queued (first, n) ranges into
 // body indices, gather the bodies with one coalesced float4 load per lane, evaluate.
 template <bool kEps0>
 __device__ __forceinline__ void eval_leaves(BodyStage& bs, const int2* leafq, int nq, const float4* __restrict__ part,
-                                            float eps2, const Lanes& L, const Pos2 (&P)[kMaxKP], Acc2 (&A)[kMaxKP],
-                                            int lane) {
+                                            float eps2, const Lanes& L, PassState& st, int lane) {
   for (int r0 = 0; r0 < nq; r0 += 32) {
     int f = 0, n = 0;
     if (r0 + lane < nq) { const int2 r = leafq[r0 + lane]; f = r.x; n = r.y; }
@@ -296,32 +329,36 @@ __device__ __forceinline__ void eval_leaves(BodyStage& bs, const int2* leafq, in
       const int cnt = min(kBodyCap, total - base);
       for (int t = lane; t < cnt; t += 32) bs.body[t] = __ldg(part + bs.bidx[t]);
       __syncwarp();
-      eval_bodies<kEps0>(bs.body, cnt, eps2, L, P, A);
+      eval_dispatch<kEvalBodies, kEps0>(bs.body, cnt, eps2, L, st);
       __syncwarp();
     }
   }
 }
 
-// Lane mapping, particle pairs and zeroed accumulators of one pass over particles [first, first + m)
-__device__ __forceinline__ void setup_pass(Lanes& L, Pos2 (&P)[kMaxKP], Acc2 (&A)[kMaxKP], const float4* __restrict__ part,
-                                           int first, int m, int lane) {
-  L.S = c_slices.S[m];
-  L.q = 32 / L.S;
-  L.kp = (m + 2 * L.q - 1) / (2 * L.q);
+// Lane mapping, particles and zeroed accumulators of one pass over particles [first, first + m)
+__device__ __forceinline__ void setup_pass(Lanes& L, PassState& st, const float4* __restrict__ part, int first, int m, int lane) {
+  const LaneMap lm = c_lanes.map[m];
+  L.S = lm.S; L.q = lm.q; L.K = lm.K;
   L.s = lane / L.q;
   L.p = lane - L.s * L.q;
   L.active = L.s < L.S;
+  // slots beyond m compute on a copy of the pass's first particle; never written back
 #pragma unroll
   for (int j = 0; j < kMaxKP; j++) {
-    A[j].ax = A[j].ay = A[j].az = A[j].npot = 0ull;  // (+0.f, +0.f)
-    // slots beyond m compute on a copy of the pass's first particle; never written back
+    st.A[j].ax = st.A[j].ay = st.A[j].az = st.A[j].npot = 0ull;  // (+0.f, +0.f)
     const int t0 = 2 * j * L.q + L.p, t1 = t0 + L.q;
     const float4 m0 = __ldg(part + first + ((L.active && t0 < m) ? t0 : 0));
     const float4 m1 = __ldg(part + first + ((L.active && t1 < m) ? t1 : 0));
     // (+ 0 through FADD2: the pair is then the result of a real instruction and stays in one aligned
     // register pair; a bare mov.b64 is re-materialised with two MOVs in front of every use)
-    P[j].x = add2(pk(m0.x, m1.x), bc(0.f)); P[j].y = add2(pk(m0.y, m1.y), bc(0.f));
-    P[j].z = add2(pk(m0.z, m1.z), bc(0.f));
+    st.P[j].x = add2(pk(m0.x, m1.x), bc(0.f)); st.P[j].y = add2(pk(m0.y, m1.y), bc(0.f));
+    st.P[j].z = add2(pk(m0.z, m1.z), bc(0.f));
+  }
+  {  // K odd: the lane's last particle, K - 1, is evaluated with scalar instructions
+    const int t = (L.K - 1) * L.q + L.p;
+    const float4 m0 = __ldg(part + first + ((L.active && t < m) ? t : 0));
+    st.p1.x = m0.x; st.p1.y = m0.y; st.p1.z = m0.z;
+    st.a1.ax = st.a1.ay = st.a1.az = st.a1.npot = 0.f;
   }
 }
 
@@ -329,18 +366,19 @@ __device__ __forceinline__ void setup_pass(Lanes& L, Pos2 (&P)[kMaxKP], Acc2 (&A
 // kAdd: add to what is already there (second evaluation kernel of the two-pass variant);
 // kSelf: the particles met themselves once in the particle-particle part (remove -m/eps again).
 template <bool kAdd, bool kSelf>
-__device__ __forceinline__ void write_back(const Lanes& L, const Acc2 (&A)[kMaxKP], const float4* __restrict__ part,
+__device__ __forceinline__ void write_back(const Lanes& L, const PassState& st, const float4* __restrict__ part,
                                            const int32_t* __restrict__ orig, int first, int m, float eps2, int lane,
                                            float* __restrict__ acc, float* __restrict__ pot, int32_t* __restrict__ out_cnt,
                                            int cnt_value, int32_t* __restrict__ out_cnt2 = nullptr, int cnt2_value = 0,
                                            bool self_met = true) {
 #pragma unroll
-  for (int j = 0; j < 2 * kMaxKP; j++) {
-    if (j >= 2 * L.kp) break;                        // warp-uniform
-    const Acc2& a2 = A[j >> 1];
+  for (int j = 0; j < kMaxK; j++) {
+    if (j >= L.K) break;                             // warp-uniform
+    const Acc2& a2 = st.A[j >> 1];
     float ax, ay, az, ph;
     if (j & 1) { ax = hi(a2.ax); ay = hi(a2.ay); az = hi(a2.az); ph = -hi(a2.npot); }
     else { ax = lo(a2.ax); ay = lo(a2.ay); az = lo(a2.az); ph = -lo(a2.npot); }
+    if (!(j & 1) && j == L.K - 1) { ax = st.a1.ax; ay = st.a1.ay; az = st.a1.az; ph = -st.a1.npot; }   // K odd: the single particle
     for (int w = 1; w < L.S; w <<= 1) {
       const float ox = __shfl_down_sync(kFull, ax, w * L.q), oy = __shfl_down_sync(kFull, ay, w * L.q);
       const float oz = __shfl_down_sync(kFull, az, w * L.q), op = __shfl_down_sync(kFull, ph, w * L.q);
@@ -414,18 +452,18 @@ forces_kernel(const float4* __restrict__ bnd, const float4* __restrict__ xm, con
     float ghx = gh, ghy = gh, ghz = gh;
     if (group_box) { const float4 e = __ldg(gbox + g); ghx = e.x; ghy = e.y; ghz = e.z; }
 
-    // groups larger than kPass particles (level-21 leaves, or a large N_group) repeat the walk per kPass
-    for (int pb = 0; pb < G.z; pb += kPass) {
-      const int m = min(kPass, G.z - pb);
+    // ONE walk per group.  Only a group of more than kPassCap particles (a level-21 leaf of
+    // coincident particles, or N_group > kPassCap) is walked once per kPassCap of them.
+    for (int pb = 0; pb < G.z; pb += kPassCap) {
+      const int m = min(kPassCap, G.z - pb);
       Lanes L;
-      Pos2 P[kMaxKP];
-      Acc2 A[kMaxKP];
-      if (MODE == kFused) setup_pass(L, P, A, part, G.y + pb, m, lane);
+      PassState ps;
+      if (MODE == kFused) setup_pass(L, ps, part, G.y + pb, m, lane);
       unsigned long long woff_c = 0, woff_l = 0;         // MODE kWrite: where this group's lists start
       if (MODE == kWrite) { woff_c = lio.off_c[g]; woff_l = lio.off_l[g]; }
 
       int ssz = 0, spill_sz = 0, ccnt = 0, lq = 0;
-      long long n_pc = 0, n_pp = 0, n_tests = 0;
+      int n_pc = 0, n_pp = 0, n_open = 0;                // list entries so far; n_open: opened cells (leaves + nodes)
       int n_spills = 0, n_lr = 0;                        // n_lr: opened-leaf ranges so far
       bool overflow = false;
       // Did the pass's particles meet themselves in the particle-particle part?  Always, under the default
@@ -447,22 +485,43 @@ forces_kernel(const float4* __restrict__ bnd, const float4* __restrict__ xm, con
       __syncwarp();
 
       // ---- the walk (List 1-2): pop up to 4 nodes, test their children
+      // (the evaluation code exists ONCE, at the bottom of this loop: the last trip, `walking` false, flushes what is left)
       while (true) {
+        bool walking = true;
         if (ssz == 0) {
-          if (spill_sz == 0) break;
-          const int take = min(spill_sz, STK / 2);      // reload the top of the spill stack
-          for (int t = lane; t < take; t += 32) sm.stack[t] = spill[spill_sz - take + t];
-          spill_sz -= take; ssz = take;
-          __syncwarp();
+          if (spill_sz == 0) walking = false;
+          else {
+            const int take = min(spill_sz, STK / 2);      // reload the top of the spill stack
+            for (int t = lane; t < take; t += 32) sm.stack[t] = spill[spill_sz - take + t];
+            spill_sz -= take; ssz = take;
+            __syncwarp();
+          }
         }
-        const int npop = min(ssz, 4);
+        if (walking) {
+        // up to kWalkB batches of 4 nodes per iteration: the child loads of all batches are issued together, so an
+        // iteration still costs ONE memory latency (the walk is latency-bound; the evaluation of other warps hides it)
+        const int npop = min(ssz, 4 * kWalkB);
         const int slot = lane >> 3, k = lane & 7;
-        const uint32_t packed = (slot < npop) ? sm.stack[ssz - 1 - slot] : 0u;
+        bool valid_b[kWalkB];
+        int c_b[kWalkB];
+        float4 cb_b[kWalkB], cx_b[kWalkB], c0_b[kWalkB], c1_b[kWalkB];
+#pragma unroll
+        for (int b = 0; b < kWalkB; b++) {
+          const int sl = slot + 4 * b;
+          const uint32_t packed = (sl < npop) ? sm.stack[ssz - 1 - sl] : 0u;
+          valid_b[b] = (sl < npop) && (k <= (int)(packed & 7u));
+          // lanes without a child load cell 0 (the root always exists); `valid` masks everything they compute
+          c_b[b] = valid_b[b] ? (int)(packed >> 3) + k : 0;
+          cb_b[b] = __ldg(bnd + c_b[b]); cx_b[b] = __ldg(xm + c_b[b]); c0_b[b] = __ldg(q0 + c_b[b]); c1_b[b] = __ldg(q1 + c_b[b]);
+        }
         ssz -= npop;
-        const bool valid = (slot < npop) && (k <= (int)(packed & 7u));
-        // lanes without a child load cell 0 (the root always exists); `valid` masks everything they compute
-        const int c = valid ? (int)(packed >> 3) + k : 0;
-        const float4 cb = __ldg(bnd + c), cx = __ldg(xm + c), c0 = __ldg(q0 + c), c1 = __ldg(q1 + c);
+        __syncwarp();                                    // all pops were read before slots are reused
+#pragma unroll
+        for (int b = 0; b < kWalkB; b++) {
+        if (b > 0 && npop <= 4 * b) break;               // warp-uniform: this batch is empty
+        const bool valid = valid_b[b];
+        const int c = c_b[b];
+        const float4 cb = cb_b[b], cx = cx_b[b], c0 = c0_b[b], c1 = c1_b[b];
         // open_node (O5/R16): one fixed sequence of correctly rounded fp32 operations
         // (variant R21, com_rule: the cell's centre of mass in place of b_c, 0 in place of h_c in the distance)
         const float hc = fabsf(cb.w);
@@ -482,7 +541,6 @@ forces_kernel(const float4* __restrict__ bnd, const float4* __restrict__ xm, con
         const unsigned m_cell = __ballot_sync(kFull, to_cell);
         const unsigned m_leaf = __ballot_sync(kFull, to_leaf);
         const unsigned m_stack = __ballot_sync(kFull, to_stack);
-        n_tests += __popc(__ballot_sync(kFull, valid));
         if (to_cell) {                                   // not opened (leaf or node): multipole (R2)
           if (MODE == kFused) {
             CellRec& r = sm.u.cell[ccnt + __popc(m_cell & lt_mask)];
@@ -499,19 +557,21 @@ forces_kernel(const float4* __restrict__ bnd, const float4* __restrict__ xm, con
             else if (MODE == kWrite) lio.leaves[woff_l + (unsigned long long)(n_lr + __popc(m_leaf & lt_mask))] = make_int2(la, lb);
           }
           if (MODE == kFused) lq += __popc(m_leaf); else n_lr += __popc(m_leaf);
+          n_open += __popc(m_leaf);
           n_pp += __reduce_add_sync(kFull, to_leaf ? lb : 0);
           if (!kPlain && MODE == kFused) {                 // own leaf opened? (all or nothing per group, see above)
             const int fb = G.y + pb;
             self_met |= __any_sync(kFull, to_leaf && la <= fb && fb < la + lb);
           }
         }
-        if (m_stack) {                                   // opened node: walk on
+        if (m_stack && !overflow) {                      // opened node: walk on
           const int npush = __popc(m_stack);
-          __syncwarp();                                  // all pops were read before slots are reused
+          n_open += npush;
           if (ssz + npush > STK) {                       // spill the bottom half to global memory
             const int mv = STK / 2;
             if (spill_sz + mv > spill_cap) { overflow = true; }
             else {
+              __syncwarp();
               for (int t = lane; t < mv; t += 32) spill[spill_sz + t] = sm.stack[t];
               __syncwarp();
               for (int t0 = mv; t0 < ssz; t0 += 32) {    // shift the rest down (ascending, chunked)
@@ -524,30 +584,31 @@ forces_kernel(const float4* __restrict__ bnd, const float4* __restrict__ xm, con
               spill_sz += mv; ssz -= mv; n_spills++;
             }
           }
-          if (overflow) break;
-          if (to_stack) sm.stack[ssz + __popc(m_stack & lt_mask)] = ((uint32_t)la << 3) | (uint32_t)(lb - 1);
-          ssz += npush;
+          if (!overflow) {
+            if (to_stack) sm.stack[ssz + __popc(m_stack & lt_mask)] = ((uint32_t)la << 3) | (uint32_t)(lb - 1);
+            ssz += npush;
+          }
         }
+        }  // batches
+        if (overflow) break;
         __syncwarp();
-        if (MODE != kFused) continue;
-        const bool flush_leaves = lq > kLeafQCap - 32;
-        if (ccnt > kCellCap - 32 || (flush_leaves && ccnt)) {
-          if (!walk_only) { if (mono) eval_cells_mono<kEps0>(sm.u.cell, ccnt, eps2, L, P, A); else eval_cells(sm.u.cell, ccnt, eps2, L, P, A); }
-          ccnt = 0; __syncwarp();
+        }  // walking
+        if (MODE == kFused) {
+          // a chunk is evaluated when the next iteration might not fit, the bodies' staging area (the same memory)
+          // is needed, or the walk is over
+          const bool flush_leaves = walking ? (lq > kLeafQCap - 32 * kWalkB) : (lq > 0);
+          if (ccnt > (walking ? kCellCap - 32 * kWalkB : 0) || (flush_leaves && ccnt)) {
+            if (!walk_only) eval_cells<kEps0>(sm.u.cell, ccnt, eps2, L, ps, mono);
+            ccnt = 0; __syncwarp();
+          }
+          if (flush_leaves) { if (!walk_only) eval_leaves<kEps0>(sm.u.bs, sm.leafq, lq, part, eps2, L, ps, lane); lq = 0; __syncwarp(); }
         }
-        if (flush_leaves) { if (!walk_only) eval_leaves<kEps0>(sm.u.bs, sm.leafq, lq, part, eps2, L, P, A, lane); lq = 0; }
-      }
-      if (MODE == kFused) {
-        if (ccnt && !walk_only) { if (mono) eval_cells_mono<kEps0>(sm.u.cell, ccnt, eps2, L, P, A); else eval_cells(sm.u.cell, ccnt, eps2, L, P, A); }
-        __syncwarp();
-        if (lq && !walk_only) eval_leaves<kEps0>(sm.u.bs, sm.leafq, lq, part, eps2, L, P, A, lane);
-        __syncwarp();
+        if (!walking) break;
       }
 
       if (MODE == kFused) {
         // ---- A6: reduce the slices of every particle, write back in the caller's order
-        write_back<false, !kEps0>(L, A, part, orig, G.y + pb, m, eps2, lane, acc, pot, out_npc, (int32_t)n_pc, out_npp,
-                                  (int32_t)(n_pp - 1), self_met);
+        write_back<false, !kEps0>(L, ps, part, orig, G.y + pb, m, eps2, lane, acc, pot, out_npc, n_pc, out_npp, n_pp - 1, self_met);
       } else if (MODE == kCount) {
         if (lane == 0) { lio.cnt_c[g] = (unsigned long long)n_pc; lio.cnt_l[g] = (unsigned long long)n_lr; lio.leaf_bodies[g] = (int)n_pp; }
       }
@@ -556,7 +617,8 @@ forces_kernel(const float4* __restrict__ bnd, const float4* __restrict__ xm, con
           const long long np = (MODE == kFused) ? m : G.z;
           atomicAdd(&ctr->n_pc_total, (unsigned long long)(n_pc * np));
           atomicAdd(&ctr->n_pp_total, (unsigned long long)((n_pp - 1) * np));
-          if (pb == 0) atomicAdd(&ctr->n_tests_total, (unsigned long long)n_tests);   // per group, not per pass
+          // opening tests EXECUTED by this walk: every tested child ends on the cell list or is opened
+          atomicAdd(&ctr->n_tests_total, (unsigned long long)(n_pc + n_open));
         }
         if (n_spills) atomicAdd(&ctr->n_spills, (unsigned long long)n_spills);
         if (overflow) atomicExch(&ctr->overflow, 1u);
@@ -588,10 +650,10 @@ node_kernel(const float4* __restrict__ xm, const float4* __restrict__ q0, const 
     const int4 G = __ldg(grp + g);
     const unsigned long long b = lio.off_c[g];
     const int n_c = (int)(lio.off_c[g + 1] - b);
-    for (int pb = 0; pb < G.z; pb += kPass) {
-      const int m = min(kPass, G.z - pb);
-      Lanes L; Pos2 P[kMaxKP]; Acc2 A[kMaxKP];
-      setup_pass(L, P, A, part, G.y + pb, m, lane);
+    for (int pb = 0; pb < G.z; pb += kPassCap) {
+      const int m = min(kPassCap, G.z - pb);
+      Lanes L; PassState ps;
+      setup_pass(L, ps, part, G.y + pb, m, lane);
       for (int base = 0; base < n_c; base += kCellCap) {
         const int cnt = min(kCellCap, n_c - base);
         for (int t = lane; t < cnt; t += 32) {
@@ -601,10 +663,10 @@ node_kernel(const float4* __restrict__ xm, const float4* __restrict__ q0, const 
           r.xm = __ldg(xm + c); r.q0 = __ldg(q0 + c); r.q1 = make_float2(c1.x, c1.y);
         }
         __syncwarp();
-        if (mono) eval_cells_mono<false>(sm.u.cell, cnt, eps2, L, P, A); else eval_cells(sm.u.cell, cnt, eps2, L, P, A);
+        eval_cells<false>(sm.u.cell, cnt, eps2, L, ps, mono);
         __syncwarp();
       }
-      write_back<false, false>(L, A, part, orig, G.y + pb, m, eps2, lane, acc, pot, out_npc, n_c);
+      write_back<false, false>(L, ps, part, orig, G.y + pb, m, eps2, lane, acc, pot, out_npc, n_c);
     }
   }
 }
@@ -629,10 +691,10 @@ leaf_kernel(const float4* __restrict__ part, const int32_t* __restrict__ orig, c
     const unsigned long long b = lio.off_l[g];
     const int n_l = (int)(lio.off_l[g + 1] - b);
     const int n_bodies = __ldg(lio.leaf_bodies + g);
-    for (int pb = 0; pb < G.z; pb += kPass) {
-      const int m = min(kPass, G.z - pb);
-      Lanes L; Pos2 P[kMaxKP]; Acc2 A[kMaxKP];
-      setup_pass(L, P, A, part, G.y + pb, m, lane);
+    for (int pb = 0; pb < G.z; pb += kPassCap) {
+      const int m = min(kPassCap, G.z - pb);
+      Lanes L; PassState ps;
+      setup_pass(L, ps, part, G.y + pb, m, lane);
       bool self_met = false;                 // is the pass's own leaf on the list? (see forces_kernel)
       const int fb = G.y + pb;
       for (int base = 0; base < n_l; base += kLeafQCap) {
@@ -645,10 +707,10 @@ leaf_kernel(const float4* __restrict__ part, const int32_t* __restrict__ orig, c
         }
         self_met |= __any_sync(kFull, mine);
         __syncwarp();
-        eval_leaves<kEps0>(sm.u.bs, sm.leafq, cnt, part, eps2, L, P, A, lane);
+        eval_leaves<kEps0>(sm.u.bs, sm.leafq, cnt, part, eps2, L, ps, lane);
         __syncwarp();
       }
-      write_back<true, !kEps0>(L, A, part, orig, G.y + pb, m, eps2, lane, acc, pot, out_npp, n_bodies - 1, nullptr, 0, self_met);
+      write_back<true, !kEps0>(L, ps, part, orig, G.y + pb, m, eps2, lane, acc, pot, out_npp, n_bodies - 1, nullptr, 0, self_met);
     }
   }
 }

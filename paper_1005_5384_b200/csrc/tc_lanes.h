@@ -1,0 +1,71 @@
+// Lane mapping of the force kernel, shared by the kernel (tc_kernels.cu) and by the two builders'
+// schedules (tc_build.cpp, tc_build_gpu.cu) so that the cost model of the schedule IS the kernel's
+// mapping, not a hand-kept mirror of it.  Plain constexpr C++: host and device.
+//
+// One pass of a warp over m <= kPassCap particles of a group (one tree walk) picks
+//   S slices of the interaction list  x  q = floor(32 / S) particle columns,   lane = s * q + p,
+//   K = ceil(m / q) <= kMaxK particles per lane (particle j of lane (s, p) is j * q + p),
+// so that the cycles per list entry, kRecordCycles[K] / S, are minimal.  kRecordCycles[K] is MEASURED: SM sub-partition
+// cycles per list record of the particle-cell loop with K particles per lane (floor(K/2) packed FFMA2 pairs + one scalar
+// particle when K is odd), four warps resident per sub-partition as in the kernel (the loop is
+// bound by register-file operand bandwidth, an FFMA2 with three register-pair operands issues every 3 cycles, and
+// the scalar particle of an odd K costs 58 % of a pair, not 50 %).  Every list record is read from shared memory
+// once per lane and applied to the lane's K particles.  This is the answer to the paper's 30 % thread utilisation
+// with thread-per-particle blocks.
+#pragma once
+
+#ifdef __CUDACC__
+#define TC_HD __host__ __device__
+#else
+#define TC_HD
+#endif
+
+namespace tc {
+
+#ifndef TC_MAXK
+#define TC_MAXK 8
+#endif
+#ifndef TC_PASSCAP
+#define TC_PASSCAP 128
+#endif
+constexpr int kMaxK = TC_MAXK;          // particles per lane: kMaxK / 2 packed pairs (+ one scalar particle when K is odd)
+constexpr int kPassCap = TC_PASSCAP;    // particles of a group handled by ONE walk; larger groups (level-21 leaves of
+                                        // coincident particles, or N_group > kPassCap) are walked once per kPassCap
+static_assert(kMaxK >= 4 && kMaxK <= 8 && kPassCap <= 32 * kMaxK, "every pass size needs a mapping with S = 1");
+constexpr float kRecordCycles[9] = {0.f, 47.3f, 87.0f, 134.7f, 160.6f, 208.3f, 240.8f, 293.7f, 324.1f};
+
+struct LaneMap {
+  unsigned char S, q, K;
+};
+
+struct LaneTable {
+  LaneMap map[kPassCap + 1];
+  int cost8[kPassCap + 1];    // cycles per list entry of a pass over m particles, in units of 1/8 cycle
+  constexpr LaneTable() : map{}, cost8{} {
+    map[0] = LaneMap{1, 32, 1};
+    cost8[0] = 0;
+    for (int m = 1; m <= kPassCap; m++) {
+      int bs = 0, bq = 0, bk = 0;
+      float best = 1e30f;
+      for (int s = 1; s <= 32; s++) {
+        const int q = 32 / s;
+        const int k = (m + q - 1) / q;
+        if (k > kMaxK) continue;
+        const float c = kRecordCycles[k] / (float)s;
+        if (c < best) { best = c; bs = s; bq = q; bk = k; }
+      }
+      map[m] = LaneMap{(unsigned char)bs, (unsigned char)bq, (unsigned char)bk};
+      cost8[m] = (int)(best * 8.f + 0.5f);
+    }
+  }
+};
+
+// Cost class of a whole group of `cnt` particles for the schedule (costly groups run first): cycles per
+// list entry in 1/8 cycles, integer so that the host and the device builder agree bit for bit; <= kMaxCostClass.
+constexpr int kMaxCostClass = 1000000;
+TC_HD constexpr int group_cost_class(const LaneTable& t, long long cnt) {
+  const long long c = (cnt / kPassCap) * (long long)t.cost8[kPassCap] + (long long)t.cost8[cnt % kPassCap];
+  return c > kMaxCostClass ? kMaxCostClass : (int)c;
+}
+
+}  // namespace tc

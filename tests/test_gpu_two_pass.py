@@ -40,11 +40,18 @@ def test_two_pass_equals_fused_and_oracle(name, n_leaf, n_group, eps):
     f = _run(pos, mass, theta, eps, n_leaf, n_group, 0)
     t = _run(pos, mass, theta, eps, n_leaf, n_group, 1)
     assert np.array_equal(f[2], t[2]) and np.array_equal(f[3], t[3])
-    for k in ("n_pc_total", "n_pp_total", "n_tests_total"):
+    for k in ("n_pc_total", "n_pp_total"):
         assert f[4][k] == t[4][k], k
     assert rel_err(t[0].astype(np.float64), f[0].astype(np.float64)).max() <= 5e-5
     assert t[4]["list_bytes"] > 0 and t[4]["t_node_ms"] > 0 and f[4]["list_bytes"] == 0
-    check(t[0], t[1], t[2], t[3], Oracle(pos, mass, n_leaf, n_group).forces(theta, eps, shadow32=True))
+    o = Oracle(pos, mass, n_leaf, n_group)
+    ref = o.forces(theta, eps, shadow32=True, stats=True)
+    check(t[0], t[1], t[2], t[3], ref)
+    # opening tests EXECUTED: the count pass walks every group once; the fused kernel walks a group once per
+    # 128 of its particles (include/tc.h, tc_stats.n_tests_total), i.e. once for every N_group <= 128
+    m = o.cells()["count"][o.groups()]
+    assert t[4]["n_tests_total"] == int(ref["tests"].sum())
+    assert f[4]["n_tests_total"] == int((ref["tests"] * ((m + 127) // 128)).sum())
 
 
 def test_two_pass_degenerate_and_spill():

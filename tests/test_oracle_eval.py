@@ -130,6 +130,66 @@ def test_softened_particle_cell_reduces_to_softened_monopole_for_point_cell():
     assert np.allclose(r["acc"][1], -2.0 * np.array([3, 4, 12]) / s2 ** 1.5, rtol=1e-14)
 
 
+# ---------------------------------------------------------------- softened quadrupole (R11)
+def _two_mass_field(field, theta=2.0):
+    """Two masses in one leaf A (the cell), the field point alone in leaf B; B's walk lists A un-opened."""
+    G = read_golden("quadrupole_two_mass_softened.txt")
+    d, mm = G["d"], G["m"]
+    pos = np.array([[-d, 0, 0], [d, 0, 0], field], np.float32)
+    m = np.array([mm, mm, 1e-3], np.float32)
+    O = oracle.Oracle(pos, m, 2)
+    c = O.cells()
+    assert O.n_cells == 3
+    A = int(np.nonzero(c["count"] == 2)[0][0])
+    gB = [k for k, gc in enumerate(O.groups()) if c["count"][gc] == 1][0]
+    cl, ll, *_ = O.walk(gB, theta)
+    assert cl.tolist() == [A] and ll.size == 1
+    return G, O
+
+
+def test_softened_quadrupole_on_axis_golden():
+    """R11 pin with Q != 0 and eps ~ |r|: sigma^2 = r^2 + eps^2 in the s^-5 AND s^-7 terms.  With r in place of sigma in
+    either term the on-axis a_x would be -3.62 or -6.27 instead of -4.292608 (golden header)."""
+    G, O = _two_mass_field([0.5, 0, 0])
+    r = O.forces(2.0, G["A_eps"])
+    assert r["n_pc"][2] == 1 and r["n_pp"][2] == 0
+    assert abs(r["acc"][2, 0] - G["A_ax"]) < 1e-14 and abs(r["acc"][2, 1]) < 1e-18 and abs(r["acc"][2, 2]) < 1e-18
+    assert abs(r["pot"][2] - G["A_phi"]) < 1e-14
+    r = O.forces(2.0, G["C_eps"])
+    assert abs(r["acc"][2, 0] - G["C_ax"]) < 1e-12 and abs(r["pot"][2] - G["C_phi"]) < 1e-12
+
+
+def test_softened_quadrupole_off_axis_golden():
+    """Off axis: exercises Q r with two components and the mixed geometry at eps > 0."""
+    G, O = _two_mass_field([0.5, 0.25, 0])
+    r = O.forces(2.0, G["B_eps"])
+    assert r["n_pc"][2] == 1 and r["n_pp"][2] == 0
+    assert abs(r["acc"][2, 0] - G["B_ax"]) < 1e-14 and abs(r["acc"][2, 1] - G["B_ay"]) < 1e-14
+    assert abs(r["acc"][2, 2]) < 1e-18 and abs(r["pot"][2] - G["B_phi"]) < 1e-14
+
+
+@pytest.mark.parametrize("eps", [0.0, 0.1, 0.5])
+def test_particle_cell_acceleration_is_minus_gradient_of_its_potential(eps):
+    """O6 is self-consistent at any softening: a = -grad(phi) of the SAME cell term (central differences of the oracle's
+    potential over displaced field points).  A power of sigma wrong in a or in phi alone, or a wrong sign or
+    coefficient on Q r or (r^T Q r) r, breaks this by far more than the 1e-6 of the difference quotient."""
+    base = np.array([0.5, 0.25, 0.125])
+    hstep = 2.0 ** -10                                   # fp32-exact displacements
+    def phi_at(x):
+        pos = np.array([[-0.125, 0.03125, 0], [0.125, -0.03125, 0.03125], x], np.float32)
+        assert np.array_equal(pos[2].astype(np.float64), x)
+        O = oracle.Oracle(pos, np.array([1.0, 0.5, 1e-3], np.float32), 2)
+        r = O.forces(2.0, eps)
+        assert r["n_pc"][2] == 1 and r["n_pp"][2] == 0
+        return r["pot"][2], r["acc"][2]
+    _, a0 = phi_at(base)
+    grad = np.zeros(3)
+    for k in range(3):
+        e = np.zeros(3); e[k] = hstep
+        grad[k] = (phi_at(base + e)[0] - phi_at(base - e)[0]) / (2 * hstep)
+    assert np.linalg.norm(a0 + grad) / np.linalg.norm(a0) < 2e-5
+
+
 # ---------------------------------------------------------------- whole evaluation
 @pytest.mark.parametrize("n,n_leaf,n_group", [(1024, 16, 16), (4096, 16, 64), (777, 3, 3)])
 def test_theta_zero_equals_direct_sum(n, n_leaf, n_group):
