@@ -72,6 +72,9 @@ typedef struct tc_stats {
   double t_node_ms;       /* body-node evaluation kernel (List 3)                                   */
   double t_leaf_ms;       /* body-leaf evaluation kernel (List 4)                                   */
   int64_t list_bytes;     /* bytes of the global interaction lists                                  */
+  int64_t n_opened_total; /* of n_tests_total: tests that OPENED the cell (nodes walked on + leaves sent to the particle-particle
+                             list); the others put the cell on a group's cell list.  The paper's walk metric
+                             counts 16 bytes per test + 16 per opened cell.                 */
 } tc_stats;
 
 /* Select the current CUDA device, create the context and its stream.
@@ -105,8 +108,13 @@ int tc_build(tc_ctx* ctx, int n_leaf);
  *   device, in the CALLER's particle order.
  * Host pointers: synchronous on return.  Device pointers: stream-ordered on the
  * context's stream (tc_set_stream); errors of the kernel surface at tc_sync().
- * Errors: TC_ESTATE (tree not built / host-only), TC_EINVAL (theta < 0, eps < 0,
- * non-finite, acc NULL), TC_ECUDA, TC_EOVERFLOW.                                 */
+ * eps < 1e-10 is taken as eps = 0 (coincident pairs then contribute nothing): m / eps^3 of the self pair must stay
+ * finite in fp32; theta > 1e18 (theta^2 overflows fp32) is refused.  With eps > 0 every particle meets itself once
+ * (the term -m_i/eps is added to phi_i and taken out again in fp32), so phi_i carries an absolute error of about
+ * 6e-8 m_i/eps: negligible for N-body softening lengths (m/eps ~ 1e-4 at config 3), above the 1e-4 bar once
+ * m_i/eps > ~1e3 |phi_i|.
+ * Errors: TC_ESTATE (tree not built / host-only / shard_count > 1: use tc_forces_shard), TC_EINVAL
+ * (theta < 0, theta > 1e18, eps < 0, non-finite, acc NULL), TC_ECUDA, TC_EOVERFLOW.                 */
 int tc_forces(tc_ctx* ctx, float theta, float eps, float* acc, float* pot);
 
 /* Options (double-valued).  Keys:
@@ -123,20 +131,13 @@ int tc_forces(tc_ctx* ctx, float theta, float eps, float* acc, float* pot);
  *                 still conservative, about 1 % fewer interactions.  Combines with "open_rule".
  *   "quadrupole"  1 (default: monopole + quadrupole) or 0: monopole-only cells (variant R22, the expansion of
  *                 the Hamada et al. code the paper compares with).
- *   "shard_count", "shard_rank"   multi-GPU sharding of ONE force evaluation (groups are independent
- *                 given the read-only tree): with shard_count = k > 1 tc_forces evaluates only the
- *                 groups at positions rank, rank + k, ... of the cost-ordered schedule.  acc, pot and the counts
- *                 of every particle OUTSIDE the shard are then ZERO on return, so the k shards (one context per
- *                 GPU, each holding the same particles and tree) combine by summation (one all-reduce); the
- *                 totals in tc_stats are per shard.  Default 1 / 0.  Fused kernel only (TC_EINVAL with two_pass).
+ *   "shard_count", "shard_rank"   ONE force evaluation over k GPUs (tc_forces_shard below): this context is
+ *                 rank shard_rank of shard_count.  Default 1 / 0.
  *   "two_pass"    0 (default: the fused kernel) or 1: the paper-literal pipeline —
  *                 walk-count kernel, scan of the list sizes, walk-write kernel (lists in global memory),
  *                 body-node kernel, body-leaf kernel; same lists, same counts, same results up to
  *                 summation order; an A/B against the fused design, timed per kernel in tc_stats.
- *   "walk_only"   measurement aid, 0 (default) or 1: tc_forces walks the tree and builds every interaction
- *                 list (A1-A3) but skips their evaluation; acc and pot are then ZERO, counts and
- *                 n_tests_total are valid.  bench.py uses it to report the paper's second metric, the
- *                 data rate of the tree walk.
+ *   "walk_only"   measurement aid of bench.py, documented in include/tc_bench.h
  *   "stack_smem"  walk-stack entries kept in shared memory per warp before
  *                 spilling to global memory: 256 (default) or 64 (test of the
  *                 spill path)
@@ -210,13 +211,31 @@ int tc_get_group_boxes(tc_ctx* ctx, float* half_ext);
  * TC_ENOMEM, TC_ECUDA.                                                                              */
 int tc_direct(tc_ctx* ctx, float eps, const int64_t* targets, int64_t n_targets, double* acc, double* pot);
 
-/* Measured FP32 peak of the current device: an FFMA-only microbenchmark (16 independent
- * fma.rn.f32 chains per thread, 8 CTAs of 256 threads per SM, CUDA events on the context's
- * stream).  *tflops = 2 flops x FFMA lane-instructions / time.  This is the denominator the
- * roofline of bench.py quotes beside the nominal SMs x 128 lanes x 2 x clock: the
- * force kernel is bound by FP32 issue, not by HBM or tensor throughput (PAPER.md:175 measures
- * "instruction throughput" the same way).  Errors: TC_ESTATE (host-only), TC_EINVAL, TC_ECUDA.  */
-int tc_fp32_peak(tc_ctx* ctx, double* tflops);
+/* ---- ONE force evaluation over k GPUs ------------------------------------
+ * Groups are independent given the read-only tree (one walk per group, nothing is exchanged between
+ * groups), so the path shards without any collective inside the walk or the evaluation.  One context per GPU, each
+ * with the SAME particles, options and tree, and options "shard_count" = k, "shard_rank" = r.  Rank r evaluates the
+ * groups at positions r, r + k, ... of the cost-ordered schedule (neighbours in the schedule cost the same: balanced)
+ * and writes ONLY its own particles, compactly: one row (ax, ay, az, phi) per particle, its groups in schedule order,
+ * particles in tree order inside a group.  The caller all-gathers the rows of all ranks (16 bytes per particle in
+ * total — the one exchange of the path; NCCL all-gather) and tc_shard_scatter puts them in the caller's particle order.
+ *
+ * tc_shard_size:    *n_slots = rows every rank contributes = max over ranks of the particles a rank evaluates
+ *                   (the same number on every rank; rows beyond a rank's own count are never written).
+ * tc_forces_shard:  A1-A6 for this rank's groups.  out4 [n_slots,4] fp32 and cnt2 [n_slots,2] int32 ((n_pc, n_pp) per
+ *                   row) or NULL: DEVICE buffers of the caller, stream-ordered.  theta, eps as tc_forces.  The totals
+ *                   in tc_stats are those of the shard; tc_get_counts is not valid after a shard (TC_ESTATE).
+ * tc_shard_scatter: gathered4 [k, n_slots, 4] (rank-major, as an all-gather delivers it) and gathered_cnt2
+ *                   [k, n_slots, 2] or NULL -> acc [n,3], pot [n] or NULL, n_pc / n_pp [n] or NULL in the CALLER's
+ *                   particle order.  All DEVICE buffers, stream-ordered.  With k = 1 the pair
+ *                   tc_forces_shard + tc_shard_scatter gives bit for bit the result of tc_forces; for k > 1 too:
+ *                   every particle is computed by exactly one rank with the arithmetic of the single-GPU launch.
+ * Errors: TC_ESTATE (no tree / host-only), TC_EINVAL (null or host pointer, shard_rank >= shard_count, two_pass),
+ * TC_ENOMEM, TC_ECUDA, TC_EOVERFLOW.                                                                              */
+int tc_shard_size(tc_ctx* ctx, int64_t* n_slots);
+int tc_forces_shard(tc_ctx* ctx, float theta, float eps, float* out4, int32_t* cnt2);
+int tc_shard_scatter(tc_ctx* ctx, const float* gathered4, const int32_t* gathered_cnt2, float* acc, float* pot,
+                     int32_t* n_pc, int32_t* n_pp);
 
 #ifdef __cplusplus
 }

@@ -23,10 +23,11 @@ LIB_PATH = os.environ.get("TC_B200_LIB") or os.path.join(_HERE, "libtc_b200.so")
 TC_OK, TC_EINVAL, TC_ESTATE, TC_ECUDA, TC_ENOMEM, TC_EOVERFLOW = 0, -1, -2, -3, -4, -5
 TC_FLAG_HOST_ONLY = 1
 
-#: every symbol include/tc.h declares (checked by tests/test_abi.py)
+#: every symbol include/tc.h and include/tc_bench.h declare (checked by tests/test_abi.py)
 SYMBOLS = ["tc_create", "tc_create_ex", "tc_destroy", "tc_set_particles", "tc_build", "tc_forces",
            "tc_set_option", "tc_get_counts", "tc_get_stats", "tc_set_stream", "tc_sync",
-           "tc_last_error", "tc_get_tree", "tc_get_group_boxes", "tc_leapfrog", "tc_fp32_peak", "tc_direct"]
+           "tc_last_error", "tc_get_tree", "tc_get_group_boxes", "tc_leapfrog", "tc_fp32_peak", "tc_direct",
+           "tc_shard_size", "tc_forces_shard", "tc_shard_scatter"]
 
 
 class tc_stats(C.Structure):
@@ -36,7 +37,7 @@ class tc_stats(C.Structure):
                 ("n_spills", C.c_int64), ("t_host_ms", C.c_double), ("t_copy_ms", C.c_double),
                 ("t_gpu_ms", C.c_double), ("tree_bytes", C.c_int64),
                 ("t_walk_count_ms", C.c_double), ("t_walk_write_ms", C.c_double), ("t_node_ms", C.c_double),
-                ("t_leaf_ms", C.c_double), ("list_bytes", C.c_int64)]
+                ("t_leaf_ms", C.c_double), ("list_bytes", C.c_int64), ("n_opened_total", C.c_int64)]
 
     def asdict(self):
         return {k: getattr(self, k) for k, _ in self._fields_ if k != "reserved"}
@@ -82,21 +83,37 @@ def lib():
     L.tc_leapfrog.argtypes = [vp, vp, vp, vp, i64, f32, i32, i32, f32, f32, vp, vp, i32]
     L.tc_fp32_peak.argtypes = [vp, C.POINTER(C.c_double)]
     L.tc_direct.argtypes = [vp, f32, vp, i64, vp, vp]
+    L.tc_shard_size.argtypes = [vp, C.POINTER(C.c_int64)]
+    L.tc_forces_shard.argtypes = [vp, f32, f32, vp, vp]
+    L.tc_shard_scatter.argtypes = [vp, vp, vp, vp, vp, vp, vp]
     _lib = L
     return L
 
 
-def _ptr(a):
-    """Raw pointer of a numpy array (host) or a torch tensor (host or device); None -> NULL."""
+def _ptr(a, dtype=None, shape=None, name="buffer"):
+    """Raw pointer of a numpy array (host) or a torch tensor (host or device); None -> NULL.
+
+    `dtype` (numpy dtype) and `shape` (tuple, None = any extent) are CHECKED before the C call: the library sees
+    plain pointers and would reinterpret a float64 array, or a [3,n] one, byte by byte."""
     if a is None:
         return None
     if isinstance(a, np.ndarray):
-        assert a.flags["C_CONTIGUOUS"], "array must be C-contiguous"
-        return C.c_void_p(a.ctypes.data)
-    if hasattr(a, "data_ptr"):
-        assert a.is_contiguous(), "tensor must be contiguous"
-        return C.c_void_p(a.data_ptr())
-    raise TypeError(f"unsupported buffer type {type(a)}")
+        if not a.flags["C_CONTIGUOUS"]:
+            raise TypeError(f"{name}: array must be C-contiguous")
+        got, p = a.dtype, C.c_void_p(a.ctypes.data)
+    elif hasattr(a, "data_ptr"):
+        if not a.is_contiguous():
+            raise TypeError(f"{name}: tensor must be contiguous")
+        got, p = np.dtype(str(a.dtype).replace("torch.", "")), C.c_void_p(a.data_ptr())
+    else:
+        raise TypeError(f"{name}: unsupported buffer type {type(a)}")
+    if dtype is not None and got != np.dtype(dtype):
+        raise TypeError(f"{name}: dtype must be {np.dtype(dtype)}, got {got}")
+    if shape is not None:
+        sh = tuple(a.shape)
+        if len(sh) != len(shape) or any(w is not None and int(w) != int(g) for w, g in zip(shape, sh)):
+            raise TypeError(f"{name}: shape must be {tuple('n' if w is None else w for w in shape)}, got {sh}")
+    return p
 
 
 def _check(ctx, rc):
@@ -118,7 +135,7 @@ def tc_destroy(ctx):
 
 def tc_set_particles(ctx, pos, mass, n=None):
     n = int(pos.shape[0]) if n is None else int(n)
-    _check(ctx, lib().tc_set_particles(ctx, _ptr(pos), _ptr(mass), n))
+    _check(ctx, lib().tc_set_particles(ctx, _ptr(pos, np.float32, (None, 3), "pos"), _ptr(mass, np.float32, (pos.shape[0],), "mass"), n))
 
 
 def tc_build(ctx, n_leaf: int):
@@ -126,7 +143,8 @@ def tc_build(ctx, n_leaf: int):
 
 
 def tc_forces(ctx, theta: float, eps: float, acc, pot=None):
-    _check(ctx, lib().tc_forces(ctx, float(theta), float(eps), _ptr(acc), _ptr(pot)))
+    _check(ctx, lib().tc_forces(ctx, float(theta), float(eps), _ptr(acc, np.float32, (None, 3), "acc"),
+                                _ptr(pot, np.float32, (acc.shape[0],), "pot")))
 
 
 def tc_set_option(ctx, key: str, value: float):
@@ -174,8 +192,11 @@ def tc_get_group_boxes(ctx) -> np.ndarray:
 def tc_leapfrog(ctx, pos, vel, mass, dt: float, steps: int, n_leaf: int, theta: float, eps: float, acc, pot=None,
                 have_acc: bool = False):
     """`steps` KDK steps on the device; pos, vel, mass, acc, pot are torch CUDA tensors updated in place."""
-    _check(ctx, lib().tc_leapfrog(ctx, _ptr(pos), _ptr(vel), _ptr(mass), int(mass.shape[0]), float(dt), int(steps),
-                                  int(n_leaf), float(theta), float(eps), _ptr(acc), _ptr(pot), int(bool(have_acc))))
+    n = int(mass.shape[0])
+    _check(ctx, lib().tc_leapfrog(ctx, _ptr(pos, np.float32, (n, 3), "pos"), _ptr(vel, np.float32, (n, 3), "vel"),
+                                  _ptr(mass, np.float32, (n,), "mass"), n, float(dt), int(steps), int(n_leaf), float(theta),
+                                  float(eps), _ptr(acc, np.float32, (n, 3), "acc"), _ptr(pot, np.float32, (n,), "pot"),
+                                  int(bool(have_acc))))
 
 
 def tc_direct(ctx, eps: float, targets, acc, pot=None):
@@ -183,7 +204,30 @@ def tc_direct(ctx, eps: float, targets, acc, pot=None):
     nt = 0 if targets is None else int(len(targets))
     if targets is not None:
         assert isinstance(targets, np.ndarray) and targets.dtype == np.int64, "targets must be a host int64 array"
-    _check(ctx, lib().tc_direct(ctx, float(eps), _ptr(targets), nt, _ptr(acc), _ptr(pot)))
+    _check(ctx, lib().tc_direct(ctx, float(eps), _ptr(targets, np.int64, (nt,), "targets"), nt, _ptr(acc, np.float64, (None, 3), "acc"),
+                                _ptr(pot, np.float64, (acc.shape[0],), "pot")))
+
+
+def tc_shard_size(ctx) -> int:
+    """Rows every rank contributes to the all-gather of a sharded evaluation (options shard_count / shard_rank)."""
+    v = C.c_int64(0)
+    _check(ctx, lib().tc_shard_size(ctx, C.byref(v)))
+    return int(v.value)
+
+
+def tc_forces_shard(ctx, theta: float, eps: float, out4, cnt2=None):
+    """This rank's shard into compact DEVICE rows out4 [n_slots,4] (+ cnt2 [n_slots,2] int32)."""
+    _check(ctx, lib().tc_forces_shard(ctx, float(theta), float(eps), _ptr(out4, np.float32, (None, 4), "out4"),
+                                      _ptr(cnt2, np.int32, (out4.shape[0], 2), "cnt2")))
+
+
+def tc_shard_scatter(ctx, gathered4, gathered_cnt2, acc, pot=None, n_pc=None, n_pp=None):
+    """All-gathered rows [k,n_slots,4] (+ counts) -> acc / pot / counts in the caller's order (DEVICE tensors)."""
+    n = int(acc.shape[0])
+    _check(ctx, lib().tc_shard_scatter(ctx, _ptr(gathered4, np.float32, (None, None, 4), "gathered4"),
+                                       _ptr(gathered_cnt2, np.int32, tuple(gathered4.shape[:2]) + (2,), "gathered_cnt2"),
+                                       _ptr(acc, np.float32, (n, 3), "acc"), _ptr(pot, np.float32, (n,), "pot"),
+                                       _ptr(n_pc, np.int32, (n,), "n_pc"), _ptr(n_pp, np.int32, (n,), "n_pp")))
 
 
 def tc_fp32_peak(ctx) -> float:
@@ -248,6 +292,16 @@ class TreeCode:
 
     def counts(self):
         return tc_get_counts(self.ctx)
+
+    # one evaluation over k GPUs (include/tc.h, "ONE force evaluation over k GPUs"): this context is one rank
+    def shard_size(self) -> int:
+        return tc_shard_size(self.ctx)
+
+    def forces_shard(self, theta, eps, out4, cnt2=None):
+        tc_forces_shard(self.ctx, theta, eps, out4, cnt2)
+
+    def shard_scatter(self, gathered4, gathered_cnt2, acc, pot=None, n_pc=None, n_pp=None):
+        tc_shard_scatter(self.ctx, gathered4, gathered_cnt2, acc, pot, n_pc, n_pp)
 
     def stats(self):
         return tc_get_stats(self.ctx)

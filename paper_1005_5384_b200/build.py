@@ -12,8 +12,8 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libtc_b200.so")
-SOURCES = ["tc_api.cpp", "tc_build.cpp", "tc_kernels.cu", "tc_build_gpu.cu"]
-HEADERS = ["tc_internal.h", "tc_lanes.h", os.path.join("..", "..", "include", "tc.h")]
+SOURCES = ["tc_api.cpp", "tc_build.cpp", "tc_kernels.cu", "tc_build_gpu.cu", "tc_shard.cu"]
+HEADERS = ["tc_internal.h", "tc_lanes.h", os.path.join("..", "..", "include", "tc.h"), os.path.join("..", "..", "include", "tc_bench.h")]
 
 NVCC_FLAGS = [
     "-std=c++17", "-O3", "-lineinfo",

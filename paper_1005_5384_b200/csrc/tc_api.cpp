@@ -31,6 +31,8 @@ struct tc_ctx {
   bool two_pass = false;
   tc::TwoPassScratch tps;
   bool last_two_pass = false;
+  tc::ShardLayout shard;              // layout of the shards of one evaluation over shard_count ranks (tc_shard.cu)
+  bool counts_valid = false;          // d_npc / d_npp hold the counts of the last tc_forces (a shard writes them to its rows)
   // particles (host copy, caller order)
   std::vector<float4> xyzm;                 // the context's host copy of the particles: (x, y, z, m), caller's order
   bool bbox_valid = false;                  // bbox[] = per-axis min (0-2) and max (3-5) of xyzm, taken by the pass that copied it in
@@ -125,6 +127,7 @@ int collect(tc_ctx* c) {
   }
   c->stats.n_pc_total = (int64_t)h.n_pc_total; c->stats.n_pp_total = (int64_t)h.n_pp_total;
   c->stats.n_tests_total = (int64_t)h.n_tests_total; c->stats.n_spills = (int64_t)h.n_spills;
+  c->stats.n_opened_total = (int64_t)h.n_opened_total;
   if (h.overflow) {
     cudaMemset((char*)c->d_ctr + offsetof(tc::DeviceCounters, overflow), 0, sizeof(unsigned int));
   }
@@ -203,6 +206,7 @@ void tc_destroy(tc_ctx* c) {
     cudaFree(c->d_ctr); cudaFree(c->d_spill);
     c->dscr.release();
     c->tps.release();
+    c->shard.release();
     if (c->h_src) cudaFreeHost(c->h_src);
     cudaFree(c->d_flags); cudaFree(c->d_raw);
     cudaFree(c->d_src); cudaFree(c->d_tgt); cudaFree(c->d_dacc); cudaFree(c->d_dpot);
@@ -369,7 +373,7 @@ int tc_build(tc_ctx* c, int n_leaf) {
   if (!c) return TC_EINVAL;
   if (c->n < 1) return fail(c, TC_ESTATE, "tc_build: no particles (call tc_set_particles first)");
   if (n_leaf < 1) return fail(c, TC_EINVAL, "tc_build: n_leaf must be >= 1");
-  c->built = false; c->forces_done = false;
+  c->built = false; c->forces_done = false; c->shard.k = 0;
   if (!c->host_only) TC_CUDA(c, cudaStreamSynchronize(c->stream));  // the pinned buffer may still be in flight
   if (c->device_build) {
     { const int rc = ensure_src(c); if (rc != TC_OK) return rc; }
@@ -424,18 +428,36 @@ int tc_build(tc_ctx* c, int n_leaf) {
   return TC_OK;
 }
 
-int tc_forces(tc_ctx* c, float theta, float eps, float* acc, float* pot) {
-  if (!c) return TC_EINVAL;
-  if (c->host_only) return fail(c, TC_ESTATE, "tc_forces: host-only context has no device (there is no CPU fallback)");
-  if (!c->built) return fail(c, TC_ESTATE, "tc_forces: no tree (call tc_build first)");
-  if (!acc) return fail(c, TC_EINVAL, "tc_forces: acc is null");
+namespace {
+// theta and eps as the kernels may take them.  eps < kEpsMin is eps = 0: the self pair and coincident pairs
+// have s^2 = eps^2, and m / eps^3 must stay finite in fp32 for their (zero) contribution m d / s^3 not to become
+// inf * 0 = NaN (a subnormal eps^2 is even flushed to 0 by rsqrt.approx.ftz and gives inf at once); fp32 coordinates
+// cannot resolve separations below 1e-10 anyway unless |x| < 1e-3.  theta whose square overflows fp32 is refused
+// (d^2 theta^2 = 0 * inf = NaN would leave a group's own ancestors un-opened).
+constexpr float kEpsMin = 1e-10f;
+int check_theta_eps(tc_ctx* c, const char* who, float theta, float& eps) {
   if (!(theta >= 0.f) || !std::isfinite(theta) || !(eps >= 0.f) || !std::isfinite(eps))
-    return fail(c, TC_EINVAL, "tc_forces: theta and eps must be finite and >= 0");
-  if (c->shard_count > 1 && c->shard_rank >= c->shard_count) return fail(c, TC_EINVAL, "tc_forces: shard_rank must be < shard_count");
-  if (c->shard_count > 1 && c->two_pass) return fail(c, TC_EINVAL, "tc_forces: sharding runs the fused kernel only (two_pass must be 0)");
+    return fail(c, TC_EINVAL, std::string(who) + ": theta and eps must be finite and >= 0");
+  if (theta > 1e18f) return fail(c, TC_EINVAL, std::string(who) + ": theta must be <= 1e18 (theta^2 overflows fp32)");
+  if (eps < kEpsMin) eps = 0.f;
+  return TC_OK;
+}
+
+// A1-A6 on the context's stream.  shard_out4 == nullptr: the whole evaluation into acc / pot (host or device, caller's
+// order).  shard_out4 != nullptr (device [n_slots,4]): this rank's shard into compact rows (tc_forces_shard).
+int forces_impl(tc_ctx* c, const char* who, float theta, float eps, float* acc, float* pot, float* shard_out4, int32_t* shard_cnt2) {
+  if (c->host_only) return fail(c, TC_ESTATE, std::string(who) + ": host-only context has no device (there is no CPU fallback)");
+  if (!c->built) return fail(c, TC_ESTATE, std::string(who) + ": no tree (call tc_build first)");
+  { const int rc = check_theta_eps(c, who, theta, eps); if (rc != TC_OK) return rc; }
+  const bool shard = shard_out4 != nullptr;
   const int64_t n = c->n;
-  const bool acc_dev = is_device_ptr(c, acc), pot_dev = pot ? is_device_ptr(c, pot) : acc_dev;
-  if (pot && acc_dev != pot_dev) return fail(c, TC_EINVAL, "tc_forces: acc and pot must both be host or both be device pointers");
+  bool acc_dev = true;
+  if (!shard) {
+    if (!acc) return fail(c, TC_EINVAL, std::string(who) + ": acc is null");
+    acc_dev = is_device_ptr(c, acc);
+    const bool pot_dev = pot ? is_device_ptr(c, pot) : acc_dev;
+    if (pot && acc_dev != pot_dev) return fail(c, TC_EINVAL, std::string(who) + ": acc and pot must both be host or both be device pointers");
+  }
   if (c->cnt_cap < n) {
     cudaFree(c->d_npc); cudaFree(c->d_npp); c->d_npc = c->d_npp = nullptr; c->cnt_cap = 0;
     TC_CUDA(c, cudaMalloc((void**)&c->d_npc, sizeof(int32_t) * (size_t)n));
@@ -461,12 +483,9 @@ int tc_forces(tc_ctx* c, float theta, float eps, float* acc, float* pot) {
   L.n_pc = c->d_npc; L.n_pp = c->d_npp; L.counters = c->d_ctr; L.spill = c->d_spill; L.spill_cap = c->spill_cap;
   L.stack_smem = c->stack_smem; L.n_sm = c->n_sm; L.flags = (c->walk_only ? 1 : 0) | (c->open_rule ? 2 : 0) | (c->quadrupole ? 0 : 4) | (c->group_box ? 8 : 0);
   L.max_grid = (int)(warps / (size_t)tc::forces_warps_per_cta());
-  L.shard_rank = c->shard_count > 1 ? c->shard_rank : 0; L.shard_count = c->shard_count;
-  if (c->shard_count > 1) {   // entries outside the shard are ZERO, so the shards of all ranks combine by summation
-    TC_CUDA(c, cudaMemsetAsync(L.acc, 0, sizeof(float) * 3 * (size_t)n, c->stream));
-    if (L.pot) TC_CUDA(c, cudaMemsetAsync(L.pot, 0, sizeof(float) * (size_t)n, c->stream));
-    TC_CUDA(c, cudaMemsetAsync(L.n_pc, 0, sizeof(int32_t) * (size_t)n, c->stream));
-    TC_CUDA(c, cudaMemsetAsync(L.n_pp, 0, sizeof(int32_t) * (size_t)n, c->stream));
+  if (shard) {
+    L.shard_rank = c->shard_rank; L.shard_count = c->shard_count;
+    L.shard_out4 = shard_out4; L.shard_cnt2 = shard_cnt2; L.shard_off = c->shard.off;
   }
   // stream-ordered: no host synchronisation between queued calls; the overflow flag is sticky until collect()
   TC_CUDA(c, cudaMemsetAsync(c->d_ctr, 0, offsetof(tc::DeviceCounters, overflow), c->stream));
@@ -475,7 +494,7 @@ int tc_forces(tc_ctx* c, float theta, float eps, float* acc, float* pot) {
   if (le != 0) return cuda_fail(c, (cudaError_t)le, "forces kernel launch");
   c->last_two_pass = c->two_pass;
   TC_CUDA(c, cudaEventRecord(c->ev1, c->stream));
-  c->timing_pending = true; c->forces_done = true;
+  c->timing_pending = true; c->forces_done = true; c->counts_valid = !shard;
   if (!acc_dev) {
     TC_CUDA(c, cudaMemcpyAsync(acc, c->d_acc, sizeof(float) * 3 * (size_t)n, cudaMemcpyDeviceToHost, c->stream));
     if (pot) TC_CUDA(c, cudaMemcpyAsync(pot, c->d_pot, sizeof(float) * (size_t)n, cudaMemcpyDeviceToHost, c->stream));
@@ -485,9 +504,61 @@ int tc_forces(tc_ctx* c, float theta, float eps, float* acc, float* pot) {
   return TC_OK;
 }
 
+// the shard layout of the built tree for the current shard_count (built on first use, kept until tc_build)
+int ensure_shard_layout(tc_ctx* c, const char* who) {
+  if (c->host_only) return fail(c, TC_ESTATE, std::string(who) + ": host-only context has no device");
+  if (!c->built) return fail(c, TC_ESTATE, std::string(who) + ": no tree (call tc_build first)");
+  if (c->shard_rank >= c->shard_count) return fail(c, TC_EINVAL, std::string(who) + ": shard_rank must be < shard_count");
+  if (c->shard.k == c->shard_count) return TC_OK;
+  const int e = tc::build_shard_layout(c->dview, c->shard_count, c->shard, c->stream);
+  if (e != 0) return cuda_fail(c, (cudaError_t)e, "shard layout");
+  return TC_OK;
+}
+}  // namespace
+
+int tc_forces(tc_ctx* c, float theta, float eps, float* acc, float* pot) {
+  if (!c) return TC_EINVAL;
+  if (c->shard_count > 1)
+    return fail(c, TC_ESTATE, "tc_forces: shard_count > 1 — a shard of a multi-GPU evaluation is computed by tc_forces_shard");
+  return forces_impl(c, "tc_forces", theta, eps, acc, pot, nullptr, nullptr);
+}
+
+int tc_shard_size(tc_ctx* c, int64_t* n_slots) {
+  if (!c || !n_slots) return fail(c, TC_EINVAL, "tc_shard_size: null argument");
+  const int rc = ensure_shard_layout(c, "tc_shard_size");
+  if (rc != TC_OK) return rc;
+  *n_slots = (int64_t)c->shard.n_slots;
+  return TC_OK;
+}
+
+int tc_forces_shard(tc_ctx* c, float theta, float eps, float* out4, int32_t* cnt2) {
+  if (!c) return TC_EINVAL;
+  if (!out4) return fail(c, TC_EINVAL, "tc_forces_shard: out4 is null");
+  if (c->two_pass) return fail(c, TC_EINVAL, "tc_forces_shard: sharding runs the fused kernel only (two_pass must be 0)");
+  if (!c->host_only && (!is_device_ptr(c, out4) || (cnt2 && !is_device_ptr(c, cnt2))))
+    return fail(c, TC_EINVAL, "tc_forces_shard: out4 and cnt2 must be device pointers");
+  const int rc = ensure_shard_layout(c, "tc_forces_shard");
+  if (rc != TC_OK) return rc;
+  return forces_impl(c, "tc_forces_shard", theta, eps, nullptr, nullptr, out4, cnt2);
+}
+
+int tc_shard_scatter(tc_ctx* c, const float* gathered4, const int32_t* gathered_cnt2, float* acc, float* pot, int32_t* n_pc,
+                     int32_t* n_pp) {
+  if (!c) return TC_EINVAL;
+  if (!gathered4 || !acc) return fail(c, TC_EINVAL, "tc_shard_scatter: gathered4 and acc must not be null");
+  const int rc = ensure_shard_layout(c, "tc_shard_scatter");
+  if (rc != TC_OK) return rc;
+  for (const void* p : {(const void*)gathered4, (const void*)gathered_cnt2, (const void*)acc, (const void*)pot, (const void*)n_pc, (const void*)n_pp})
+    if (p && !is_device_ptr(c, p)) return fail(c, TC_EINVAL, "tc_shard_scatter: all buffers must be device pointers");
+  const int e = tc::launch_shard_scatter(c->dview, c->shard, gathered4, gathered_cnt2, acc, pot, n_pc, n_pp, c->stream);
+  if (e != 0) return cuda_fail(c, (cudaError_t)e, "shard scatter");
+  return TC_OK;
+}
+
 int tc_get_counts(tc_ctx* c, int32_t* n_pc, int32_t* n_pp) {
   if (!c) return TC_EINVAL;
   if (!c->forces_done) return fail(c, TC_ESTATE, "tc_get_counts: no tc_forces since the last tc_build");
+  if (!c->counts_valid) return fail(c, TC_ESTATE, "tc_get_counts: the last evaluation was a shard (its counts are in the cnt2 rows of tc_forces_shard)");
   TC_CUDA(c, cudaStreamSynchronize(c->stream));
   if (n_pc) TC_CUDA(c, cudaMemcpy(n_pc, c->d_npc, sizeof(int32_t) * (size_t)c->n, cudaMemcpyDeviceToHost));
   if (n_pp) TC_CUDA(c, cudaMemcpy(n_pp, c->d_npp, sizeof(int32_t) * (size_t)c->n, cudaMemcpyDeviceToHost));
@@ -508,6 +579,7 @@ int tc_direct(tc_ctx* c, float eps, const int64_t* targets, int64_t n_targets, d
   if (c->n < 1) return fail(c, TC_ESTATE, "tc_direct: no particles (call tc_set_particles first)");
   if (!acc) return fail(c, TC_EINVAL, "tc_direct: acc is null");
   if (!(eps >= 0.f) || !std::isfinite(eps)) return fail(c, TC_EINVAL, "tc_direct: eps must be finite and >= 0");
+  if (eps < 1e-10f) eps = 0.f;   // as tc_forces (check_theta_eps): m / eps^3 of the self pair must stay finite
   const int64_t n = c->n;
   const int64_t nt = targets ? n_targets : n;
   if (nt < 1) return fail(c, TC_EINVAL, "tc_direct: n_targets must be >= 1");

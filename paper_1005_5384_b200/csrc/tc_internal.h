@@ -9,6 +9,7 @@
 #include <vector_functions.h>  // float4 / int4 / make_float4 (CUDA toolkit header, host-safe)
 
 #include "../../include/tc.h"
+#include "../../include/tc_bench.h"
 
 namespace tc {
 
@@ -89,6 +90,7 @@ struct DeviceCounters {
   unsigned long long n_pp_total;
   unsigned long long n_tests_total;
   unsigned long long n_spills;
+  unsigned long long n_opened_total;
   unsigned int next_group;  // dynamic work counter (persistent warps)
   unsigned int overflow;    // != 0: a spill stack overflowed -> TC_EOVERFLOW
 };
@@ -107,7 +109,31 @@ struct ForceLaunch {
   int n_sm = 148;
   int max_grid = 0;           // CTAs the spill buffer has room for (0: no limit)
   int shard_rank = 0, shard_count = 1;   // this launch runs schedule positions rank, rank + count, ... (fused kernel)
+  // shard of a multi-GPU evaluation: compact rows instead of the caller's order (all three set, or none)
+  float* shard_out4 = nullptr;           // device [n_slots,4]  (ax, ay, az, phi)
+  int32_t* shard_cnt2 = nullptr;         // device [n_slots,2]  (n_pc, n_pp) or nullptr
+  const int32_t* shard_off = nullptr;    // device [n_groups] by schedule position: first row of the group in its rank's shard
 };
+
+// Layout of the shards of ONE evaluation over k ranks: rank r evaluates the schedule positions
+// r, r + k, ...; its rows are its groups in that order, particles in tree order inside a group.
+//   off [i]  (i = schedule position)   first row of group sched[i] inside the shard of rank i % k
+//   slot[t]  (t = tree-order particle) row of particle t in the all-gathered buffer [k, n_slots]: (i % k) n_slots + off[i] + ...
+// Scratch owned by the context, grow-only.
+struct ShardLayout {
+  int32_t *off = nullptr, *slot = nullptr, *cnt = nullptr, *scan = nullptr;
+  size_t cap_off = 0, cap_slot = 0, cap_cnt = 0, cap_scan = 0;
+  char* tmp = nullptr; size_t cap_tmp = 0;
+  int k = 0;                 // the layout was built for this shard_count (0: none)
+  long long n_slots = 0;     // rows per rank in the gathered buffer = max over ranks of the particles a rank evaluates
+  void release();
+};
+// builds L for k ranks on `stream` (synchronises it once to read the k shard sizes).  cudaError_t as int.
+int build_shard_layout(const DeviceTree& T, int k, ShardLayout& L, void* stream);
+// gathered [k, n_slots, 4] (+ gathered_cnt [k, n_slots, 2] or nullptr) -> acc [n,3], pot [n] or nullptr, n_pc / n_pp [n] or nullptr,
+// all DEVICE, in the caller's order.  cudaError_t as int.
+int launch_shard_scatter(const DeviceTree& T, const ShardLayout& L, const float* gathered, const int32_t* gathered_cnt, float* acc,
+                         float* pot, int32_t* n_pc, int32_t* n_pp, void* stream);
 
 // Launches the fused walk+evaluate kernel on `stream` (a cudaStream_t).  Returns a
 // cudaError_t as int (0 = success).  Defined in tc_kernels.cu.

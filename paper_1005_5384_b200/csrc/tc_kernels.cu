@@ -44,6 +44,9 @@ namespace {
 #define TC_WALKB 2
 #endif
 constexpr int kWalkB = TC_WALKB;   // batches of 4 nodes (32 child tests) per walk iteration
+#ifndef TC_BULK_BODIES
+#define TC_BULK_BODIES 0         // 1: stage opened-leaf bodies with cp.async.bulk (1-D TMA) + mbarrier instead of ldg + sts
+#endif
 #ifndef TC_UNROLL2_MAXK
 #define TC_UNROLL2_MAXK 2   // particle-cell loop: two records in flight up to this many particles per lane
 #endif
@@ -86,6 +89,10 @@ struct __align__(16) WarpSmem {
   } u;
   int2 leafq[kLeafQCap];         // (first_body, n_body)
   uint32_t stack[STK];           // nodes to expand: first_child << 3 | (n_child - 1)
+#if TC_BULK_BODIES
+  unsigned long long mbar;       // mbarrier of the bulk copies that stage opened-leaf bodies (A/B of DESIGN.md section 6)
+  unsigned long long pad_;
+#endif
 };
 
 // Lane mapping of a pass over m particles (tc_lanes.h): S slices x q columns, K particles per lane
@@ -311,9 +318,13 @@ __device__ __forceinline__ void eval_cells(const CellRec* rec, int cnt, float ep
 
 // Opened leaves (List 4): flatten the queued (first, n) ranges into
 // body indices, gather the bodies with one coalesced float4 load per lane, evaluate.
+// mbar != nullptr (build with TC_BULK_BODIES): the ranges are contiguous runs of 16-byte records, so every lane
+// moves its range with ONE cp.async.bulk (1-D TMA copy, no register staging) completing on the warp's mbarrier.
+[[maybe_unused]] __device__ __forceinline__ unsigned smem_u32(const void* p) { return (unsigned)__cvta_generic_to_shared(p); }
 template <bool kEps0>
 __device__ __forceinline__ void eval_leaves(BodyStage& bs, const int2* leafq, int nq, const float4* __restrict__ part,
-                                            float eps2, const Lanes& L, PassState& st, int lane) {
+                                            float eps2, const Lanes& L, PassState& st, int lane,
+                                            unsigned long long* mbar = nullptr, unsigned* phase = nullptr) {
   for (int r0 = 0; r0 < nq; r0 += 32) {
     int f = 0, n = 0;
     if (r0 + lane < nq) { const int2 r = leafq[r0 + lane]; f = r.x; n = r.y; }
@@ -324,11 +335,31 @@ __device__ __forceinline__ void eval_leaves(BodyStage& bs, const int2* leafq, in
     const int total = __shfl_sync(kFull, incl, 31);
     for (int base = 0; base < total; base += kBodyCap) {
       const int k0 = max(0, base - off), k1 = min(n, base + kBodyCap - off);
-      for (int k = k0; k < k1; k++) bs.bidx[off + k - base] = f + k;
-      __syncwarp();
       const int cnt = min(kBodyCap, total - base);
-      for (int t = lane; t < cnt; t += 32) bs.body[t] = __ldg(part + bs.bidx[t]);
-      __syncwarp();
+#if TC_BULK_BODIES
+      if (mbar) {
+        const unsigned bar = smem_u32(mbar);
+        // the generic-proxy accesses of the staging area (previous round, or the cell chunk) come before the async writes
+        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+        if (lane == 0) asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" :: "r"(bar), "r"(cnt * 16) : "memory");
+        __syncwarp();
+        if (k1 > k0)
+          asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                       :: "r"(smem_u32(bs.body + (off + k0 - base))), "l"(part + f + k0), "r"((k1 - k0) * 16), "r"(bar) : "memory");
+        unsigned ok;
+        do {
+          asm volatile("{ .reg .pred p; mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2; selp.u32 %0, 1, 0, p; }"
+                       : "=r"(ok) : "r"(bar), "r"(*phase) : "memory");
+        } while (!ok);
+        *phase ^= 1u;
+      } else
+#endif
+      {
+        for (int k = k0; k < k1; k++) bs.bidx[off + k - base] = f + k;
+        __syncwarp();
+        for (int t = lane; t < cnt; t += 32) bs.body[t] = __ldg(part + bs.bidx[t]);
+        __syncwarp();
+      }
       eval_dispatch<kEvalBodies, kEps0>(bs.body, cnt, eps2, L, st);
       __syncwarp();
     }
@@ -362,7 +393,17 @@ __device__ __forceinline__ void setup_pass(Lanes& L, PassState& st, const float4
   }
 }
 
-// A6: reduce the slices of every particle, write back in the caller's order.
+// Where the results of a pass go.  Default: the caller's order (acc [n,3], pot [n], counts [n]).  A SHARD of a
+// multi-GPU evaluation writes (ax, ay, az, phi) rows and (n_pc, n_pp) pairs COMPACTLY instead,
+// row = the group's offset in this rank's shard + the particle's index in the group: only this rank's particles,
+// coalesced 16-byte stores, ready for one all-gather.
+struct ShardOut {
+  float4* out4 = nullptr;          // [n_slots] or nullptr (not a shard)
+  int2* cnt2 = nullptr;            // [n_slots] or nullptr
+  const int32_t* off = nullptr;    // [n_groups] by schedule position: first row of the group in its rank's shard
+};
+
+// A6: reduce the slices of every particle, write back in the caller's order (or into the shard's compact rows).
 // kAdd: add to what is already there (second evaluation kernel of the two-pass variant);
 // kSelf: the particles met themselves once in the particle-particle part (remove -m/eps again).
 template <bool kAdd, bool kSelf>
@@ -370,7 +411,7 @@ __device__ __forceinline__ void write_back(const Lanes& L, const PassState& st, 
                                            const int32_t* __restrict__ orig, int first, int m, float eps2, int lane,
                                            float* __restrict__ acc, float* __restrict__ pot, int32_t* __restrict__ out_cnt,
                                            int cnt_value, int32_t* __restrict__ out_cnt2 = nullptr, int cnt2_value = 0,
-                                           bool self_met = true) {
+                                           bool self_met = true, float4* __restrict__ rows = nullptr, int2* __restrict__ row_cnt = nullptr) {
 #pragma unroll
   for (int j = 0; j < kMaxK; j++) {
     if (j >= L.K) break;                             // warp-uniform
@@ -387,8 +428,13 @@ __device__ __forceinline__ void write_back(const Lanes& L, const PassState& st, 
     const int tq = j * L.q + lane;
     if (lane < L.q && tq < m) {
       const int t = first + tq;
-      const int i = __ldg(orig + t);
       if (kSelf && self_met) ph += __ldg(part + t).w * rsqrt_approx(eps2);     // the particle met itself once
+      if (!kAdd && rows) {                                                     // shard: compact rows, tree order inside the group
+        rows[tq] = make_float4(ax, ay, az, ph);
+        if (row_cnt) row_cnt[tq] = make_int2(cnt_value, cnt2_value);
+        continue;
+      }
+      const int i = __ldg(orig + t);
       float* a3 = acc + 3 * (size_t)i;
       if (kAdd) { a3[0] += ax; a3[1] += ay; a3[2] += az; if (pot) pot[i] += ph; }
       else { a3[0] = ax; a3[1] = ay; a3[2] = az; if (pot) pot[i] = ph; }
@@ -418,13 +464,25 @@ forces_kernel(const float4* __restrict__ bnd, const float4* __restrict__ xm, con
               const int4* __restrict__ grp, const float4* __restrict__ gbox, int n_groups, float theta, float eps,
               float* __restrict__ acc, float* __restrict__ pot, int32_t* __restrict__ out_npc,
               int32_t* __restrict__ out_npp, DeviceCounters* __restrict__ ctr, uint32_t* __restrict__ spill_all,
-              int spill_cap, int flags, ListIO lio, int shard_rank, int shard_count) {
+              int spill_cap, int flags, ListIO lio, int shard_rank, int shard_count, ShardOut sho) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   WarpSmem<STK>& sm = reinterpret_cast<WarpSmem<STK>*>(smem_raw)[warp];
   uint32_t* spill = spill_all + (size_t)(blockIdx.x * kWarpsPerCta + warp) * (size_t)spill_cap;
   const float eps2 = eps * eps;
   const float th2 = __fmul_rn(theta, theta);
+  unsigned long long* mbar = nullptr;
+  unsigned bulk_phase = 0;
+#if TC_BULK_BODIES
+  if (MODE == kFused) {
+    mbar = &sm.mbar;
+    if (lane == 0) {
+      asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" :: "r"(smem_u32(mbar)) : "memory");
+      asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    __syncwarp();
+  }
+#endif
   const unsigned lt_mask = (1u << lane) - 1u;
   const bool walk_only = flags & kFlagWalkOnly;
   const bool com_rule = !kPlain && (flags & kFlagComRule), mono = !kPlain && (flags & kFlagMonopole);
@@ -444,6 +502,7 @@ forces_kernel(const float4* __restrict__ bnd, const float4* __restrict__ xm, con
     // (neighbours in the cost-ordered schedule cost about the same, so the shards are balanced)
     if (g >= (n_groups - shard_rank + shard_count - 1) / shard_count) break;
     g = g * shard_count + shard_rank;
+    const int shard_row = sho.out4 ? __ldg(sho.off + g) : 0;   // first compact row of this group (shards only)
     g = __ldg(&grp[g].w);                    // schedule: costly groups first (tc_build)
     const int4 G = __ldg(grp + g);           // (cell, first_body, n_body, -)
     const float4 gb = __ldg(bnd + G.x);
@@ -601,14 +660,15 @@ forces_kernel(const float4* __restrict__ bnd, const float4* __restrict__ xm, con
             if (!walk_only) eval_cells<kEps0>(sm.u.cell, ccnt, eps2, L, ps, mono);
             ccnt = 0; __syncwarp();
           }
-          if (flush_leaves) { if (!walk_only) eval_leaves<kEps0>(sm.u.bs, sm.leafq, lq, part, eps2, L, ps, lane); lq = 0; __syncwarp(); }
+          if (flush_leaves) { if (!walk_only) eval_leaves<kEps0>(sm.u.bs, sm.leafq, lq, part, eps2, L, ps, lane, mbar, &bulk_phase); lq = 0; __syncwarp(); }
         }
         if (!walking) break;
       }
 
       if (MODE == kFused) {
         // ---- A6: reduce the slices of every particle, write back in the caller's order
-        write_back<false, !kEps0>(L, ps, part, orig, G.y + pb, m, eps2, lane, acc, pot, out_npc, n_pc, out_npp, n_pp - 1, self_met);
+        write_back<false, !kEps0>(L, ps, part, orig, G.y + pb, m, eps2, lane, acc, pot, out_npc, n_pc, out_npp, n_pp - 1, self_met,
+                                  sho.out4 ? sho.out4 + shard_row + pb : nullptr, sho.cnt2 ? sho.cnt2 + shard_row + pb : nullptr);
       } else if (MODE == kCount) {
         if (lane == 0) { lio.cnt_c[g] = (unsigned long long)n_pc; lio.cnt_l[g] = (unsigned long long)n_lr; lio.leaf_bodies[g] = (int)n_pp; }
       }
@@ -619,6 +679,7 @@ forces_kernel(const float4* __restrict__ bnd, const float4* __restrict__ xm, con
           atomicAdd(&ctr->n_pp_total, (unsigned long long)((n_pp - 1) * np));
           // opening tests EXECUTED by this walk: every tested child ends on the cell list or is opened
           atomicAdd(&ctr->n_tests_total, (unsigned long long)(n_pc + n_open));
+          atomicAdd(&ctr->n_opened_total, (unsigned long long)n_open);
         }
         if (n_spills) atomicAdd(&ctr->n_spills, (unsigned long long)n_spills);
         if (overflow) atomicExch(&ctr->overflow, 1u);
@@ -729,9 +790,11 @@ int launch_t(const DeviceTree& T, const ForceLaunch& L, cudaStream_t st, int* ct
   // persistent grid: every SM full, groups handed out by an atomic counter
   // (never more CTAs than the spill buffer was sized for: forces_total_warps)
   const int grid = L.max_grid > 0 ? std::min(L.n_sm * per_sm, L.max_grid) : L.n_sm * per_sm;
+  ShardOut sho;
+  sho.out4 = reinterpret_cast<float4*>(L.shard_out4); sho.cnt2 = reinterpret_cast<int2*>(L.shard_cnt2); sho.off = L.shard_off;
   kern<<<grid, kWarpsPerCta * 32, smem, st>>>(T.bnd, T.xm, T.q0, T.q1, T.part, T.orig, T.grp, T.gbox, (int)T.n_groups,
                                                L.theta, L.eps, L.acc, L.pot, L.n_pc, L.n_pp, L.counters, L.spill,
-                                               L.spill_cap, L.flags, lio, L.shard_rank, L.shard_count);
+                                               L.spill_cap, L.flags, lio, L.shard_rank, L.shard_count, sho);
   return (int)cudaGetLastError();
 }
 

@@ -26,16 +26,22 @@ def energy(mass, vel, pot):
 
 
 def leapfrog_kdk(tc: "B.TreeCode", pos, vel, mass, dt: float, steps: int, theta: float, eps: float,
-                 n_leaf: int = 16, log=None, native: bool = False):
+                 n_leaf: int = 16, log=None, native: bool = False, state: dict | None = None):
     """Advance (pos, vel) in place by `steps` KDK steps; returns a list of per-step dicts.
 
     v += a dt/2 ; x += v dt ; rebuild tree ; a = forces(x) ; v += a dt/2     (BASELINE.json config 5)
     Each entry: step, t_host_ms, t_copy_ms, t_gpu_ms (PAPER.md:155,165 split), wall_ms, E, dE_rel, |sum m v|.
+    `state`, if given, receives the accelerations and potentials of the last force evaluation (`acc`, `pot`).
+    The library works on its own stream: it is pointed at torch's current stream here, so that the torch
+    kicks / drift and the library's reads of `pos` are ordered (tc.h: device pointers are stream-ordered).
     """
+    tc.set_stream(torch.cuda.current_stream(pos.device).cuda_stream)
     n = pos.shape[0]
     dev = pos.device
     acc = torch.empty((n, 3), dtype=torch.float32, device=dev)
     pot = torch.empty(n, dtype=torch.float32, device=dev)
+    if state is not None:
+        state["acc"], state["pot"] = acc, pot
 
     def force():
         tc.set_particles(pos, mass)

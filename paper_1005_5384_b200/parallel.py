@@ -1,24 +1,23 @@
-"""ONE force evaluation over several GPUs (DESIGN.md §8, SURVEY.md 8(e)): one process per GPU, plumbing by
+"""ONE force evaluation over several GPUs (DESIGN.md section 8, SURVEY.md 8(e)): one process per GPU, plumbing by
 ``torch.distributed``.
 
 Groups are independent given the read-only tree (one walk per group, no communication between
 groups), so the path shards with NO collective inside the walk or the evaluation: every rank holds the same
-particles, builds the same tree (the device build takes ~1 ms at N = 2^20 — cheaper than broadcasting the
-37 MB packed tree), evaluates the groups at schedule positions rank, rank + world, ... (library options
-"shard_count" / "shard_rank": neighbours in the cost-ordered schedule cost the same, so the shards are
-balanced) and leaves ZEROS for every particle outside its shard.  The only exchange is the one that hands
-every rank the full result: one all-reduce (SUM) of acc and pot — over NCCL that is an NVSwitch in-switch
-reduction of 16 bytes per particle.  Adding zeros is exact, so the combined result is bit-for-bit the
-single-GPU result (tests/test_gpu_shard.py runs the shards one after the other on one GPU).
+particles and builds the same tree, rank r evaluates the groups at schedule positions r, r + world, ... (library
+options "shard_count" / "shard_rank"; neighbours in the cost-ordered schedule cost the same, so strided shards are
+balanced) and writes ONLY its own particles, as compact rows (ax, ay, az, phi).  The one exchange is the one that
+hands every rank the rows of the others: ONE all-gather of 16 bytes per particle (NCCL over NVLink / NVSwitch),
+then the library scatters the gathered rows to the caller's particle order (``tc_shard_scatter``).  Every particle
+is computed by exactly one rank with the arithmetic of the single-GPU launch, so the result is bit for bit the
+single-GPU result (tests/test_gpu_shard.py runs the shards one after the other on one GPU;
+tests/test_multirank_cpu.py runs this module's protocol over gloo with two processes).
 
-Marshalling only: all arithmetic is in the library's kernels or in the collective.
+Marshalling only: all arithmetic is in the library's kernels.
 """
 from __future__ import annotations
 
 import torch
 import torch.distributed as dist
-
-from . import binding as B
 
 
 def shard_of(rank: int, world: int, n_groups: int) -> range:
@@ -26,107 +25,47 @@ def shard_of(rank: int, world: int, n_groups: int) -> range:
     return range(rank, n_groups, world)
 
 
-def combine(acc: "torch.Tensor", pot: "torch.Tensor | None" = None, counts=(), group=None) -> None:
-    """Sum the zero-padded shard results of all ranks in place (every rank ends with the full arrays)."""
-    if not dist.is_initialized() or dist.get_world_size(group) == 1:
-        return
-    work = [dist.all_reduce(acc, op=dist.ReduceOp.SUM, group=group, async_op=True)]
-    if pot is not None:
-        work.append(dist.all_reduce(pot, op=dist.ReduceOp.SUM, group=group, async_op=True))
-    for c in counts:
-        work.append(dist.all_reduce(c, op=dist.ReduceOp.SUM, group=group, async_op=True))
-    for w in work:
-        w.wait()
+def all_gather_rows(rows: "torch.Tensor", group=None) -> "torch.Tensor":
+    """[n_slots, c] on every rank -> [world, n_slots, c], rank-major (the layout tc_shard_scatter reads)."""
+    world = dist.get_world_size(group) if dist.is_initialized() else 1
+    out = torch.empty((world * rows.shape[0],) + tuple(rows.shape[1:]), dtype=rows.dtype, device=rows.device)
+    if world == 1:
+        out.copy_(rows)
+    else:
+        dist.all_gather_into_tensor(out, rows, group=group)      # concatenation along dim 0 = rank-major
+    return out.view((world,) + tuple(rows.shape))
 
 
-def forces_sharded(tc: "B.TreeCode", theta: float, eps: float, acc: "torch.Tensor", pot: "torch.Tensor | None" = None,
-                   group=None) -> None:
-    """tc_forces of this rank's shard into the DEVICE tensors acc [n,3] / pot [n], then ``combine``.
+def forces_sharded(tc, theta: float, eps: float, acc: "torch.Tensor", pot: "torch.Tensor | None" = None, group=None,
+                   n_pc: "torch.Tensor | None" = None, n_pp: "torch.Tensor | None" = None, scratch: dict | None = None) -> None:
+    """This rank's shard, the all-gather, the scatter: acc [n,3] / pot [n] (and the counts, if asked for) end up
+    complete and in the caller's order on EVERY rank.  Device tensors; stream-ordered on torch's current stream
+    (the context must have been pointed at it with ``tc.set_stream``).
 
-    Every rank must have called set_particles / build with the same particles and options.
+    Every rank must have called set_particles / build with the same particles and options.  `tc` is a
+    ``binding.TreeCode`` (anything with set_option / shard_size / forces_shard / shard_scatter works: the CPU test
+    drives this function with a stand-in).  `scratch` keeps the row buffers between calls.
     """
     world = dist.get_world_size(group) if dist.is_initialized() else 1
     rank = dist.get_rank(group) if dist.is_initialized() else 0
     tc.set_option("shard_count", world)
     tc.set_option("shard_rank", rank)
     try:
-        B.tc_forces(tc.ctx, theta, eps, acc, pot)
-        tc.sync()
+        n_slots = tc.shard_size()
+        sc = scratch if scratch is not None else {}
+        rows = sc.get("rows")
+        if rows is None or rows.shape[0] != n_slots or rows.device != acc.device:
+            rows = sc["rows"] = torch.empty((n_slots, 4), dtype=torch.float32, device=acc.device)
+            sc["cnt"] = None
+        cnt = None
+        if n_pc is not None or n_pp is not None:
+            cnt = sc.get("cnt")
+            if cnt is None:
+                cnt = sc["cnt"] = torch.empty((n_slots, 2), dtype=torch.int32, device=acc.device)
+        tc.forces_shard(theta, eps, rows, cnt)
+        gathered = all_gather_rows(rows, group)
+        gathered_cnt = all_gather_rows(cnt, group) if cnt is not None else None
+        tc.shard_scatter(gathered, gathered_cnt, acc, pot, n_pc, n_pp)
     finally:
         tc.set_option("shard_count", 1)
         tc.set_option("shard_rank", 0)
-    combine(acc, pot, group=group)
-
-
-def main(argv=None) -> None:
-    """Strong-scaling timing of ONE config-3 force evaluation over the ranks of a torchrun launch:
-
-        python -m torch.distributed.run --nnodes=1 --nproc-per-node N --master-addr 127.0.0.1 \\
-            -m paper_1005_5384_b200.parallel --steps 10
-
-    Every rank holds the same particles and builds the same tree on its GPU; the timed region is the sharded
-    ``tc_forces`` plus the all-reduce, CUDA events on the launching stream, max over ranks.  Rank 0 prints one
-    JSON line.  (``bench.py`` keeps the weak-scaling contract: independent evaluations per rank, no collective.)
-    """
-    import argparse
-    import json
-    import os
-
-    import numpy as np
-
-    from . import build as tc_build
-    from . import inputs
-
-    ap = argparse.ArgumentParser()
-    ap.add_argument("--steps", type=int, default=10)
-    ap.add_argument("--warmup", type=int, default=3)
-    ap.add_argument("--workload", default="plummer_1m")
-    args = ap.parse_args(argv)
-    world = int(os.environ.get("WORLD_SIZE", "1"))
-    rank = int(os.environ.get("RANK", "0"))
-    local = int(os.environ.get("LOCAL_RANK", "0"))
-    torch.cuda.set_device(local)
-    dev = torch.device("cuda", local)
-    if world > 1:
-        dist.init_process_group("nccl", device_id=dev)
-    if rank == 0:
-        tc_build.build()
-    if world > 1:
-        dist.barrier()
-    pos, mass, theta, eps, n_leaf = inputs.make(args.workload)
-    n = len(mass)
-    stream = torch.cuda.Stream(device=dev)
-    with B.TreeCode() as tc, torch.cuda.stream(stream):
-        tc.set_stream(stream.cuda_stream)
-        tc.set_option("device_build", 1)
-        d_pos, d_mass = torch.from_numpy(pos).to(dev), torch.from_numpy(mass).to(dev)
-        acc = torch.empty((n, 3), dtype=torch.float32, device=dev)
-        pot = torch.empty(n, dtype=torch.float32, device=dev)
-        tc.set_particles(d_pos, d_mass)
-        tc.build(n_leaf)
-        ms = []
-        for i in range(args.warmup + args.steps):
-            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-            if world > 1:
-                dist.barrier()
-            a.record(stream)
-            forces_sharded(tc, theta, eps, acc, pot)
-            b.record(stream)
-            torch.cuda.synchronize()
-            t = torch.tensor([a.elapsed_time(b)], dtype=torch.float64, device=dev)
-            if world > 1:
-                dist.all_reduce(t, op=dist.ReduceOp.MAX)
-            if i >= args.warmup:
-                ms.append(float(t))
-        checksum = float(acc.double().abs().sum())
-    if rank == 0:
-        print(json.dumps({"what": "one force evaluation sharded over the ranks (groups strided over the cost-ordered schedule, "
-                                  "one all-reduce of acc and pot)", "workload": args.workload, "n": n, "n_gpus": world,
-                          "scaling": "strong", "ms_per_evaluation": float(np.mean(ms)), "ms_min": float(np.min(ms)),
-                          "checksum_abs_acc": checksum}))
-    if world > 1:
-        dist.destroy_process_group()
-
-
-if __name__ == "__main__":
-    main()

@@ -1,4 +1,4 @@
-"""The C-ABI library builds, loads and exports every symbol include/tc.h declares.
+"""The C-ABI library builds, loads and exports every symbol include/*.h declares.
 No compute call needs a GPU here; the host-only context covers call-order errors."""
 import os
 import re
@@ -18,7 +18,7 @@ def _built():
 
 
 def test_header_symbols_are_exported():
-    hdr = open(os.path.join(ROOT, "include", "tc.h")).read()
+    hdr = "".join(open(os.path.join(ROOT, "include", h)).read() for h in sorted(os.listdir(os.path.join(ROOT, "include"))))
     declared = set(re.findall(r"\b(tc_[a-z0-9_]+)\s*\(", hdr)) - {"tc_ctx"}
     assert declared == set(B.SYMBOLS), declared ^ set(B.SYMBOLS)
     L = B.lib()
@@ -27,9 +27,9 @@ def test_header_symbols_are_exported():
 
 
 def test_stats_struct_size_matches_header():
-    # 4 int64 + 4 int32 + 4 int64 + 3 double + 1 int64 + 4 double + 1 int64
+    # 4 int64 + 4 int32 + 4 int64 + 3 double + 1 int64 + 4 double + 2 int64
     import ctypes
-    assert ctypes.sizeof(B.tc_stats) == 4 * 8 + 4 * 4 + 4 * 8 + 3 * 8 + 8 + 4 * 8 + 8
+    assert ctypes.sizeof(B.tc_stats) == 4 * 8 + 4 * 4 + 4 * 8 + 3 * 8 + 8 + 4 * 8 + 2 * 8
 
 
 def test_no_cpu_fallback_host_only_refuses_forces():

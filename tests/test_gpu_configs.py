@@ -73,25 +73,51 @@ def test_config4_accuracy_versus_time_1m():
         assert rr[0]["median"] * 4 < rr[1]["median"]                 # 0.3 -> 0.5: at least (5/3)^3
     r05 = [r for r in rows if r["n_leaf"] == 16 and r["theta"] == 0.5][0]
     assert 2e-5 < r05["median"] < 4e-4                               # SURVEY 8(c) sanity band around 8.7e-5
-    # one oracle parity point away from the headline parameters, sampled groups
-    o = Oracle(pos, mass, 8, 64)
-    gsel = np.arange(7, o.n_groups, o.n_groups // 192, dtype=np.int64)
-    ref = o.forces(0.3, eps, shadow32=True, groups=gsel)
-    with B.TreeCode(n_group=64) as tc:
-        tc.set_particles(pos, mass)
-        tc.build(8)
-        acc, pot = tc.forces(0.3, eps)
-        n_pc, n_pp = tc.counts()
-    check(acc, pot, n_pc, n_pp, ref, ref["n_pc"] >= 0)
+
+
+def test_config4_oracle_parity_at_every_sweep_point_1m():
+    """Oracle parity on sampled groups at ALL twelve (theta, N_leaf) points of config 4, full size."""
+    pos, mass, _, eps, _ = inputs.make("plummer_1m")
+    for n_leaf in (8, 16, 32):
+        o = Oracle(pos, mass, n_leaf, 64)
+        gsel = np.arange(7 + n_leaf, o.n_groups, o.n_groups // 192, dtype=np.int64)
+        with B.TreeCode(n_group=64) as tc:
+            tc.set_particles(pos, mass)
+            tc.build(n_leaf)
+            for theta in (0.3, 0.5, 0.75, 1.0):
+                ref = o.forces(theta, eps, shadow32=True, groups=gsel)
+                acc, pot = tc.forces(theta, eps)
+                n_pc, n_pp = tc.counts()
+                sel = ref["n_pc"] >= 0
+                rel, prel = check(acc, pot, n_pc, n_pp, ref, sel)
+                print(f"config4 parity N_leaf={n_leaf:2d} theta={theta:4.2f}: {int(sel.sum())} particles of {len(gsel)} groups, "
+                      f"acc q99.9={np.quantile(rel, 0.999):.2e} max={rel.max():.2e} pot max={prel.max():.2e}")
+
+
+def _sampled_parity(tag, pos_host, mass, d_acc, d_pot, n_pc, n_pp, theta, eps, n_leaf, n_group, n_sample, seed):
+    """Oracle (own tree on these positions) on n_sample random groups against the library's result."""
+    o = Oracle(pos_host, mass, n_leaf, n_group)
+    gsel = np.sort(np.random.default_rng(seed).choice(o.n_groups, n_sample, replace=False)).astype(np.int64)
+    ref = o.forces(theta, eps, shadow32=True, groups=gsel, stats=True)
+    shape = (o.n_cells, o.n_leaves, o.n_groups, o.depth)
+    del o
+    sel = ref["n_pc"] >= 0
+    rel, prel = check(d_acc.cpu().numpy(), d_pot.cpu().numpy(), n_pc, n_pp, ref, sel)
+    print(f"config5 {tag}: {int(sel.sum())} particles of {n_sample} groups, flips={int(ref['flips'].sum())}, "
+          f"acc q99.9={np.quantile(rel, 0.999):.2e} max={rel.max():.2e} pot max={prel.max():.2e}")
+    return shape
 
 
 def test_config5_two_plummer_16m_parity_and_leapfrog():
+    """Config 5 at full size: oracle parity at step 0 AND on the step-10 positions on 4096 sampled groups,
+    10 KDK steps with a host tree rebuild each step (the torch harness), then the same 10 steps with the library's own
+    device-side leapfrog (`tc_leapfrog`, device tree build) ending in the same state."""
     import torch
     from paper_1005_5384_b200 import integrate
-    n, theta, eps, n_leaf, dt, steps = 1 << 24, 0.5, 0.005, 16, 1.0 / 128, 10
+    n, theta, eps, n_leaf, dt, steps, n_group = 1 << 24, 0.5, 0.005, 16, 1.0 / 128, 10, 64
     pos, mass, vel = inputs.two_plummer(n, with_velocities=True)
     st = torch.cuda.Stream()
-    with torch.cuda.stream(st), B.TreeCode(n_group=64) as tc:
+    with torch.cuda.stream(st), B.TreeCode(n_group=n_group) as tc:
         tc.set_stream(st.cuda_stream)
         d_pos, d_vel, d_mass = torch.from_numpy(pos).cuda(), torch.from_numpy(vel).cuda(), torch.from_numpy(mass).cuda()
         # ---- parity at step 0 on sampled groups (full size, the configuration the loop runs)
@@ -103,16 +129,13 @@ def test_config5_two_plummer_16m_parity_and_leapfrog():
         tc.sync()
         s0 = tc.stats()
         n_pc, n_pp = tc.counts()
-        o = Oracle(pos, mass, n_leaf, 64)
-        assert (s0["n_cells"], s0["n_leaves"], s0["n_groups"], s0["depth"]) == (o.n_cells, o.n_leaves, o.n_groups, o.depth)
-        gsel = np.sort(np.random.default_rng(5).choice(o.n_groups, 256, replace=False)).astype(np.int64)
-        ref = o.forces(theta, eps, shadow32=True, groups=gsel)
-        del o
-        check(d_acc.cpu().numpy(), d_pot.cpu().numpy(), n_pc, n_pp, ref, ref["n_pc"] >= 0)
+        shape = _sampled_parity("step 0", pos, mass, d_acc, d_pot, n_pc, n_pp, theta, eps, n_leaf, n_group, 4096, 5)
+        assert (s0["n_cells"], s0["n_leaves"], s0["n_groups"], s0["depth"]) == shape
         print(f"config5 step 0: cells={s0['n_cells']} groups={s0['n_groups']} T_host={s0['t_host_ms']:.0f} ms "
               f"T_copy={s0['t_copy_ms']:.1f} ms T_gpu={s0['t_gpu_ms']:.1f} ms interactions={s0['n_pc_total'] + s0['n_pp_total']:.3e}")
         # ---- 10 KDK steps, host tree rebuild each step
-        log = integrate.leapfrog_kdk(tc, d_pos, d_vel, d_mass, dt, steps, theta, eps, n_leaf,
+        state = {}
+        log = integrate.leapfrog_kdk(tc, d_pos, d_vel, d_mass, dt, steps, theta, eps, n_leaf, state=state,
                                      log=lambda r: print("config5 step {step:2d}: T_host={t_host_ms:6.0f} ms T_copy={t_copy_ms:5.1f} ms "
                                                          "T_gpu={t_gpu_ms:6.1f} ms wall={wall_ms:6.0f} ms dE/E={dE_rel:.2e} |dP|={dP:.2e}".format(**r)))
         _dump("config5_leapfrog.json", log)
@@ -123,3 +146,25 @@ def test_config5_two_plummer_16m_parity_and_leapfrog():
         n1 = (3 * n) // 4
         x1 = float(d_pos[:n1, 0].double().mean()); x2 = float(d_pos[n1:, 0].double().mean())
         assert 6.0 - 0.06 < (x2 - x1) < 6.0 - 0.02
+        # ---- parity on the step-10 positions: the loop's last force evaluation against an oracle tree built on them
+        pos10 = d_pos.cpu().numpy()
+        n_pc, n_pp = tc.counts()
+        shape10 = _sampled_parity("step 10", pos10, mass, state["acc"], state["pot"], n_pc, n_pp, theta, eps, n_leaf, n_group, 4096, 6)
+        s10 = tc.stats()
+        assert (s10["n_cells"], s10["n_leaves"], s10["n_groups"], s10["depth"]) == shape10
+        # ---- the same 10 steps with the library's device-side leapfrog (native=True, device tree build)
+        d_pos2, d_vel2 = torch.from_numpy(pos).cuda(), torch.from_numpy(vel).cuda()
+        tc.set_option("device_build", 1)
+        state2 = {}
+        log2 = integrate.leapfrog_kdk(tc, d_pos2, d_vel2, d_mass, dt, steps, theta, eps, n_leaf, native=True, state=state2)
+        _dump("config5_leapfrog_native.json", log2)
+        print("config5 native (tc_leapfrog, device build): " + ", ".join(f"{r['wall_ms']:.0f}" for r in log2[1:]) + " ms per step; "
+              f"dE/E max={max(r['dE_rel'] for r in log2):.2e}")
+        assert max(r["dE_rel"] for r in log2) < 2e-4 and max(r["dP"] for r in log2) < 1e-4
+        # same algorithm, same fp32 arithmetic per step (fma kicks vs torch's mul-add differ by an ulp per step)
+        dx = (d_pos2 - d_pos).abs().max().item(); dv = (d_vel2 - d_vel).abs().max().item()
+        print(f"config5 native vs torch harness after {steps} steps: max |dx|={dx:.2e} max |dv|={dv:.2e}")
+        assert dx < 1e-4 and dv < 1e-4
+        n_pc2, n_pp2 = tc.counts()
+        _sampled_parity("step 10 (native)", d_pos2.cpu().numpy(), mass, state2["acc"], state2["pot"], n_pc2, n_pp2, theta, eps,
+                        n_leaf, n_group, 1024, 7)

@@ -120,22 +120,35 @@ def test_config2_64k(name, n_group):
     assert res <= 1e-4
 
 
-# ---- config 3 at FULL size in the launch configuration bench.py times: sampled groups ----
-def test_config3_plummer_1m_sampled():
+# ---- config 3 (headline) at FULL size, EVERY particle, in the launch configuration bench.py times --------
+def flip_bound(n_groups):
+    """Documented borderline opening flips (R16): fp32 decision != fp64 decision; a handful per 1e4 groups."""
+    return max(8, n_groups // 2000)
+
+
+@pytest.mark.parametrize("n_group", ["bench", 16])
+def test_config3_plummer_1m_every_particle(n_group):
+    """Whole-population parity (the error metric is per particle over the whole system): all
+    groups of config 3 through the oracle, at bench.py's N_group and at the paper-literal N_group = N_leaf = 16
+    (PAPER.md:145)."""
     pos, mass, theta, eps, n_leaf = inputs.make("plummer_1m")
     import bench
-    n_group = bench.N_GROUP          # the launch configuration bench.py times
+    n_group = bench.N_GROUP if n_group == "bench" else n_group
     acc, pot, n_pc, n_pp, st = gpu_forces(pos, mass, theta, eps, n_leaf, n_group, device=True)
     o = Oracle(pos, mass, n_leaf, n_group)
     assert (st["n_cells"], st["n_leaves"], st["n_groups"], st["depth"]) == (o.n_cells, o.n_leaves, o.n_groups, o.depth)
-    gsel = np.sort(np.random.default_rng(3).choice(o.n_groups, 1024, replace=False)).astype(np.int64)
-    ref = o.forces(theta, eps, shadow32=True, groups=gsel, stats=True)
-    sel = ref["n_pc"] >= 0
-    assert sel.sum() >= 1024
-    check(acc, pot, n_pc, n_pp, ref, sel)
+    ref = o.forces(theta, eps, shadow32=True, stats=True)
+    assert (ref["n_pc"] >= 0).all()                      # every particle was evaluated by the oracle
+    rel, prel = check(acc, pot, n_pc, n_pp, ref)
+    assert st["n_tests_total"] == int(ref["tests"].sum())
+    assert st["n_pc_total"] == int(ref["n_pc"].sum()) and st["n_pp_total"] == int(ref["n_pp"].sum())
+    flips = int(ref["flips"].sum())
+    print(f"config3 N_group={n_group}: {len(mass)} particles, {o.n_groups} groups, interactions={ref['interactions']}, "
+          f"flips(fp32 vs fp64 decision)={flips}, acc q50={np.median(rel):.2e} q99.9={np.quantile(rel, 0.999):.2e} "
+          f"max={rel.max():.2e}, pot max={prel.max():.2e}")
+    assert flips <= flip_bound(o.n_groups)
     # properties that hold at any size
     assert np.isfinite(acc).all() and np.isfinite(pot).all() and (pot < 0).all()
-    assert st["n_pc_total"] == int(n_pc.astype(np.int64).sum()) and st["n_pp_total"] == int(n_pp.astype(np.int64).sum())
     a64 = acc.astype(np.float64)
     res = np.linalg.norm((mass[:, None] * a64).sum(0)) / (mass * np.linalg.norm(a64, axis=1)).sum()
     assert res <= 1e-4
