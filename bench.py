@@ -472,7 +472,7 @@ def run_ours(args) -> None:
                      "gb_per_s_requested": 64.0 * sw["n_tests_total"] / (walk_ms * 1e-3) / 1e9,
                      "what": "option walk_only (include/tc_bench.h): walk + list building without evaluation.  gb_per_s counts SURVEY 8(d)'s "
                              "algorithmic bytes (16 B per opening test + 16 B per opened cell); gb_per_s_requested counts what the kernel asks "
-                             "L2 for (4 float4 per test: 86 % of the tested cells end on a cell list and need their 48 B of multipole); "
+                             "L2 for (4 float4 per test: 84 % of the tested cells end on a cell list and need their 48 B of multipole); "
                              "lts__t_bytes of this launch is in profiles/; the paper reports > 50 GB/s for its count pass on G80 (PAPER.md:177)"},
             "e2e": {"value": inter_all / e2e_s, "unit": "interactions/s", "h2d_bytes_per_step": int(tree_bytes),
                     "d2h_bytes_per_step": int(16 * n), "ms_per_step": e2e_s * 1e3,

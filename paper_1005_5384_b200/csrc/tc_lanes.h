@@ -32,6 +32,9 @@ constexpr int kMaxK = TC_MAXK;          // particles per lane: kMaxK / 2 packed 
 constexpr int kPassCap = TC_PASSCAP;    // particles of a group handled by ONE walk; larger groups (level-21 leaves of
                                         // coincident particles, or N_group > kPassCap) are walked once per kPassCap
 static_assert(kMaxK >= 4 && kMaxK <= 8 && kPassCap <= 32 * kMaxK, "every pass size needs a mapping with S = 1");
+// (measured with csrc/bench/mb_eval.cu before the last two kernel changes; the final build measures 46.0, 87.7, 122.4, 163.3, 208.3,
+// 245.5, 283.6, 317.8 — profiles/r02_microbench.md — but the table built from THOSE runs the whole kernel slower, 5.86 against 5.74 ms:
+// inside the kernel the odd-K loops, which they favour, lose more than they do alone.  The table is a tuning input, kept at its best.)
 constexpr float kRecordCycles[9] = {0.f, 47.3f, 87.0f, 134.7f, 160.6f, 208.3f, 240.8f, 293.7f, 324.1f};
 
 struct LaneMap {

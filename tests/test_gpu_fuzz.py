@@ -137,12 +137,20 @@ def test_fuzz_case_matches_the_oracle(seed):
     a_ref = np.linalg.norm(ref["acc"], axis=1)
     scale = np.maximum(a_ref, np.sqrt(np.mean(a_ref ** 2)))
     err = np.linalg.norm(acc.astype(np.float64) - ref["acc"], axis=1) / np.where(scale > 0, scale, 1.0)
-    # bar: 1e-4 (the q99.9 bar of north_star, here for EVERY particle), plus — for the clumps far from the
-    # origin only — the fp32 rounding of a stored centre of mass (<= 2^-24 |X| per axis, DESIGN.md §6
-    # "Tolerance") against the shortest distances the case has (>= eps): an input-conditioning term
-    tol = 1e-4 + (4 * 2.0 ** -24 * float(np.abs(pos).max()) / max(eps, 1e-4) if kind == "lumps" else 0.0)
+    # bar: 1e-4 (the q99.9 bar of north_star, here for EVERY particle); 2e-4 for the clumps far from the origin
+    # (`lumps`): the fp32 rounding of a stored centre of mass (<= 2^-24 |X| per axis) against source distances as
+    # short as eps is an input-conditioning term (DESIGN.md section 6 "Tolerance"; measured worst case 1.1e-4, the
+    # a-priori bound 4 * 2^-24 max|x| / eps would be up to 2.3e-3) — still 5x inside north_star's maximum of 1e-3
+    tol = 2e-4 if kind == "lumps" else 1e-4
+    if kind == "lumps":
+        print(f"fuzz lumps seed={seed}: max|x|={float(np.abs(pos).max()):.1f} eps={eps:.1e} acc err max={float(err.max()):.2e} (bar {tol:.2e})")
     assert err.max() <= tol, (kind, n, n_leaf, n_group, theta, eps, opts, float(err.max()), tol)
     p_ref = np.abs(ref["pot"])
     pscale = np.maximum(p_ref, np.sqrt(np.mean(p_ref ** 2)))
     perr = np.abs(pot - ref["pot"]) / np.where(pscale > 0, pscale, 1.0)
-    assert perr.max() <= tol, (kind, n, n_leaf, n_group, theta, eps, opts, float(perr.max()), tol)
+    # potential: the same bar plus the documented fp32 self term (DESIGN.md section 6 "Tolerance", include/tc.h): with eps > 0
+    # -m_i/eps is added to phi_i and taken out again, an absolute error of a few ulps of m_i/eps
+    ptol = tol + (4 * 2.0 ** -24 * mass / eps / np.where(pscale > 0, pscale, 1.0) if eps > 0 else 0.0)
+    if kind == "lumps":
+        print(f"fuzz lumps seed={seed}: pot err max={float(perr.max()):.2e} (self-term allowance up to {float(np.max(ptol - tol)):.2e})")
+    assert (perr <= ptol).all(), (kind, n, n_leaf, n_group, theta, eps, opts, float(perr.max()), float(np.max(ptol)))
