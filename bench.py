@@ -227,11 +227,14 @@ def run_ours(args) -> None:
         if world == 1 and args.gpus > 1:
             raise SystemExit("bench.py --gpus N>1 must be launched with torch.distributed.run (one rank per GPU)")
     assert torch.cuda.is_available(), "bench.py needs a CUDA device: there is no CPU fallback for the product path"
+    local = local % torch.cuda.device_count()
     torch.cuda.set_device(local)
     dev = torch.device("cuda", local)
     if world > 1:
         import torch.distributed as dist
-        dist.init_process_group("nccl", device_id=dev)
+        # NCCL over NVLink / NVSwitch; TC_BENCH_BACKEND=gloo exists only to walk this code path on a one-GPU box
+        backend = os.environ.get("TC_BENCH_BACKEND", "nccl")
+        dist.init_process_group(backend, **({"device_id": dev} if backend == "nccl" else {}))
     from paper_1005_5384_b200 import binding as B
     from paper_1005_5384_b200 import build as tc_build
     from paper_1005_5384_b200 import inputs, parallel
