@@ -484,6 +484,7 @@ int build_host_tree(const float4* xyzm, int64_t n, int n_leaf, int n_group,
   // itself reads.  Stable: Morton order inside a cost class keeps neighbouring groups together.
   {
     static constexpr LaneTable lanes = LaneTable();
+    const int shift = schedule_class_shift((long long)groups.size());
     // counting sort by cost class, descending; stable, so Morton order survives inside a class
     const size_t ng = groups.size();
     std::vector<int32_t> cls(ng);
@@ -491,7 +492,7 @@ int build_host_tree(const float4* xyzm, int64_t n, int n_leaf, int n_group,
 #pragma omp parallel for schedule(static) reduction(max : cmax)
     for (size_t g = 0; g < ng; g++) {
       const int64_t cnt = c_count[groups[g]];
-      cls[g] = group_cost_class(lanes, cnt);
+      cls[g] = group_cost_class(lanes, cnt, shift);
       cmax = std::max(cmax, cls[g]);
     }
     std::vector<int32_t> start((size_t)cmax + 2, 0);

@@ -272,13 +272,13 @@ __global__ void k_pack_particles(const float4* __restrict__ src, const unsigned 
 // group records: key for the Morton order = first body; cost class for the schedule
 __constant__ LaneTable c_lanes_build = LaneTable();   // the kernel's lane mapping (tc_lanes.h): cost model of the schedule
 __global__ void k_group_keys(const int* __restrict__ gcell, int ng, const int* __restrict__ c_begin, const int* __restrict__ c_count,
-                             unsigned int* __restrict__ first_body, unsigned int* __restrict__ cls_key) {
+                             unsigned int* __restrict__ first_body, unsigned int* __restrict__ cls_key, int shift) {
   const int g = blockIdx.x * blockDim.x + threadIdx.x;
   if (g >= ng) return;
   const int c = gcell[g];
   first_body[g] = (unsigned int)c_begin[c];
   const int cnt = c_count[c];
-  cls_key[g] = (unsigned int)(kMaxCostClass - group_cost_class(c_lanes_build, cnt));   // ascending key = descending cost
+  cls_key[g] = (unsigned int)(kMaxCostClass - group_cost_class(c_lanes_build, cnt, shift));   // ascending key = descending cost
 }
 
 __global__ void k_iota(unsigned int* a, int n) {
@@ -478,7 +478,7 @@ int build_device_tree(const float4* src, int64_t n, int n_leaf, int n_group, Dev
   TCG_GROW(S.gcell_sorted, S.cap_gcells, ng, false);
   {
     // (1) sort the group cells by first body: keys = first body, values = cell id
-    k_group_keys<<<blocks(ng), 256, 0, st>>>(S.gcell, (int)ng, S.c_begin, S.c_count, S.gkey, S.gval);
+    k_group_keys<<<blocks(ng), 256, 0, st>>>(S.gcell, (int)ng, S.c_begin, S.c_count, S.gkey, S.gval, schedule_class_shift((long long)ng));
     cub::DoubleBuffer<unsigned int> kb(S.gkey, S.gkey_alt);
     cub::DoubleBuffer<int> vb(S.gcell, S.gcell_sorted);
     size_t need = 0;
@@ -488,7 +488,7 @@ int build_device_tree(const float4* src, int64_t n, int n_leaf, int n_group, Dev
     if (vb.Current() != S.gcell_sorted) { std::swap(S.gcell, S.gcell_sorted); std::swap(S.cap_gcell, S.cap_gcells); }
     if (kb.Current() != S.gkey) { std::swap(S.gkey, S.gkey_alt); std::swap(S.cap_gkey, S.cap_gkeya); }
     // (2) schedule: stable sort of the Morton-ordered group indices by descending cost class
-    k_group_keys<<<blocks(ng), 256, 0, st>>>(S.gcell_sorted, (int)ng, S.c_begin, S.c_count, S.gkey_alt, S.gkey);
+    k_group_keys<<<blocks(ng), 256, 0, st>>>(S.gcell_sorted, (int)ng, S.c_begin, S.c_count, S.gkey_alt, S.gkey, schedule_class_shift((long long)ng));
     k_iota<<<blocks(ng), 256, 0, st>>>(S.gval, (int)ng);
     cub::DoubleBuffer<unsigned int> kb2(S.gkey, S.gkey_alt);
     cub::DoubleBuffer<unsigned int> vb2(S.gval, S.gval_alt);

@@ -35,7 +35,19 @@ static_assert(kMaxK >= 4 && kMaxK <= 8 && kPassCap <= 32 * kMaxK, "every pass si
 // (measured with csrc/bench/mb_eval.cu before the last two kernel changes; the final build measures 46.0, 87.7, 122.4, 163.3, 208.3,
 // 245.5, 283.6, 317.8 — profiles/r02_microbench.md — but the table built from THOSE runs the whole kernel slower, 5.86 against 5.74 ms:
 // inside the kernel the odd-K loops, which they favour, lose more than they do alone.  The table is a tuning input, kept at its best.)
-constexpr float kRecordCycles[9] = {0.f, 47.3f, 87.0f, 134.7f, 160.6f, 208.3f, 240.8f, 293.7f, 324.1f};
+#ifndef TC_RC3
+#define TC_RC3 134.7f
+#endif
+#ifndef TC_RC5
+#define TC_RC5 208.3f
+#endif
+#ifndef TC_RC7
+#define TC_RC7 293.7f
+#endif
+#ifndef TC_RC8
+#define TC_RC8 324.1f
+#endif
+constexpr float kRecordCycles[9] = {0.f, 47.3f, 87.0f, TC_RC3, 160.6f, TC_RC5, 240.8f, TC_RC7, TC_RC8};
 
 struct LaneMap {
   unsigned char S, q, K;
@@ -65,10 +77,19 @@ struct LaneTable {
 
 // Cost class of a whole group of `cnt` particles for the schedule (costly groups run first): cycles per
 // list entry in 1/8 cycles, integer so that the host and the device builder agree bit for bit; <= kMaxCostClass.
+// `shift` coarsens the classes (schedule_class_shift below): inside a class the groups stay in Morton order.
 constexpr int kMaxCostClass = 1000000;
-TC_HD constexpr int group_cost_class(const LaneTable& t, long long cnt) {
-  const long long c = (cnt / kPassCap) * (long long)t.cost8[kPassCap] + (long long)t.cost8[cnt % kPassCap];
+TC_HD constexpr int group_cost_class(const LaneTable& t, long long cnt, int shift) {
+  const long long c = ((cnt / kPassCap) * (long long)t.cost8[kPassCap] + (long long)t.cost8[cnt % kPassCap]) >> shift;
   return c > kMaxCostClass ? kMaxCostClass : (int)c;
 }
+// Costly-first order only matters for the tail of the launch: with few groups per warp (config 3: 35 603 groups on 2 368
+// persistent warps) the exact order is worth 5 % (5.78 against 6.10 ms in pure Morton order).  With hundreds of groups per
+// warp the tail is nothing and PURE MORTON order keeps the warps in flight on neighbouring groups, which is what the L2
+// sees when the tree no longer fits in it (N = 2^24: 0.6 GB of tree, profiles/r02_walk_literal_config5.md).
+#ifndef TC_MORTON_MIN_GROUPS
+#define TC_MORTON_MIN_GROUPS 400000
+#endif
+TC_HD constexpr int schedule_class_shift(long long n_groups) { return n_groups >= TC_MORTON_MIN_GROUPS ? 30 : 0; }
 
 }  // namespace tc

@@ -183,3 +183,24 @@ def test_pinned_host_inputs_take_the_direct_dma_path_and_bad_values_are_still_re
         tc.build(n_leaf)
         acc, _ = tc.forces(theta, eps)
         assert np.abs(acc - out[0][0]).max() <= 2e-6 * np.abs(out[0][0]).max()
+
+
+def test_pure_morton_schedule_with_very_many_groups():
+    """>= 400 000 groups: both builders schedule in pure Morton order (tc_lanes.h, schedule_class_shift); the schedule
+    changes only WHEN a group runs, so counts are identical and forces agree to summation-order rounding."""
+    pos, mass = inputs.uniform_cube(1 << 19, 33)
+    res = {}
+    for dev in (0, 1):
+        with B.TreeCode(n_group=1) as tc:
+            tc.set_option("device_build", dev)
+            tc.set_particles(pos, mass)
+            tc.build(1)
+            assert tc.stats()["n_groups"] >= 400000
+            acc, pot = tc.forces(0.7, 0.01)
+            res[dev] = (acc, pot) + tc.counts()
+    assert np.array_equal(res[0][2], res[1][2]) and np.array_equal(res[0][3], res[1][3])
+    assert np.allclose(res[0][0], res[1][0], rtol=2e-5, atol=1e-7) and np.allclose(res[0][1], res[1][1], rtol=2e-5)
+    o = Oracle(pos, mass, 1, 1)
+    gsel = np.arange(0, o.n_groups, o.n_groups // 500, dtype=np.int64)
+    ref = o.forces(0.7, 0.01, shadow32=True, groups=gsel)
+    check(res[1][0], res[1][1], res[1][2], res[1][3], ref, ref["n_pc"] >= 0)
