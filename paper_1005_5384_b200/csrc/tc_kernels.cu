@@ -224,6 +224,10 @@ struct Lanes {
   int S, q, K;   // warp-uniform
   int s, p;      // this lane's slice and particle column
   bool active;   // lane < S * q
+  // the TAIL of the pass (tc_lanes.h): its last mB particles, tree-order indices tail .. tail + mB - 1, are not in the
+  // mapping; every lane applies its own records (S = 32, q = 1) to all of them.  The mapping covers mA = m - mB.
+  int mA, mB, tail;
+  const float4* part;
 };
 
 // one list record applied to the lane's KP pairs (+ ODD single particle)
@@ -310,10 +314,67 @@ __device__ __forceinline__ void eval_dispatch(const void* list, int cnt, float e
     eval_dispatch<WHAT, kEps0, K + 1>(list, cnt, eps2, L, st);
   }
 }
+// The tail particles (Lanes::mB of them): lane l takes list entries l, l + 32, ... and applies each to ALL tail particles in
+// scalar arithmetic.  Their accumulators are the halves of the TOP register pairs of the state (the lane table leaves
+// those pairs to the tail): unpacked to scalars for the loop, packed again after it.
+template <int MB, int WHAT, bool kEps0>
+__device__ __forceinline__ void eval_tail_m(const void* list, int cnt, float eps2, const Lanes& L, PassState& st, int lane) {
+  Pos1 p[MB];
+  Acc1 a[MB];
+#pragma unroll
+  for (int j = 0; j < MB; j++) {
+    const float4 m0 = __ldg(L.part + L.tail + j);          // warp-uniform address
+    p[j].x = m0.x; p[j].y = m0.y; p[j].z = m0.z;
+    const Acc2& a2 = st.A[kMaxKP - 1 - (j >> 1)];
+    if (j & 1) { a[j].ax = hi(a2.ax); a[j].ay = hi(a2.ay); a[j].az = hi(a2.az); a[j].npot = hi(a2.npot); }
+    else { a[j].ax = lo(a2.ax); a[j].ay = lo(a2.ay); a[j].az = lo(a2.az); a[j].npot = lo(a2.npot); }
+  }
+  if (WHAT == kEvalBodies) {
+    const float4* b = static_cast<const float4*>(list) + lane;
+    const float4* const end = static_cast<const float4*>(list) + cnt;
+    for (; b < end; b += 32) {
+      const float4 bb = b[0];
+#pragma unroll
+      for (int j = 0; j < MB; j++) pp_interact<kEps0>(p[j], eps2, bb, a[j]);
+    }
+  } else {
+    const CellRec* r = static_cast<const CellRec*>(list) + lane;
+    const CellRec* const end = static_cast<const CellRec*>(list) + cnt;
+    for (; r < end; r += 32) {
+      const float4 xm = r->xm, q0 = r->q0; const float2 q1 = r->q1;
+#pragma unroll
+      for (int j = 0; j < MB; j++) {
+        if (WHAT == kEvalMono) pp_interact<kEps0>(p[j], eps2, xm, a[j]);
+        else pc_interact(p[j], eps2, xm, q0, q1, a[j]);
+      }
+    }
+  }
+#pragma unroll
+  for (int jj = 0; jj < (MB + 1) / 2; jj++) {
+    Acc2& a2 = st.A[kMaxKP - 1 - jj];
+    const int j0 = 2 * jj, j1 = (2 * jj + 1 < MB) ? 2 * jj + 1 : 2 * jj;
+    const bool two = 2 * jj + 1 < MB;
+    // (+ 0 through FADD2: see setup_pass)
+    a2.ax = add2(pk(a[j0].ax, two ? a[j1].ax : 0.f), bc(0.f)); a2.ay = add2(pk(a[j0].ay, two ? a[j1].ay : 0.f), bc(0.f));
+    a2.az = add2(pk(a[j0].az, two ? a[j1].az : 0.f), bc(0.f)); a2.npot = add2(pk(a[j0].npot, two ? a[j1].npot : 0.f), bc(0.f));
+  }
+}
+template <int WHAT, bool kEps0, int MB = 1>
+__device__ __forceinline__ void eval_tail(const void* list, int cnt, float eps2, const Lanes& L, PassState& st, int lane) {
+  if constexpr (kMaxTail >= 1) {
+    if (MB == kMaxTail || L.mB == MB) eval_tail_m<MB, WHAT, kEps0>(list, cnt, eps2, L, st, lane);
+    else if constexpr (MB < kMaxTail) eval_tail<WHAT, kEps0, MB + 1>(list, cnt, eps2, L, st, lane);
+  }
+}
+
 template <bool kEps0>
-__device__ __forceinline__ void eval_cells(const CellRec* rec, int cnt, float eps2, const Lanes& L, PassState& st, bool mono) {
+__device__ __forceinline__ void eval_cells(const CellRec* rec, int cnt, float eps2, const Lanes& L, PassState& st, bool mono, int lane) {
   if (mono) eval_dispatch<kEvalMono, kEps0>(rec, cnt, eps2, L, st);
   else eval_dispatch<kEvalCells, kEps0>(rec, cnt, eps2, L, st);
+  if (L.mB) {                                          // warp-uniform
+    if (mono) eval_tail<kEvalMono, kEps0>(rec, cnt, eps2, L, st, lane);
+    else eval_tail<kEvalCells, kEps0>(rec, cnt, eps2, L, st, lane);
+  }
 }
 
 // Opened leaves (List 4): flatten the queued (first, n) ranges into
@@ -361,6 +422,7 @@ __device__ __forceinline__ void eval_leaves(BodyStage& bs, const int2* leafq, in
         __syncwarp();
       }
       eval_dispatch<kEvalBodies, kEps0>(bs.body, cnt, eps2, L, st);
+      if (L.mB) eval_tail<kEvalBodies, kEps0>(bs.body, cnt, eps2, L, st, lane);
       __syncwarp();
     }
   }
@@ -370,6 +432,8 @@ __device__ __forceinline__ void eval_leaves(BodyStage& bs, const int2* leafq, in
 __device__ __forceinline__ void setup_pass(Lanes& L, PassState& st, const float4* __restrict__ part, int first, int m, int lane) {
   const LaneMap lm = c_lanes.map[m];
   L.S = lm.S; L.q = lm.q; L.K = lm.K;
+  L.mB = lm.mB; L.mA = m - L.mB; L.tail = first + L.mA; L.part = part;
+  m = L.mA;                                              // the mapping covers the particles in front of the tail
   L.s = lane / L.q;
   L.p = lane - L.s * L.q;
   L.active = L.s < L.S;
@@ -406,12 +470,34 @@ struct ShardOut {
 // A6: reduce the slices of every particle, write back in the caller's order (or into the shard's compact rows).
 // kAdd: add to what is already there (second evaluation kernel of the two-pass variant);
 // kSelf: the particles met themselves once in the particle-particle part (remove -m/eps again).
+// one particle's result: tree-order index t (row tq of the group), to the caller's order or to the shard's compact rows
+template <bool kAdd, bool kSelf>
+__device__ __forceinline__ void store_particle(int t, int tq, float ax, float ay, float az, float ph, const float4* __restrict__ part,
+                                               const int32_t* __restrict__ orig, float eps2, float* __restrict__ acc,
+                                               float* __restrict__ pot, int32_t* __restrict__ out_cnt, int cnt_value,
+                                               int32_t* __restrict__ out_cnt2, int cnt2_value, bool self_met,
+                                               float4* __restrict__ rows, int2* __restrict__ row_cnt) {
+  if (kSelf && self_met) ph += __ldg(part + t).w * rsqrt_approx(eps2);     // the particle met itself once
+  if (!kAdd && rows) {                                                     // shard: compact rows, tree order inside the group
+    rows[tq] = make_float4(ax, ay, az, ph);
+    if (row_cnt) row_cnt[tq] = make_int2(cnt_value, cnt2_value);
+    return;
+  }
+  const int i = __ldg(orig + t);
+  float* a3 = acc + 3 * (size_t)i;
+  if (kAdd) { a3[0] += ax; a3[1] += ay; a3[2] += az; if (pot) pot[i] += ph; }
+  else { a3[0] = ax; a3[1] = ay; a3[2] = az; if (pot) pot[i] = ph; }
+  out_cnt[i] = cnt_value;
+  if (out_cnt2) out_cnt2[i] = cnt2_value;
+}
+
 template <bool kAdd, bool kSelf>
 __device__ __forceinline__ void write_back(const Lanes& L, const PassState& st, const float4* __restrict__ part,
                                            const int32_t* __restrict__ orig, int first, int m, float eps2, int lane,
                                            float* __restrict__ acc, float* __restrict__ pot, int32_t* __restrict__ out_cnt,
                                            int cnt_value, int32_t* __restrict__ out_cnt2 = nullptr, int cnt2_value = 0,
                                            bool self_met = true, float4* __restrict__ rows = nullptr, int2* __restrict__ row_cnt = nullptr) {
+  // ---- the particles of the lane mapping: slices reduced with shuffles
 #pragma unroll
   for (int j = 0; j < kMaxK; j++) {
     if (j >= L.K) break;                             // warp-uniform
@@ -426,22 +512,28 @@ __device__ __forceinline__ void write_back(const Lanes& L, const PassState& st, 
       if ((L.s % (2 * w)) == 0 && L.s + w < L.S) { ax += ox; ay += oy; az += oz; ph += op; }
     }
     const int tq = j * L.q + lane;
-    if (lane < L.q && tq < m) {
-      const int t = first + tq;
-      if (kSelf && self_met) ph += __ldg(part + t).w * rsqrt_approx(eps2);     // the particle met itself once
-      if (!kAdd && rows) {                                                     // shard: compact rows, tree order inside the group
-        rows[tq] = make_float4(ax, ay, az, ph);
-        if (row_cnt) row_cnt[tq] = make_int2(cnt_value, cnt2_value);
-        continue;
-      }
-      const int i = __ldg(orig + t);
-      float* a3 = acc + 3 * (size_t)i;
-      if (kAdd) { a3[0] += ax; a3[1] += ay; a3[2] += az; if (pot) pot[i] += ph; }
-      else { a3[0] = ax; a3[1] = ay; a3[2] = az; if (pot) pot[i] = ph; }
-      out_cnt[i] = cnt_value;
-      if (out_cnt2) out_cnt2[i] = cnt2_value;
-    }
+    if (lane < L.q && tq < L.mA)
+      store_particle<kAdd, kSelf>(first + tq, tq, ax, ay, az, ph, part, orig, eps2, acc, pot, out_cnt, cnt_value, out_cnt2, cnt2_value,
+                                  self_met, rows, row_cnt);
   }
+  // ---- the tail: every lane holds a partial sum of every tail particle (halves of the top register pairs)
+#pragma unroll
+  for (int j = 0; j < kMaxTail; j++) {
+    if (j >= L.mB) break;                            // warp-uniform
+    const Acc2& a2 = st.A[kMaxKP - 1 - (j >> 1)];
+    float ax, ay, az, ph;
+    if (j & 1) { ax = hi(a2.ax); ay = hi(a2.ay); az = hi(a2.az); ph = -hi(a2.npot); }
+    else { ax = lo(a2.ax); ay = lo(a2.ay); az = lo(a2.az); ph = -lo(a2.npot); }
+#pragma unroll
+    for (int w = 16; w >= 1; w >>= 1) {
+      ax += __shfl_xor_sync(kFull, ax, w); ay += __shfl_xor_sync(kFull, ay, w);
+      az += __shfl_xor_sync(kFull, az, w); ph += __shfl_xor_sync(kFull, ph, w);
+    }
+    if (lane == 0)
+      store_particle<kAdd, kSelf>(L.tail + j, L.mA + j, ax, ay, az, ph, part, orig, eps2, acc, pot, out_cnt, cnt_value, out_cnt2,
+                                  cnt2_value, self_met, rows, row_cnt);
+  }
+  (void)m;
 }
 
 // Global interaction lists of the paper-literal two-pass variant (count, scan, write).
@@ -657,7 +749,7 @@ forces_kernel(const float4* __restrict__ bnd, const float4* __restrict__ xm, con
           // is needed, or the walk is over
           const bool flush_leaves = walking ? (lq > kLeafQCap - 32 * kWalkB) : (lq > 0);
           if (ccnt > (walking ? kCellCap - 32 * kWalkB : 0) || (flush_leaves && ccnt)) {
-            if (!walk_only) eval_cells<kEps0>(sm.u.cell, ccnt, eps2, L, ps, mono);
+            if (!walk_only) eval_cells<kEps0>(sm.u.cell, ccnt, eps2, L, ps, mono, lane);
             ccnt = 0; __syncwarp();
           }
           if (flush_leaves) { if (!walk_only) eval_leaves<kEps0>(sm.u.bs, sm.leafq, lq, part, eps2, L, ps, lane, mbar, &bulk_phase); lq = 0; __syncwarp(); }
@@ -724,7 +816,7 @@ node_kernel(const float4* __restrict__ xm, const float4* __restrict__ q0, const 
           r.xm = __ldg(xm + c); r.q0 = __ldg(q0 + c); r.q1 = make_float2(c1.x, c1.y);
         }
         __syncwarp();
-        eval_cells<false>(sm.u.cell, cnt, eps2, L, ps, mono);
+        eval_cells<false>(sm.u.cell, cnt, eps2, L, ps, mono, lane);
         __syncwarp();
       }
       write_back<false, false>(L, ps, part, orig, G.y + pb, m, eps2, lane, acc, pot, out_npc, n_c);

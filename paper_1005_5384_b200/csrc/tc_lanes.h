@@ -49,27 +49,48 @@ static_assert(kMaxK >= 4 && kMaxK <= 8 && kPassCap <= 32 * kMaxK, "every pass si
 #endif
 constexpr float kRecordCycles[9] = {0.f, 47.3f, 87.0f, TC_RC3, 160.6f, TC_RC5, 240.8f, TC_RC7, TC_RC8};
 
+// TAIL: the lane mapping wastes lane-slots whenever m is not S*q*K-shaped (37 particles in 40 slots on 30 lanes).  So up
+// to kMaxTail particles of the pass, its LAST mB ones, can be taken out of the mapping and evaluated differently: every
+// lane is its own slice (S = 32, q = 1) and applies ITS records to all mB tail particles in scalar arithmetic; the
+// mapping then covers the m - mB particles in front (32 + 5 instead of 37: 100 % and 94 % of the lanes busy).  The tail's
+// accumulators live in the halves of the top register pairs of the mapping's state, which is why a tail of mB particles
+// leaves the mapping 4 - ceil(mB/2) pairs: floor(K/2) + ceil(mB/2) <= kMaxK/2.
+#ifndef TC_MAXTAIL
+#define TC_MAXTAIL 4
+#endif
+constexpr int kMaxTail = TC_MAXTAIL;
+static_assert(kMaxTail >= 0 && kMaxTail <= 4, "the tail lives in the top two register pairs");
+#ifndef TC_TAIL_OVER
+#define TC_TAIL_OVER 1.0f
+#endif
+constexpr float kTailCycles = 47.3f / 32.f;   // cycles per list entry and tail particle: the K = 1 loop at S = 32
+constexpr float kTailOverhead = TC_TAIL_OVER; // per list entry: the tail's own loop set-up per chunk (positions, unpack / repack);
+                                              // measured: tail off 5.777 ms, on 5.746 (overhead 0.3) / 5.738 (1.0) at config 3
+
 struct LaneMap {
-  unsigned char S, q, K;
+  unsigned char S, q, K, mB;   // mB: particles of the tail (the mapping covers m - mB)
 };
 
 struct LaneTable {
   LaneMap map[kPassCap + 1];
   int cost8[kPassCap + 1];    // cycles per list entry of a pass over m particles, in units of 1/8 cycle
   constexpr LaneTable() : map{}, cost8{} {
-    map[0] = LaneMap{1, 32, 1};
+    map[0] = LaneMap{1, 32, 1, 0};
     cost8[0] = 0;
     for (int m = 1; m <= kPassCap; m++) {
-      int bs = 0, bq = 0, bk = 0;
+      int bs = 0, bq = 0, bk = 0, bb = 0;
       float best = 1e30f;
-      for (int s = 1; s <= 32; s++) {
-        const int q = 32 / s;
-        const int k = (m + q - 1) / q;
-        if (k > kMaxK) continue;
-        const float c = kRecordCycles[k] / (float)s;
-        if (c < best) { best = c; bs = s; bq = q; bk = k; }
+      for (int mb = 0; mb <= kMaxTail && mb < m; mb++) {
+        const float tail = mb ? kTailCycles * (float)mb + kTailOverhead : 0.f;
+        for (int s = 1; s <= 32; s++) {
+          const int q = 32 / s;
+          const int k = (m - mb + q - 1) / q;
+          if (k > kMaxK || k / 2 + (mb + 1) / 2 > kMaxK / 2) continue;
+          const float c = kRecordCycles[k] / (float)s + tail;
+          if (c < best) { best = c; bs = s; bq = q; bk = k; bb = mb; }
+        }
       }
-      map[m] = LaneMap{(unsigned char)bs, (unsigned char)bq, (unsigned char)bk};
+      map[m] = LaneMap{(unsigned char)bs, (unsigned char)bq, (unsigned char)bk, (unsigned char)bb};
       cost8[m] = (int)(best * 8.f + 0.5f);
     }
   }
