@@ -4,7 +4,7 @@
 Metric: interactions/s (and ms per force evaluation = `ms_per_step`) of ONE force
 evaluation — the whole hot path A1-A6 of DESIGN.md section 1 (tree walk + interaction
 list evaluation + write-back) — on config 3: Plummer sphere N = 2^20 (seed 3),
-theta = 0.5, eps = 0.01, N_leaf = 16, N_group = 96 (tuned; option `n_group`), monopole+quadrupole, fp32.
+theta = 0.5, eps = 0.01, N_leaf = 16, N_group = 128 (tuned; option `n_group`), monopole+quadrupole, fp32.
 
   python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference]
 
@@ -41,7 +41,7 @@ if ROOT not in sys.path:
     sys.path.insert(0, ROOT)
 
 WORKLOAD = "plummer_1m"           # BASELINE.json configs[2]: the configuration the metric is quoted on
-N_GROUP = 96
+N_GROUP = 128
 # flops per interaction, SASS convention (FFMA = 2, FADD/FMUL = 1, MUFU.RSQ = 1) — DESIGN.md section 6
 FLOPS_PC, FLOPS_PP = 54, 20
 # paper convention (fn. 3)

@@ -96,7 +96,7 @@ int tc_set_particles(tc_ctx* ctx, const float* pos, const float* mass, int64_t n
 
 /* Host octree: root cube, recursive 8-way split until a cell
  * holds <= n_leaf particles (or level 21), tight bounding boxes, boundary cubes,
- * fp64 moments rounded to fp32, groups (N_group from tc_set_option, default 96),
+ * fp64 moments rounded to fp32, groups (N_group from tc_set_option, default 128),
  * SoA float4 packing, one bulk host->device copy.
  * Errors: TC_ESTATE (no particles), TC_EINVAL (n_leaf < 1), TC_ENOMEM, TC_ECUDA. */
 int tc_build(tc_ctx* ctx, int n_leaf);
@@ -131,6 +131,10 @@ int tc_forces(tc_ctx* ctx, float theta, float eps, float* acc, float* pot);
  *                 still conservative, about 1 % fewer interactions.  Combines with "open_rule".
  *   "quadrupole"  1 (default: monopole + quadrupole) or 0: monopole-only cells (variant R22, the expansion of
  *                 the Hamada et al. code the paper compares with).
+ *   "kernel_config" launch configuration of the fused kernel: 0 (default) = chosen by the mean number of particles per
+ *                 group, 1 = sparse (16 warps per SM, for small groups), 2 = dense (12 warps per SM with larger
+ *                 shared-memory chunks and more registers, for large groups).  Same arithmetic, same lists: results differ
+ *                 by summation order only (the chunk boundaries move).
  *   "shard_count", "shard_rank"   ONE force evaluation over k GPUs (tc_forces_shard below): this context is
  *                 rank shard_rank of shard_count.  Default 1 / 0.
  *   "two_pass"    0 (default: the fused kernel) or 1: the paper-literal pipeline —

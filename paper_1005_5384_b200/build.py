@@ -12,7 +12,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libtc_b200.so")
-SOURCES = ["tc_api.cpp", "tc_build.cpp", "tc_kernels.cu", "tc_build_gpu.cu", "tc_shard.cu"]
+SOURCES = ["tc_api.cpp", "tc_build.cpp", "tc_kernels.cu", "tc_kernels_dense.cu", "tc_build_gpu.cu", "tc_shard.cu"]
 HEADERS = ["tc_internal.h", "tc_lanes.h", os.path.join("..", "..", "include", "tc.h"), os.path.join("..", "..", "include", "tc_bench.h")]
 
 NVCC_FLAGS = [

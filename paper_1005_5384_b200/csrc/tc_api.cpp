@@ -15,6 +15,10 @@
 
 #include "tc_internal.h"
 
+#ifndef TC_DENSE_MIN_MEAN
+#define TC_DENSE_MIN_MEAN 24.0
+#endif
+
 struct tc_ctx {
   uint32_t flags = 0;
   bool host_only = false;
@@ -23,11 +27,12 @@ struct tc_ctx {
   cudaEvent_t ev0 = nullptr, ev1 = nullptr;
   std::string err;
   // options
-  int n_group = 96;
+  int n_group = 128;
   bool device_build = false;          // option "device_build": tc_build_gpu.cu instead of tc_build.cpp
   int stack_smem = 256;
   int walk_only = 0, open_rule = 0, quadrupole = 1, group_box = 0;
   int shard_rank = 0, shard_count = 1;
+  int kernel_config = 0;              // option "kernel_config": 0 = by the mean group size, 1 = sparse, 2 = dense (tc_kernels.cu)
   bool two_pass = false;
   tc::TwoPassScratch tps;
   bool last_two_pass = false;
@@ -235,6 +240,10 @@ int tc_set_option(tc_ctx* c, const char* key, double v) {
     if (v != 0.0 && v != 1.0) return fail(c, TC_EINVAL, "tc_set_option: open_rule must be 0 or 1");
     c->open_rule = (int)v; return TC_OK;
   }
+  if (!std::strcmp(key, "kernel_config")) {
+    if (v != 0.0 && v != 1.0 && v != 2.0) return fail(c, TC_EINVAL, "tc_set_option: kernel_config must be 0 (auto), 1 (sparse) or 2 (dense)");
+    c->kernel_config = (int)v; return TC_OK;
+  }
   if (!std::strcmp(key, "shard_count")) {
     if (!(v >= 1.0) || v > 65536.0 || v != std::floor(v)) return fail(c, TC_EINVAL, "tc_set_option: shard_count must be an integer in [1, 65536]");
     c->shard_count = (int)v; return TC_OK;
@@ -435,6 +444,8 @@ namespace {
 // cannot resolve separations below 1e-10 anyway unless |x| < 1e-3.  theta whose square overflows fp32 is refused
 // (d^2 theta^2 = 0 * inf = NaN would leave a group's own ancestors un-opened).
 constexpr float kEpsMin = 1e-10f;
+// the dense launch configuration pays from this many particles per group on (measured crossover)
+constexpr double kDenseMinMean = TC_DENSE_MIN_MEAN;
 int check_theta_eps(tc_ctx* c, const char* who, float theta, float& eps) {
   if (!(theta >= 0.f) || !std::isfinite(theta) || !(eps >= 0.f) || !std::isfinite(eps))
     return fail(c, TC_EINVAL, std::string(who) + ": theta and eps must be finite and >= 0");
@@ -470,7 +481,10 @@ int forces_impl(tc_ctx* c, const char* who, float theta, float eps, float* acc, 
     TC_CUDA(c, cudaMalloc((void**)&c->d_pot, sizeof(float) * (size_t)n));
     c->out_cap = n;
   }
-  const size_t warps = (size_t)tc::forces_total_warps(c->n_sm, c->stack_smem);
+  // launch configuration of the fused kernel (tc_kernels.cu): dense from kDenseMinMean particles per group on
+  const bool dense = !c->two_pass && c->stack_smem == 256 &&
+                     (c->kernel_config == 2 || (c->kernel_config == 0 && (double)n >= kDenseMinMean * (double)c->tree.n_groups));
+  const size_t warps = (size_t)(dense ? tc::dense::forces_total_warps(c->n_sm, c->stack_smem) : tc::sparse::forces_total_warps(c->n_sm, c->stack_smem));
   if (c->spill_elems < warps * (size_t)c->spill_cap) {
     cudaFree(c->d_spill); c->d_spill = nullptr; c->spill_elems = 0;
     TC_CUDA(c, cudaMalloc((void**)&c->d_spill, sizeof(uint32_t) * warps * (size_t)c->spill_cap));
@@ -482,7 +496,7 @@ int forces_impl(tc_ctx* c, const char* who, float theta, float eps, float* acc, 
   L.pot = pot ? (acc_dev ? pot : c->d_pot) : nullptr;
   L.n_pc = c->d_npc; L.n_pp = c->d_npp; L.counters = c->d_ctr; L.spill = c->d_spill; L.spill_cap = c->spill_cap;
   L.stack_smem = c->stack_smem; L.n_sm = c->n_sm; L.flags = (c->walk_only ? 1 : 0) | (c->open_rule ? 2 : 0) | (c->quadrupole ? 0 : 4) | (c->group_box ? 8 : 0);
-  L.max_grid = (int)(warps / (size_t)tc::forces_warps_per_cta());
+  L.max_grid = (int)(warps / (size_t)(dense ? tc::dense::forces_warps_per_cta() : tc::sparse::forces_warps_per_cta()));
   if (shard) {
     L.shard_rank = c->shard_rank; L.shard_count = c->shard_count;
     L.shard_out4 = shard_out4; L.shard_cnt2 = shard_cnt2; L.shard_off = c->shard.off;
@@ -490,7 +504,8 @@ int forces_impl(tc_ctx* c, const char* who, float theta, float eps, float* acc, 
   // stream-ordered: no host synchronisation between queued calls; the overflow flag is sticky until collect()
   TC_CUDA(c, cudaMemsetAsync(c->d_ctr, 0, offsetof(tc::DeviceCounters, overflow), c->stream));
   TC_CUDA(c, cudaEventRecord(c->ev0, c->stream));
-  const int le = c->two_pass ? tc::launch_forces_two_pass(c->dview, L, c->tps, c->stream) : tc::launch_forces(c->dview, L, c->stream);
+  const int le = c->two_pass ? tc::launch_forces_two_pass(c->dview, L, c->tps, c->stream)
+                             : dense ? tc::dense::launch_forces(c->dview, L, c->stream) : tc::sparse::launch_forces(c->dview, L, c->stream);
   if (le != 0) return cuda_fail(c, (cudaError_t)le, "forces kernel launch");
   c->last_two_pass = c->two_pass;
   TC_CUDA(c, cudaEventRecord(c->ev1, c->stream));

@@ -137,7 +137,17 @@ int launch_shard_scatter(const DeviceTree& T, const ShardLayout& L, const float*
 
 // Launches the fused walk+evaluate kernel on `stream` (a cudaStream_t).  Returns a
 // cudaError_t as int (0 = success).  Defined in tc_kernels.cu.
+// Two builds of the same kernel source with different launch configurations (tc_kernels.cu / tc_kernels_dense.cu).
+namespace sparse {
 int launch_forces(const DeviceTree& T, const ForceLaunch& L, void* stream);
+int forces_total_warps(int n_sm, int stack_smem);   // warps the persistent grid runs (for sizing the spill buffer)
+int forces_warps_per_cta();
+}  // namespace sparse
+namespace dense {
+int launch_forces(const DeviceTree& T, const ForceLaunch& L, void* stream);
+int forces_total_warps(int n_sm, int stack_smem);
+int forces_warps_per_cta();
+}  // namespace dense
 // Two-pass variant (option "two_pass"): global interaction lists and their scratch, owned by the context.
 struct TwoPassScratch {
   unsigned long long *cnt_c = nullptr, *cnt_l = nullptr, *off_c = nullptr, *off_l = nullptr;
@@ -153,9 +163,6 @@ struct TwoPassScratch {
 // count -> scan -> write lists -> node kernel -> leaf kernel.  cudaError_t as int.
 int launch_forces_two_pass(const DeviceTree& T, const ForceLaunch& L, TwoPassScratch& S, void* stream);
 int two_pass_times(const TwoPassScratch& S, float ms[4]);
-// Number of warps the persistent grid runs (for sizing the spill buffer).
-int forces_total_warps(int n_sm, int stack_smem);
-int forces_warps_per_cta();
 // Scratch of the device-side builder (tc_build_gpu.cu); grow-only, owned by the context.
 struct DeviceBuildScratch {
   unsigned long long *keys = nullptr, *keys_alt = nullptr;  size_t cap_keys = 0, cap_keys_alt = 0;

@@ -34,6 +34,19 @@
 #include "tc_internal.h"
 #include "tc_lanes.h"
 
+// This file is compiled TWICE into libtc_b200.so (tc_kernels_dense.cu includes it with other constants): the launch
+// configuration of the fused kernel is a compile-time matter (warps per CTA, shared-memory capacities, registers), and no
+// single one is best for every tree:
+//   sparse (this file on its own): 4 CTAs x 4 warps per SM, 128 registers, 224-record chunks — many warps hide the walk's
+//          latency when groups are small and the walk is most of the work (N_group = N_leaf = 16: 8.65 ms against 9.39);
+//   dense  (tc_kernels_dense.cu):  4 CTAs x 3 warps per SM, 168 registers, 320-record chunks — fewer, longer evaluation
+//          rounds when groups are large (config 3 at N_group = 128: 5.65 ms against 5.73; N = 2^24: 105.7 against 108.8).
+// tc_api.cpp picks by the mean number of particles per group.  Everything that is not the fused kernel (two-pass variant,
+// direct summation, kicks, FP32 peak) exists once, in the sparse build.
+#ifndef TC_CFG_NS
+#define TC_CFG_NS sparse
+#endif
+
 namespace tc {
 namespace {
 
@@ -782,6 +795,7 @@ forces_kernel(const float4* __restrict__ bnd, const float4* __restrict__ xm, con
   }
 }
 
+#ifndef TC_FORCES_ONLY
 // ---- two-pass variant: the evaluation kernels of Lists 3 and 4 on global lists ------
 // node kernel: warp per group, list chunks gathered to shared memory, acc / pot / n_pc WRITTEN
 __global__ void __launch_bounds__(kWarpsPerCta * 32, TC_MINB)
@@ -868,6 +882,8 @@ leaf_kernel(const float4* __restrict__ part, const int32_t* __restrict__ orig, c
   }
 }
 
+#endif  // TC_FORCES_ONLY
+
 template <int STK, bool kEps0, int MODE = kFused, bool kPlain = false>
 int launch_t(const DeviceTree& T, const ForceLaunch& L, cudaStream_t st, int* ctas_per_sm_out, ListIO lio = ListIO()) {
   auto kern = forces_kernel<STK, kEps0, MODE, kPlain>;
@@ -900,9 +916,24 @@ int dispatch(const DeviceTree& T, const ForceLaunch& L, cudaStream_t st, int* pe
 
 }  // namespace
 
+namespace TC_CFG_NS {
 int launch_forces(const DeviceTree& T, const ForceLaunch& L, void* stream) {
   return dispatch(T, L, (cudaStream_t)stream, nullptr);
 }
+
+int forces_warps_per_cta() { return kWarpsPerCta; }
+
+int forces_total_warps(int n_sm, int stack_smem) {
+  DeviceTree T;
+  ForceLaunch L;
+  L.stack_smem = stack_smem; L.eps = 1.f;
+  int per_sm = 0;
+  if (dispatch(T, L, nullptr, &per_sm) != 0 || per_sm < 1) per_sm = 8;
+  return n_sm * per_sm * kWarpsPerCta;
+}
+}  // namespace TC_CFG_NS
+
+#ifndef TC_FORCES_ONLY
 
 // ---- the paper-literal two-pass variant (option "two_pass") ----
 namespace {
@@ -1226,15 +1257,6 @@ int measure_fp32_peak(int n_sm, void* stream, double* tflops) {
   return 0;
 }
 
-int forces_warps_per_cta() { return kWarpsPerCta; }
-
-int forces_total_warps(int n_sm, int stack_smem) {
-  DeviceTree T;
-  ForceLaunch L;
-  L.stack_smem = stack_smem; L.eps = 1.f;
-  int per_sm = 0;
-  if (dispatch(T, L, nullptr, &per_sm) != 0 || per_sm < 1) per_sm = 8;
-  return n_sm * per_sm * kWarpsPerCta;
-}
+#endif  // TC_FORCES_ONLY
 
 }  // namespace tc
