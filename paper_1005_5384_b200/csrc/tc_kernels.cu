@@ -31,21 +31,27 @@
 #include <algorithm>
 #include <cstdint>
 
-#include "tc_internal.h"
-#include "tc_lanes.h"
-
 // This file is compiled TWICE into libtc_b200.so (tc_kernels_dense.cu includes it with other constants): the launch
 // configuration of the fused kernel is a compile-time matter (warps per CTA, shared-memory capacities, registers), and no
 // single one is best for every tree:
-//   sparse (this file on its own): 4 CTAs x 4 warps per SM, 128 registers, 224-record chunks — many warps hide the walk's
-//          latency when groups are small and the walk is most of the work (N_group = N_leaf = 16: 8.65 ms against 9.39);
-//   dense  (tc_kernels_dense.cu):  4 CTAs x 3 warps per SM, 168 registers, 320-record chunks — fewer, longer evaluation
-//          rounds when groups are large (config 3 at N_group = 128: 5.65 ms against 5.73; N = 2^24: 105.7 against 108.8).
-// tc_api.cpp picks by the mean number of particles per group.  Everything that is not the fused kernel (two-pass variant,
-// direct summation, kicks, FP32 peak) exists once, in the sparse build.
+//   sparse (this file on its own): 4 CTAs x 4 warps per SM, 128 registers, 224-record chunks, no tail in the lane
+//          mapping — many warps hide the walk's latency when groups are small and the walk is most of the work
+//          (N_group = N_leaf = 16: 8.7 ms against 9.4; the tail code alone, never taken there, costs 3 %: registers);
+//   dense  (tc_kernels_dense.cu):  4 CTAs x 3 warps per SM, 168 registers, 320-record chunks, tails of up to 4 particles —
+//          fewer, longer evaluation rounds when groups are large (config 3 at N_group = 128: 5.65 ms against 5.74;
+//          N = 2^24: 105.7 against 108.8).
+// tc_api.cpp picks by the mean number of particles per group (crossover measured at ~24).  Everything that is not the
+// fused kernel (two-pass variant, direct summation, kicks, FP32 peak) exists once, in the sparse build.  The builders'
+// schedules use the lane table of tc_lanes.h with its defaults (the dense one): a cost model, not a contract.
 #ifndef TC_CFG_NS
 #define TC_CFG_NS sparse
+#ifndef TC_MAXTAIL
+#define TC_MAXTAIL 0
 #endif
+#endif
+
+#include "tc_internal.h"
+#include "tc_lanes.h"
 
 namespace tc {
 namespace {

@@ -63,6 +63,11 @@ static_assert(kMaxTail >= 0 && kMaxTail <= 4, "the tail lives in the top two reg
 #ifndef TC_TAIL_OVER
 #define TC_TAIL_OVER 1.0f
 #endif
+#ifndef TC_TAIL_MIN_M
+#define TC_TAIL_MIN_M 24
+#endif
+constexpr int kTailMinM = TC_TAIL_MIN_M;      // no tail below this pass size: small groups' chunks are short and the tail's own loop
+                                              // set-up per chunk costs more than the slots it saves (N_group = 16: 8.65 -> 8.99 ms with tails)
 constexpr float kTailCycles = 47.3f / 32.f;   // cycles per list entry and tail particle: the K = 1 loop at S = 32
 constexpr float kTailOverhead = TC_TAIL_OVER; // per list entry: the tail's own loop set-up per chunk (positions, unpack / repack);
                                               // measured: tail off 5.777 ms, on 5.746 (overhead 0.3) / 5.738 (1.0) at config 3
@@ -80,7 +85,7 @@ struct LaneTable {
     for (int m = 1; m <= kPassCap; m++) {
       int bs = 0, bq = 0, bk = 0, bb = 0;
       float best = 1e30f;
-      for (int mb = 0; mb <= kMaxTail && mb < m; mb++) {
+      for (int mb = 0; mb <= (m >= kTailMinM ? kMaxTail : 0) && mb < m; mb++) {
         const float tail = mb ? kTailCycles * (float)mb + kTailOverhead : 0.f;
         for (int s = 1; s <= 32; s++) {
           const int q = 32 / s;

@@ -133,7 +133,7 @@ def test_device_inputs_device_build_leapfrog_matches_host_build():
 def test_device_build_rejects_bad_particles_and_switches_back_to_host():
     import torch
     pos, mass, *_ = inputs.make("plummer_1k")
-    with B.TreeCode() as tc:
+    with B.TreeCode(n_group=96) as tc:
         tc.set_option("device_build", 1)
         bad = torch.from_numpy(pos).cuda().clone()
         bad[5, 1] = float("nan")

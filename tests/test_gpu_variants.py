@@ -103,7 +103,7 @@ def test_group_box_1m_sampled_groups():
     """R23 at config 3 (full size, the launch configuration of bench.py): counts exact and forces within the bars on
     sampled groups; fewer interactions than the cube rule."""
     pos, mass, theta, eps, n_leaf = inputs.make("plummer_1m")
-    with B.TreeCode() as tc:                                   # default N_group (96)
+    with B.TreeCode() as tc:                                   # default N_group
         tc.set_particles(pos, mass)
         tc.build(n_leaf)
         n_group = tc.stats()["n_group"]
