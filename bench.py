@@ -150,18 +150,19 @@ def sum_over_ranks(x: float, world: int, device=None) -> float:
     return float(t.item())
 
 
-def cpu_baseline(pos, mass, theta, eps, n_leaf, target_s: float = 15.0):
+def cpu_baseline(pos, mass, theta, eps, n_leaf, target_s: float = 30.0):
     """The fp64 oracle as it stands, timed on this box's host cores on a bounded sample of groups (all of them when
     that fits the budget).  Returns (cpu_baseline object, oracle result, group sample) — the result also serves
     the `parity` object: nothing the oracle computes here is thrown away."""
     import oracle
     o = oracle.Oracle(pos, mass, n_leaf, N_GROUP)
     ng = o.n_groups
-    probe = np.unique(np.linspace(0, ng - 1, min(ng, 128)).astype(np.int64))
+    probe = np.unique(np.linspace(0, ng - 1, min(ng, 256)).astype(np.int64))
+    o.forces(theta, eps, shadow32=True, groups=probe[:16])       # spin the OpenMP threads up before the probe is timed
     t0 = time.perf_counter()
     r = o.forces(theta, eps, shadow32=True, groups=probe)
     dt = time.perf_counter() - t0
-    k = int(min(ng, max(len(probe), len(probe) * target_s / max(dt, 1e-3))))
+    k = int(min(ng, max(len(probe), len(probe) * target_s / max(dt, 1e-3))))   # all groups when that fits target_s (it does: ~5 s)
     sel = np.unique(np.linspace(0, ng - 1, k).astype(np.int64))
     t0 = time.perf_counter()
     r = o.forces(theta, eps, shadow32=True, groups=sel, stats=True)
