@@ -205,3 +205,44 @@ def test_binding_checks_dtype_and_shape_before_the_c_call():
             B.tc_forces(tc.ctx, theta, eps, np.empty((len(mass), 3), np.float32), np.empty(len(mass) + 1, np.float32))
         with pytest.raises(TypeError):
             B.tc_direct(tc.ctx, eps, None, np.empty((len(mass), 3), np.float32))
+
+
+@pytest.mark.parametrize("cfg", [1, 2])
+def test_both_launch_configurations_match_the_oracle(cfg):
+    """The fused kernel exists in two builds (sparse / dense, option kernel_config): each is forced
+    here on small AND large groups, coincident particles (a level-21 leaf above the pass size), eps = 0, a variant
+    reading, the stack-spill-sized walk and a sharded evaluation — same lists, same tolerances."""
+    import torch
+    pos, mass = inputs.plummer(12000, 41)
+    pos[:150] = pos[0]
+    for n_leaf, n_group, theta, eps, extra in [(16, 128, 0.5, 0.01, {}), (4, 8, 0.4, 0.0, {}), (16, 96, 0.6, 0.01, {"open_rule": 1, "group_box": 1}),
+                                               (8, 256, 0.3, 0.01, {"quadrupole": 0})]:
+        opts = dict(extra, kernel_config=cfg)
+        acc, pot, n_pc, n_pp, st = gpu_forces(pos, mass, theta, eps, n_leaf, n_group, opts=opts)
+        o = Oracle(pos, mass, n_leaf, n_group, open_rule=extra.get("open_rule", 0), quadrupole=bool(extra.get("quadrupole", 1)),
+                   group_box=bool(extra.get("group_box", 0)))
+        check(acc, pot, n_pc, n_pp, o.forces(theta, eps, shadow32=True))
+    # the two builds agree with each other to summation-order rounding, and a sharded evaluation in a forced build
+    # is bit for bit the unsharded one of the same build
+    n = len(mass)
+    with B.TreeCode(n_group=128) as tc:
+        tc.set_option("kernel_config", cfg)
+        tc.set_particles(pos, mass)
+        tc.build(16)
+        a0, p0 = tc.forces(0.5, 0.01)
+        tc.set_option("shard_count", 3)
+        ns = tc.shard_size()
+        g = torch.zeros((3, ns, 4), dtype=torch.float32, device="cuda")
+        for r in range(3):
+            tc.set_option("shard_rank", r)
+            tc.forces_shard(0.5, 0.01, g[r])
+        acc = torch.empty((n, 3), dtype=torch.float32, device="cuda"); pot = torch.empty(n, dtype=torch.float32, device="cuda")
+        tc.shard_scatter(g, None, acc, pot)
+        tc.sync()
+        assert np.array_equal(acc.cpu().numpy(), a0) and np.array_equal(pot.cpu().numpy(), p0)
+        tc.set_option("shard_count", 1); tc.set_option("shard_rank", 0)
+        tc.set_option("kernel_config", 3 - cfg)
+        a1, _ = tc.forces(0.5, 0.01)
+        assert rel_err(a1.astype(np.float64), a0.astype(np.float64)).max() <= 5e-5
+        with pytest.raises(B.TcError):
+            tc.set_option("kernel_config", 3)
