@@ -33,6 +33,7 @@ struct tc_ctx {
   int walk_only = 0, open_rule = 0, quadrupole = 1, group_box = 0;
   int shard_rank = 0, shard_count = 1;
   int kernel_config = 0;              // option "kernel_config": 0 = by the mean group size, 1 = sparse, 2 = dense (tc_kernels.cu)
+  size_t grid_warps[2][2] = {{0, 0}, {0, 0}};   // warps of the persistent grid, cached: [dense][stack_smem == 64]
   bool two_pass = false;
   tc::TwoPassScratch tps;
   bool last_two_pass = false;
@@ -484,7 +485,10 @@ int forces_impl(tc_ctx* c, const char* who, float theta, float eps, float* acc, 
   // launch configuration of the fused kernel (tc_kernels.cu): dense from kDenseMinMean particles per group on
   const bool dense = !c->two_pass && c->stack_smem == 256 &&
                      (c->kernel_config == 2 || (c->kernel_config == 0 && (double)n >= kDenseMinMean * (double)c->tree.n_groups));
-  const size_t warps = (size_t)(dense ? tc::dense::forces_total_warps(c->n_sm, c->stack_smem) : tc::sparse::forces_total_warps(c->n_sm, c->stack_smem));
+  size_t& warps_cached = c->grid_warps[dense ? 1 : 0][c->stack_smem == 64 ? 1 : 0];
+  if (!warps_cached)   // (an occupancy query: once per configuration, not per call)
+    warps_cached = (size_t)(dense ? tc::dense::forces_total_warps(c->n_sm, c->stack_smem) : tc::sparse::forces_total_warps(c->n_sm, c->stack_smem));
+  const size_t warps = warps_cached;
   if (c->spill_elems < warps * (size_t)c->spill_cap) {
     cudaFree(c->d_spill); c->d_spill = nullptr; c->spill_elems = 0;
     TC_CUDA(c, cudaMalloc((void**)&c->d_spill, sizeof(uint32_t) * warps * (size_t)c->spill_cap));
