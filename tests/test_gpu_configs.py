@@ -19,6 +19,7 @@ from paper_1005_5384_b200 import inputs
 from test_gpu_parity import check, rel_err
 
 pytestmark = pytest.mark.gpu
+N_GROUP = 128          # the library's default and bench.py's setting
 ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 
 
@@ -46,7 +47,7 @@ def test_config4_accuracy_versus_time_1m():
         d_acc = torch.empty((n, 3), dtype=torch.float32, device="cuda")
         d_pot = torch.empty(n, dtype=torch.float32, device="cuda")
         for n_leaf in (8, 16, 32):
-            with B.TreeCode(n_group=64) as tc:
+            with B.TreeCode(n_group=N_GROUP) as tc:
                 tc.set_stream(st.cuda_stream)
                 tc.set_particles(pos, mass)
                 tc.build(n_leaf)
@@ -79,9 +80,9 @@ def test_config4_oracle_parity_at_every_sweep_point_1m():
     """Oracle parity on sampled groups at ALL twelve (theta, N_leaf) points of config 4, full size."""
     pos, mass, _, eps, _ = inputs.make("plummer_1m")
     for n_leaf in (8, 16, 32):
-        o = Oracle(pos, mass, n_leaf, 64)
+        o = Oracle(pos, mass, n_leaf, N_GROUP)
         gsel = np.arange(7 + n_leaf, o.n_groups, o.n_groups // 192, dtype=np.int64)
-        with B.TreeCode(n_group=64) as tc:
+        with B.TreeCode(n_group=N_GROUP) as tc:
             tc.set_particles(pos, mass)
             tc.build(n_leaf)
             for theta in (0.3, 0.5, 0.75, 1.0):
@@ -114,7 +115,7 @@ def test_config5_two_plummer_16m_parity_and_leapfrog():
     device-side leapfrog (`tc_leapfrog`, device tree build) ending in the same state."""
     import torch
     from paper_1005_5384_b200 import integrate
-    n, theta, eps, n_leaf, dt, steps, n_group = 1 << 24, 0.5, 0.005, 16, 1.0 / 128, 10, 64
+    n, theta, eps, n_leaf, dt, steps, n_group = 1 << 24, 0.5, 0.005, 16, 1.0 / 128, 10, N_GROUP
     pos, mass, vel = inputs.two_plummer(n, with_velocities=True)
     st = torch.cuda.Stream()
     with torch.cuda.stream(st), B.TreeCode(n_group=n_group) as tc:
