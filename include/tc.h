@@ -165,7 +165,8 @@ int tc_set_stream(tc_ctx* ctx, void* cuda_stream);
 int tc_sync(tc_ctx* ctx);
 
 /* Message of the last error of this context ("" if none).  Owned by the context.
- * ctx == NULL returns the message of the last failed tc_create.                  */
+ * ctx == NULL returns the message of the last failed tc_create or tc_direct_static
+ * on the calling thread.                                                          */
 const char* tc_last_error(const tc_ctx* ctx);
 
 /* Inspection of the packed host tree of the last tc_build (tests of the host
@@ -214,6 +215,51 @@ int tc_get_group_boxes(tc_ctx* ctx, float* half_ext);
  * Errors: TC_ESTATE (no particles / host-only), TC_EINVAL (null acc, bad eps, target out of range),
  * TC_ENOMEM, TC_ECUDA.                                                                              */
 int tc_direct(tc_ctx* ctx, float eps, const int64_t* targets, int64_t n_targets, double* acc, double* pot);
+
+/* ---- Direct summation WITHOUT any allocation -----------------------------------------------------------------
+ * For whom: code that is not allowed to obtain device memory at the moment it needs forces.  Examples: a plugin
+ * running inside a host application whose memory pool owns the whole GPU and hands out fixed buffers (a cudaMalloc
+ * from a guest library would fail or fragment the pool); a real-time or in-situ analysis step that may not take
+ * the driver's allocation lock, which can stall for milliseconds and synchronises the device on cudaFree; a
+ * process that has already filled the 180 GB with its own data.  Every other entry point of this library creates a
+ * context (tc_create) and grows device buffers on demand; this one does neither.
+ *
+ * What it computes: exactly tc_direct (same kernels, same arithmetic):
+ *   a_i = sum_{j != i} m_j (x_j - x_i) / s^3,  phi_i = -sum_{j != i} m_j / s,  s^2 = |x_j - x_i|^2 + eps^2
+ * over the n particles given in THIS call, for the targets listed.
+ *   pos [n,3] fp32, mass [n] fp32                INPUTS, device, caller's order, not modified
+ *   targets [n_targets] int64 or NULL            device; NULL = all n particles (n_targets ignored).  Indices must lie
+ *                                                in [0, n): they are NOT checked (checking would need a read-back);
+ *                                                a negative index leaves its output row at zero
+ *   acc [n_targets,3] fp64, pot [n_targets] fp64 or NULL     OUTPUTS, device, owned by the caller; zeroed, then written
+ *   cuda_stream                                  a cudaStream_t as void*; NULL = the legacy default stream.  All work is
+ *                                                queued on it and the call returns without synchronising: order your
+ *                                                reads of acc / pot after it on the same stream (or synchronise it).
+ * Inputs are not validated beyond the sizes (a NaN position gives NaN results).
+ *
+ * Where the working memory comes from: the kernel reads its sources as one packed (x, y, z, m) array.  Here that
+ * array is a fixed block of TC_DIRECT_STATIC_MAX_N x 16 bytes = 4 MiB inside the library image; EVERY GPU that loads
+ * libtc_b200.so holds these 4 MiB from the first use of the library on that GPU until the process exits, whether
+ * or not this function is ever called.  n and n_targets beyond TC_DIRECT_STATIC_MAX_N are refused with TC_EINVAL
+ * and a message naming the limit (use tc_direct then).  The function itself calls no cudaMalloc, cudaFree, or any
+ * library routine that allocates device memory.
+ *
+ * First call on each device: it looks up the block's address on the current device (cudaGetSymbolAddress) and the
+ * SM count, once, under a lock; later calls only launch.  Make that first call during set-up, outside any CUDA
+ * stream capture (the look-up is not a stream operation and may initialise the module).
+ *
+ * Sharing: there is ONE block per GPU, shared by every caller in the process, and it keeps what the last call put
+ * there.  Nothing in it has to start at zero (each call rewrites entries 0 .. n-1 before reading them and reads no
+ * others), so consecutive calls on one stream are independent.  Two calls that can run on the GPU at the same time
+ * — different streams, or different host threads with their own streams — overwrite each other's sources: that is
+ * a data race with wrong results and no error.  Serialise them (one stream, or an event between them).
+ *
+ * Errors: TC_EINVAL (null pos / mass / acc, n or n_targets < 1 or above the limit, eps negative or non-finite,
+ * a host pointer), TC_ECUDA (no device, not sm_100, symbol look-up or launch failed).  The message is returned by
+ * tc_last_error(NULL) on the calling thread.                                                                       */
+#define TC_DIRECT_STATIC_MAX_N 262144
+int tc_direct_static(const float* pos, const float* mass, int64_t n, float eps, const int64_t* targets,
+                     int64_t n_targets, double* acc, double* pot, void* cuda_stream);
 
 /* ---- ONE force evaluation over k GPUs ------------------------------------
  * Groups are independent given the read-only tree (one walk per group, nothing is exchanged between

@@ -27,7 +27,10 @@ TC_FLAG_HOST_ONLY = 1
 SYMBOLS = ["tc_create", "tc_create_ex", "tc_destroy", "tc_set_particles", "tc_build", "tc_forces",
            "tc_set_option", "tc_get_counts", "tc_get_stats", "tc_set_stream", "tc_sync",
            "tc_last_error", "tc_get_tree", "tc_get_group_boxes", "tc_leapfrog", "tc_fp32_peak", "tc_direct",
-           "tc_shard_size", "tc_forces_shard", "tc_shard_scatter"]
+           "tc_shard_size", "tc_forces_shard", "tc_shard_scatter", "tc_direct_static"]
+
+#: most sources / targets tc_direct_static accepts (TC_DIRECT_STATIC_MAX_N of include/tc.h: its 4 MiB static block)
+TC_DIRECT_STATIC_MAX_N = 262144
 
 
 class tc_stats(C.Structure):
@@ -86,6 +89,7 @@ def lib():
     L.tc_shard_size.argtypes = [vp, C.POINTER(C.c_int64)]
     L.tc_forces_shard.argtypes = [vp, f32, f32, vp, vp]
     L.tc_shard_scatter.argtypes = [vp, vp, vp, vp, vp, vp, vp]
+    L.tc_direct_static.argtypes = [vp, vp, i64, f32, vp, i64, vp, vp, vp]
     _lib = L
     return L
 
@@ -206,6 +210,23 @@ def tc_direct(ctx, eps: float, targets, acc, pot=None):
         assert isinstance(targets, np.ndarray) and targets.dtype == np.int64, "targets must be a host int64 array"
     _check(ctx, lib().tc_direct(ctx, float(eps), _ptr(targets, np.int64, (nt,), "targets"), nt, _ptr(acc, np.float64, (None, 3), "acc"),
                                 _ptr(pot, np.float64, (acc.shape[0],), "pot")))
+
+
+def tc_direct_static(pos, mass, eps: float, targets, acc, pot=None, cuda_stream: int = 0):
+    """Direct summation for callers that may not allocate device memory (a plugin inside an application whose pool
+    owns the GPU, a latency-critical step that must stay clear of the allocator's lock, a full device): no context,
+    no cudaMalloc — the packed sources live in a 4 MiB block inside the library, one per GPU, shared by all callers.
+
+    Every array is a torch CUDA tensor of the caller: pos [n,3] / mass [n] float32, targets int64 [n_t] or None (all),
+    acc [n_t,3] / pot [n_t] float64 outputs.  Work is queued on `cuda_stream` (0 = legacy default stream), nothing is
+    synchronised.  n, n_t <= TC_DIRECT_STATIC_MAX_N or TcError(TC_EINVAL).  Calls that overlap on the GPU race on
+    the shared block; make the first call per device outside stream capture (include/tc.h has the full contract)."""
+    n = int(mass.shape[0])
+    nt = 0 if targets is None else int(targets.shape[0])
+    rc = lib().tc_direct_static(_ptr(pos, np.float32, (n, 3), "pos"), _ptr(mass, np.float32, (n,), "mass"), n, float(eps),
+                                _ptr(targets, np.int64, (nt,), "targets"), nt, _ptr(acc, np.float64, (None, 3), "acc"),
+                                _ptr(pot, np.float64, (acc.shape[0],), "pot"), C.c_void_p(cuda_stream))
+    _check(None, rc)
 
 
 def tc_shard_size(ctx) -> int:

@@ -637,6 +637,17 @@ int tc_direct(tc_ctx* c, float eps, const int64_t* targets, int64_t n_targets, d
   return TC_OK;
 }
 
+// No context, no allocation: everything happens in tc::direct_static (tc_kernels.cu, next to the static array it uses).
+int tc_direct_static(const float* pos, const float* mass, int64_t n, float eps, const int64_t* targets, int64_t n_targets,
+                     double* acc, double* pot, void* cuda_stream) {
+  static_assert(sizeof(long long) == sizeof(int64_t), "int64_t layout");
+  std::string msg;
+  const int rc = tc::direct_static(pos, mass, (long long)n, eps, reinterpret_cast<const long long*>(targets), (long long)n_targets,
+                                   acc, pot, cuda_stream, msg);
+  if (rc != TC_OK) g_create_err = msg;
+  return rc;
+}
+
 int tc_leapfrog(tc_ctx* c, float* pos, float* vel, const float* mass, int64_t n, float dt, int steps, int n_leaf,
                 float theta, float eps, float* acc, float* pot, int have_acc) {
   if (!c) return TC_EINVAL;

@@ -198,6 +198,10 @@ int pack_src_device(const float* pos, const float* mass, int64_t n, float4* out,
 // acc [n_t,3] / pot [n_t] device fp64 (zeroed inside).  Returns a cudaError_t as int.
 int launch_direct(const float4* src, long long n, const long long* targets, long long n_t, float eps, double* acc,
                   double* pot, int n_sm, void* stream);
+// tc_direct_static: the same direct sum with its source array in a static __device__ block (no allocation of any kind;
+// tc_kernels.cu).  All pointers DEVICE.  Returns TC_OK or a TC_E* code with msg set.
+int direct_static(const float* pos, const float* mass, long long n, float eps, const long long* targets, long long n_targets,
+                  double* acc, double* pot, void* stream, std::string& msg);
 // Leapfrog pieces (tc_leapfrog): v += a dt/2 ; x += v dt  and  v += a dt/2 over [n,3] device arrays
 // (16-byte aligned).  Return a cudaError_t as int.
 int launch_kick_drift(float* pos, float* vel, const float* acc, long long n, float dt, int n_sm, void* stream);

@@ -29,7 +29,10 @@
 #include <cub/device/device_scan.cuh>
 
 #include <algorithm>
+#include <cmath>
 #include <cstdint>
+#include <mutex>
+#include <string>
 
 // This file is compiled TWICE into libtc_b200.so (tc_kernels_dense.cu includes it with other constants): the launch
 // configuration of the fused kernel is a compile-time matter (warps per CTA, shared-memory capacities, registers), and no
@@ -1157,6 +1160,86 @@ int launch_direct(const float4* src, long long n, const long long* targets, long
   if (eps * eps == 0.f) direct_kernel<true><<<grid, kDirThreads, 0, st>>>(src, n, targets, n_t, eps, acc, pot);
   else direct_kernel<false><<<grid, kDirThreads, 0, st>>>(src, n, targets, n_t, eps, acc, pot);
   return (int)cudaGetLastError();
+}
+
+// ---- tc_direct_static: the direct sum for callers that must not allocate (include/tc.h) -------------------------------
+// tc_direct keeps the sources as one (x, y, z, m) float4 array that its context cudaMallocs.  This variant keeps that array
+// in the library image instead: a file-scope __device__ array, resident on every GPU that loads the library from the moment
+// the module is loaded until the process exits.  `g_static_src` below is, in HOST code, only the handle of that symbol — not
+// a device address: a kernel must be given what cudaGetSymbolAddress returns for the CURRENT device (taken once per device,
+// below).  Same kernels and same launcher as tc_direct from there on.
+static_assert(TC_DIRECT_STATIC_MAX_N == 262144, "include/tc.h documents 4 MiB of static device memory per GPU");
+static __device__ __align__(256) float4 g_static_src[TC_DIRECT_STATIC_MAX_N];
+
+namespace {
+// pos [n,3], mass [n] -> src [n] (x, y, z, m): every entry a later read may touch (0 .. n-1) is written here first, so the
+// contents a previous call left behind are never read and nothing needs clearing
+__global__ void __launch_bounds__(256) pack_static_kernel(const float* __restrict__ pos, const float* __restrict__ mass,
+                                                          long long n, float4* __restrict__ src) {
+  const long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  src[i] = make_float4(__ldg(pos + 3 * i), __ldg(pos + 3 * i + 1), __ldg(pos + 3 * i + 2), __ldg(mass + i));
+}
+
+constexpr int kStaticMaxDevices = 64;
+struct StaticDevice { float4* src = nullptr; int n_sm = 0; bool ready = false; };
+StaticDevice g_static_dev[kStaticMaxDevices];
+std::mutex g_static_mutex;
+
+bool on_device(const void* p) {
+  cudaPointerAttributes a;
+  if (cudaPointerGetAttributes(&a, p) != cudaSuccess) { cudaGetLastError(); return false; }
+  return a.type == cudaMemoryTypeDevice || a.type == cudaMemoryTypeManaged;
+}
+}  // namespace
+
+int direct_static(const float* pos, const float* mass, long long n, float eps, const long long* targets, long long n_targets,
+                  double* acc, double* pot, void* stream, std::string& msg) {
+  auto bad = [&](int code, const std::string& m) { msg = "tc_direct_static: " + m; return code; };
+  if (!pos || !mass || !acc) return bad(TC_EINVAL, "pos, mass and acc must not be null");
+  if (n < 1) return bad(TC_EINVAL, "n must be >= 1");
+  if (n > (long long)TC_DIRECT_STATIC_MAX_N)
+    return bad(TC_EINVAL, "n = " + std::to_string(n) + " exceeds TC_DIRECT_STATIC_MAX_N = " + std::to_string(TC_DIRECT_STATIC_MAX_N) +
+                              " (the static scratch holds no more sources; use tc_direct, which allocates)");
+  const long long nt = targets ? n_targets : n;
+  if (nt < 1) return bad(TC_EINVAL, "n_targets must be >= 1");
+  if (nt > (long long)TC_DIRECT_STATIC_MAX_N)
+    return bad(TC_EINVAL, "n_targets = " + std::to_string(nt) + " exceeds TC_DIRECT_STATIC_MAX_N = " + std::to_string(TC_DIRECT_STATIC_MAX_N));
+  if (!(eps >= 0.f) || !std::isfinite(eps)) return bad(TC_EINVAL, "eps must be finite and >= 0");
+  if (eps < 1e-10f) eps = 0.f;                                   // as tc_direct
+  int dev = -1;
+  cudaError_t e = cudaGetDevice(&dev);
+  if (e != cudaSuccess) return bad(TC_ECUDA, std::string("cudaGetDevice: ") + cudaGetErrorString(e) + " (there is no CPU fallback)");
+  if (dev < 0 || dev >= kStaticMaxDevices) return bad(TC_EINVAL, "device ordinal " + std::to_string(dev) + " is beyond the table of " + std::to_string(kStaticMaxDevices));
+  if (!on_device(pos) || !on_device(mass) || !on_device(acc) || (pot && !on_device(pot)) || (targets && !on_device(targets)))
+    return bad(TC_EINVAL, "every buffer must be a DEVICE pointer (this entry point has nowhere to stage host data)");
+  StaticDevice D;
+  {
+    std::lock_guard<std::mutex> lock(g_static_mutex);
+    StaticDevice& S = g_static_dev[dev];
+    if (!S.ready) {                                               // set-up, once per device, with that device current
+      int major = 0, n_sm = 0;
+      e = cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, dev);
+      if (e == cudaSuccess) e = cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev);
+      if (e != cudaSuccess) return bad(TC_ECUDA, std::string("cudaDeviceGetAttribute: ") + cudaGetErrorString(e));
+      if (major < 10) return bad(TC_ECUDA, "this library is built for sm_100a (B200) only");
+      void* p = nullptr;
+      e = cudaGetSymbolAddress(&p, g_static_src);                 // the array's address on THIS device
+      if (e != cudaSuccess || !p) {
+        cudaGetLastError();
+        return bad(TC_ECUDA, std::string("cudaGetSymbolAddress(g_static_src): ") + cudaGetErrorString(e));
+      }
+      S.src = static_cast<float4*>(p); S.n_sm = n_sm; S.ready = true;
+    }
+    D = S;
+  }
+  cudaStream_t st = (cudaStream_t)stream;
+  pack_static_kernel<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(pos, mass, n, D.src);
+  e = cudaGetLastError();
+  if (e != cudaSuccess) return bad(TC_ECUDA, std::string("pack kernel launch: ") + cudaGetErrorString(e));
+  const int le = launch_direct(D.src, n, targets, nt, eps, acc, pot, D.n_sm, stream);   // memset of acc / pot + direct_kernel
+  if (le != 0) return bad(TC_ECUDA, std::string("direct-sum kernel launch: ") + cudaGetErrorString((cudaError_t)le));
+  return TC_OK;
 }
 
 // ---- tc_leapfrog: the kicks and the drift of a KDK step (BASELINE.json config 5), element-wise over [3n]
