@@ -157,7 +157,11 @@ int tc_get_counts(tc_ctx* ctx, int32_t* n_pc, int32_t* n_pp);
 int tc_get_stats(tc_ctx* ctx, tc_stats* out);
 
 /* Use the caller's CUDA stream (a cudaStream_t passed as void*; NULL = the
- * context's own stream).  The context never destroys a caller's stream.         */
+ * context's own stream).  The context never destroys a caller's stream.
+ * The own stream is created cudaStreamNonBlocking: it is NOT ordered with the
+ * legacy default stream.  The raw handle of the legacy default stream is 0 = NULL,
+ * so to queue the context's work on it pass cudaStreamLegacy ((cudaStream_t)0x1),
+ * or cudaStreamPerThread for the per-thread default stream.                      */
 int tc_set_stream(tc_ctx* ctx, void* cuda_stream);
 
 /* Block until all work queued by this context has finished; returns TC_ECUDA /

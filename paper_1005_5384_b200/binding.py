@@ -173,6 +173,19 @@ def tc_set_stream(ctx, cuda_stream: int):
     _check(ctx, lib().tc_set_stream(ctx, C.c_void_p(cuda_stream)))
 
 
+#: cudaStreamLegacy of cuda_runtime_api.h: the handle that NAMES the legacy default stream.  The raw handle of that
+#: stream is 0, which tc_set_stream reads as "the context's own (non-blocking) stream" — not ordered with it at all.
+CUDA_STREAM_LEGACY = 0x1
+
+
+def torch_stream_handle(device=None) -> int:
+    """Handle of torch's CURRENT stream on `device` in the form tc_set_stream needs: torch's default stream is the
+    legacy default stream (handle 0) and is passed as cudaStreamLegacy, any other stream as itself."""
+    import torch
+    h = int(torch.cuda.current_stream(device).cuda_stream)
+    return h if h != 0 else CUDA_STREAM_LEGACY
+
+
 def tc_sync(ctx):
     _check(ctx, lib().tc_sync(ctx))
 
@@ -335,3 +348,8 @@ class TreeCode:
 
     def set_stream(self, s):
         tc_set_stream(self.ctx, s)
+
+    def use_torch_stream(self, device=None):
+        """Queue the context's work on torch's current stream (default stream included): torch ops before and after a
+        call with device pointers are then ordered with it."""
+        tc_set_stream(self.ctx, torch_stream_handle(device))

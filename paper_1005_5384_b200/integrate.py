@@ -34,8 +34,10 @@ def leapfrog_kdk(tc: "B.TreeCode", pos, vel, mass, dt: float, steps: int, theta:
     `state`, if given, receives the accelerations and potentials of the last force evaluation (`acc`, `pot`).
     The library works on its own stream: it is pointed at torch's current stream here, so that the torch
     kicks / drift and the library's reads of `pos` are ordered (tc.h: device pointers are stream-ordered).
+    Torch's default stream has the raw handle 0, which tc_set_stream takes as "the context's own stream":
+    `use_torch_stream` passes it as cudaStreamLegacy instead.
     """
-    tc.set_stream(torch.cuda.current_stream(pos.device).cuda_stream)
+    tc.use_torch_stream(pos.device)
     n = pos.shape[0]
     dev = pos.device
     acc = torch.empty((n, 3), dtype=torch.float32, device=dev)

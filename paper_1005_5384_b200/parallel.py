@@ -39,8 +39,9 @@ def all_gather_rows(rows: "torch.Tensor", group=None) -> "torch.Tensor":
 def forces_sharded(tc, theta: float, eps: float, acc: "torch.Tensor", pot: "torch.Tensor | None" = None, group=None,
                    n_pc: "torch.Tensor | None" = None, n_pp: "torch.Tensor | None" = None, scratch: dict | None = None) -> None:
     """This rank's shard, the all-gather, the scatter: acc [n,3] / pot [n] (and the counts, if asked for) end up
-    complete and in the caller's order on EVERY rank.  Device tensors; stream-ordered on torch's current stream
-    (the context must have been pointed at it with ``tc.set_stream``).
+    complete and in the caller's order on EVERY rank.  Device tensors; stream-ordered on torch's current stream:
+    the context is pointed at it here (``use_torch_stream``; the default stream, raw handle 0, goes in as
+    cudaStreamLegacy), because the all-gather between the shard kernel and the scatter waits on that stream only.
 
     Every rank must have called set_particles / build with the same particles and options.  `tc` is a
     ``binding.TreeCode`` (anything with set_option / shard_size / forces_shard / shard_scatter works: the CPU test
@@ -48,6 +49,8 @@ def forces_sharded(tc, theta: float, eps: float, acc: "torch.Tensor", pot: "torc
     """
     world = dist.get_world_size(group) if dist.is_initialized() else 1
     rank = dist.get_rank(group) if dist.is_initialized() else 0
+    if acc.is_cuda:
+        tc.use_torch_stream(acc.device)
     tc.set_option("shard_count", world)
     tc.set_option("shard_rank", rank)
     try:

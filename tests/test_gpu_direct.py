@@ -73,7 +73,7 @@ def test_direct_device_pointers_and_errors():
             tc.direct(0.01)
         assert e.value.code == B.TC_ESTATE
         tc.set_particles(pos, mass)
-        tc.set_stream(torch.cuda.current_stream().cuda_stream)
+        tc.use_torch_stream()
         d_acc = torch.empty((1024, 3), dtype=torch.float64, device="cuda")
         d_pot = torch.empty(1024, dtype=torch.float64, device="cuda")
         B.tc_direct(tc.ctx, 0.01, None, d_acc, d_pot)

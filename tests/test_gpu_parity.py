@@ -33,7 +33,7 @@ def gpu_forces(pos, mass, theta, eps, n_leaf, n_group, device=False, opts=None):
             tc.set_option(k, v)
         if device:
             import torch
-            tc.set_stream(torch.cuda.current_stream().cuda_stream)
+            tc.use_torch_stream()
             d_pos, d_mass = torch.from_numpy(pos).cuda(), torch.from_numpy(mass).cuda()
             d_acc = torch.full((n, 3), float("nan"), dtype=torch.float32, device="cuda")
             d_pot = torch.full((n,), float("nan"), dtype=torch.float32, device="cuda")

@@ -142,7 +142,7 @@ def test_forces_sharded_single_process_is_the_plain_call():
     pos, mass, theta, eps, n_leaf = inputs.make("plummer_1k")
     n = len(mass)
     with B.TreeCode() as tc:
-        tc.set_stream(torch.cuda.current_stream().cuda_stream)
+        tc.use_torch_stream()
         tc.set_particles(pos, mass)
         tc.build(n_leaf)
         a0, p0 = tc.forces(theta, eps)
