@@ -76,16 +76,21 @@ struct LaneMap {
   unsigned char S, q, K, mB;   // mB: particles of the tail (the mapping covers m - mB)
 };
 
-struct LaneTable {
+// The table is a TEMPLATE over the tail limit: libtc_b200.so holds translation units with different limits (the sparse kernel
+// build has none, the dense build and the builders' cost model use 4), and one class name with two different inline
+// constructors would break the one-definition rule.  LaneTableT<0> and LaneTableT<4> are simply different types.
+template <int MaxTail>
+struct LaneTableT {
+  static_assert(MaxTail >= 0 && MaxTail <= 4, "the tail lives in the top two register pairs");
   LaneMap map[kPassCap + 1];
   int cost8[kPassCap + 1];    // cycles per list entry of a pass over m particles, in units of 1/8 cycle
-  constexpr LaneTable() : map{}, cost8{} {
+  constexpr LaneTableT() : map{}, cost8{} {
     map[0] = LaneMap{1, 32, 1, 0};
     cost8[0] = 0;
     for (int m = 1; m <= kPassCap; m++) {
       int bs = 0, bq = 0, bk = 0, bb = 0;
       float best = 1e30f;
-      for (int mb = 0; mb <= (m >= kTailMinM ? kMaxTail : 0) && mb < m; mb++) {
+      for (int mb = 0; mb <= (m >= kTailMinM ? MaxTail : 0) && mb < m; mb++) {
         const float tail = mb ? kTailCycles * (float)mb + kTailOverhead : 0.f;
         for (int s = 1; s <= 32; s++) {
           const int q = 32 / s;
@@ -99,13 +104,26 @@ struct LaneTable {
       cost8[m] = (int)(best * 8.f + 0.5f);
     }
   }
+  // every pass size has a mapping, no tail is longer than the limit the kernel of this translation unit was compiled for
+  // (a longer one would leave the last particles of a pass unevaluated, silently), and mapping + tail cover the pass
+  constexpr bool consistent() const {
+    for (int m = 1; m <= kPassCap; m++) {
+      const LaneMap& l = map[m];
+      if (l.mB > MaxTail || l.S < 1 || l.q != 32 / l.S || l.K < 1 || l.K > kMaxK) return false;
+      if ((int)l.q * l.K < m - l.mB || l.K / 2 + (l.mB + 1) / 2 > kMaxK / 2) return false;
+    }
+    return true;
+  }
 };
+using LaneTable = LaneTableT<kMaxTail>;   // the table of THIS translation unit
+static_assert(LaneTable().consistent(), "lane table: a mapping exceeds this build's tail limit or does not cover its pass");
 
 // Cost class of a whole group of `cnt` particles for the schedule (costly groups run first): cycles per
 // list entry in 1/8 cycles, integer so that the host and the device builder agree bit for bit; <= kMaxCostClass.
 // `shift` coarsens the classes (schedule_class_shift below): inside a class the groups stay in Morton order.
 constexpr int kMaxCostClass = 1000000;
-TC_HD constexpr int group_cost_class(const LaneTable& t, long long cnt, int shift) {
+template <int MaxTail>
+TC_HD constexpr int group_cost_class(const LaneTableT<MaxTail>& t, long long cnt, int shift) {
   const long long c = ((cnt / kPassCap) * (long long)t.cost8[kPassCap] + (long long)t.cost8[cnt % kPassCap]) >> shift;
   return c > kMaxCostClass ? kMaxCostClass : (int)c;
 }
