@@ -50,6 +50,8 @@ PAPER_FLOPS_PC, PAPER_FLOPS_PP = 70, 38
 N_SM, LANES = 148, 128
 L2_FLUSH_BYTES = 256 << 20        # > 126 MB L2
 ACC_Q999, ACC_MAX, POT_MAX = 1e-4, 1e-3, 1e-4      # north_star tolerances
+# SURVEY.md 8(d)'s own count (one flop fewer per interaction than the SASS convention above)
+SURVEY_FLOPS_PC, SURVEY_FLOPS_PP = 53, 19
 TRAFFIC_JSON = os.path.join(ROOT, "profiles", "traffic.json")   # DRAM bytes per launch from committed ncu captures
 
 
@@ -65,11 +67,32 @@ def measured_peaks() -> dict:
         return {}
 
 
+KERNEL_SOURCES = ["tc_kernels.cu", "tc_kernels_dense.cu", "tc_lanes.h", "tc_internal.h"]   # what tc::forces_kernel is compiled from
+
+
+def kernel_source_sha16() -> str:
+    """sha256 (first 16 hex digits) over the sources of the force kernel, in KERNEL_SOURCES order."""
+    import hashlib
+    h = hashlib.sha256()
+    for name in KERNEL_SOURCES:
+        with open(os.path.join(ROOT, "paper_1005_5384_b200", "csrc", name), "rb") as f:
+            h.update(f.read())
+    return h.hexdigest()[:16]
+
+
 def traffic(key: str):
-    """DRAM bytes of one launch (dram__bytes_read.sum + dram__bytes_write.sum) of a committed ncu capture, or None."""
+    """DRAM bytes of one launch (dram__bytes_read.sum + dram__bytes_write.sum) of a committed ncu capture, or None.
+    The capture is a static file: `traffic_stale` says whether the kernel sources have changed since it was taken
+    (profiles/traffic.json records their hash), so a figure from an older binary cannot pass as this run's."""
     try:
         with open(TRAFFIC_JSON) as f:
-            return json.load(f).get(key)
+            doc = json.load(f)
+        t = doc.get(key)
+        if t is not None:
+            t = dict(t)
+            t["kernel_source_sha16_at_capture"] = doc.get("kernel_source_sha16")
+            t["traffic_stale"] = bool(doc.get("kernel_source_sha16") != kernel_source_sha16())
+        return t
     except Exception:
         return None
 
@@ -167,6 +190,8 @@ def cpu_baseline(pos, mass, theta, eps, n_leaf, target_s: float = 30.0):
     t0 = time.perf_counter()
     r = o.forces(theta, eps, shadow32=True, groups=sel, stats=True)
     dt = time.perf_counter() - t0
+    # R16 audit of the groups whose fp32 decision differs somewhere: bookkeeping, outside the timed part
+    r["flip_audit"] = oracle.flip_audit(o, theta, r["flips"], sel)
     obj = {"value": r["interactions"] / dt, "unit": "interactions/s", "cores": oracle.num_threads(), "kind": "oracle",
            "sample": f"{len(sel)} of {ng} groups (evenly spaced in Morton order), {r['interactions']} interactions, "
                      f"{dt:.2f} s walk+evaluate in fp64 (tree build excluded)",
@@ -183,11 +208,17 @@ def parity_object(ref, sel, ng, acc, pot, n_pc, n_pp) -> dict:
     prel = np.abs(pot[m] - ref["pot"][m]) / np.abs(ref["pot"][m])
     counts_equal = bool(np.array_equal(n_pc[m], ref["n_pc"][m]) and np.array_equal(n_pp[m], ref["n_pp"][m]))
     q999, amax, pmax = float(np.quantile(rel, 0.999)), float(rel.max()), float(prel.max())
+    flips_ok = bool(all(len(cells) == f and all(s_ <= b for _, s_, b in cells) for _, f, cells in ref["flip_audit"]))
     return {"n_compared": int(m.sum()), "n_groups_compared": int(len(sel)), "n_groups": int(ng), "whole_population": bool(len(sel) == ng),
             "counts_equal": counts_equal, "acc_q50": float(np.median(rel)), "acc_q999": q999, "acc_max": amax, "pot_max": pmax,
             "flips": int(ref["flips"].sum()),
+            # R16 audit: every group whose fp32 walk differs from the fp64 one, with the cells decided differently,
+            # their fp64 slack |d theta - 2 h_c| and the bound 8 * 2^-23 * (max_k(|b_c,k| + |b_g,k|) + h_c + h_g) * max(theta, 1)
+            "flip_groups": [{"group": g, "flips": f, "cells": [{"cell": x, "slack": s_, "bound": b} for x, s_, b in cells]}
+                            for g, f, cells in ref["flip_audit"]],
+            "flips_borderline": flips_ok,
             "tolerance": {"acc_q999": ACC_Q999, "acc_max": ACC_MAX, "pot_max": POT_MAX},
-            "within_tolerance": bool(counts_equal and q999 <= ACC_Q999 and amax <= ACC_MAX and pmax <= POT_MAX),
+            "within_tolerance": bool(counts_equal and q999 <= ACC_Q999 and amax <= ACC_MAX and pmax <= POT_MAX and flips_ok),
             "what": "per-particle interaction counts (exact) and relative errors of acc / pot of the TIMED launch against the fp64 oracle "
                     "with fp32-shadow opening decisions; flips = opening tests the fp32 decision takes differently from fp64 (R16)"}
 
@@ -259,13 +290,14 @@ def run_ours(args) -> None:
         flush = torch.empty(L2_FLUSH_BYTES, dtype=torch.uint8, device=dev)
         tc.set_particles(d_pos, d_mass)
         tc.build(n_leaf)
-        scratch = {}
+        # N > 1: the shard options, the shard size and the row buffers are fixed once per tree (parallel.ShardPlan)
+        plan = parallel.ShardPlan(tc, dev) if world > 1 else None
 
         def step():
             if world == 1:
                 B.tc_forces(tc.ctx, theta, eps, d_acc, d_pot)
             else:   # this rank's shard + ONE all-gather + scatter (paper_1005_5384_b200/parallel.py)
-                parallel.forces_sharded(tc, theta, eps, d_acc, d_pot, scratch=scratch)
+                plan.forces(theta, eps, d_acc, d_pot)
 
         for _ in range(W):
             flush.zero_()
@@ -296,6 +328,8 @@ def run_ours(args) -> None:
         flops_rank = FLOPS_PC * st["n_pc_total"] + FLOPS_PP * st["n_pp_total"]
         kernel_ms_rank = st["t_gpu_ms"]
         tree_bytes = st["tree_bytes"]
+        if plan is not None:
+            plan.close()
         h_acc_res = h_pot_res = n_pc_res = n_pp_res = None
         if world == 1:
             h_acc_res, h_pot_res = d_acc.cpu().numpy(), d_pot.cpu().numpy()      # the timed launch's result, for `parity`
@@ -324,7 +358,8 @@ def run_ours(args) -> None:
                 t0 = time.perf_counter()
                 tc.set_particles(h_pos, h_mass)
                 tc.build(n_leaf)
-                parallel.forces_sharded(tc, theta, eps, d_acc, d_pot, scratch=scratch)
+                with parallel.ShardPlan(tc, dev) as pl:           # a new tree: a new shard layout
+                    pl.forces(theta, eps, d_acc, d_pot)
                 torch.from_numpy(h_acc).copy_(d_acc, non_blocking=True); torch.from_numpy(h_pot).copy_(d_pot, non_blocking=True)
                 torch.cuda.synchronize()
                 if i >= 2:
@@ -353,6 +388,21 @@ def run_ours(args) -> None:
                 "tflops": lit_flops / (float(np.median(lit_ms)) * 1e-3) / 1e12,
                 "what": "config 3 with N_group = N_leaf = 16 (groups = leaves, PAPER.md:145): fewer interactions, 5.8x the walks; "
                         "frac is against the same FP32 peak"}
+            # ---- the paper's OWN setting N_leaf = N_group = 64, same particles, theta, eps
+            tc.set_option("n_group", 64)
+            tc.build(64)
+            p64_ms = timed_forces(tc, B, torch, stream, flush, theta, eps, d_acc, d_pot, 6)[1:]
+            s64 = tc.stats()
+            p64_flops = FLOPS_PC * s64["n_pc_total"] + FLOPS_PP * s64["n_pp_total"]
+            extra["paper_setting"] = {
+                "n_leaf": 64, "n_group": 64, "n_groups": s64["n_groups"], "ms": float(np.median(p64_ms)), "ms_min": float(min(p64_ms)),
+                "interactions": s64["n_pc_total"] + s64["n_pp_total"], "n_pc": s64["n_pc_total"], "n_pp": s64["n_pp_total"],
+                "opening_tests": s64["n_tests_total"],
+                "interactions_per_s": (s64["n_pc_total"] + s64["n_pp_total"]) / (float(np.median(p64_ms)) * 1e-3),
+                "tflops": p64_flops / (float(np.median(p64_ms)) * 1e-3) / 1e12,
+                "gflops_paper_convention": (PAPER_FLOPS_PC * s64["n_pc_total"] + PAPER_FLOPS_PP * s64["n_pp_total"]) / (float(np.median(p64_ms)) * 1e-3) / 1e9,
+                "what": "config 3's particles at the paper's own N_leaf = N_group = 64 (PAPER.md:145); parity at this setting: "
+                        "tests/test_gpu_configs.py"}
             tc.set_option("n_group", N_GROUP)
             # ---- config 5's size: N = 2^24, where the packed tree (0.6 GB) streams from HBM instead of sitting in L2
             p5, m5 = inputs.two_plummer(1 << 24)
@@ -397,16 +447,17 @@ def run_ours(args) -> None:
             d_acc5 = torch.empty((n5, 3), dtype=torch.float32, device=dev); d_pot5 = torch.empty(n5, dtype=torch.float32, device=dev)
             tc.set_option("device_build", 1)
             tc.set_particles(d_pos5, d_mass5); tc.build(16)
-            sc5, ms5 = {}, []
-            for i in range(4):
-                dist.barrier()
-                a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-                a.record(stream)
-                parallel.forces_sharded(tc, 0.5, 0.005, d_acc5, d_pot5, scratch=sc5)
-                b.record(stream)
-                torch.cuda.synchronize()
-                ms5.append(a.elapsed_time(b))
-            s5 = tc.stats()
+            ms5 = []
+            with parallel.ShardPlan(tc, dev) as plan5:
+                for i in range(4):
+                    dist.barrier()
+                    a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                    a.record(stream)
+                    plan5.forces(0.5, 0.005, d_acc5, d_pot5)
+                    b.record(stream)
+                    torch.cuda.synchronize()
+                    ms5.append(a.elapsed_time(b))
+                s5 = tc.stats()
             extra["_c5_ms"] = float(np.median(ms5[1:])); extra["_c5_inter"] = s5["n_pc_total"] + s5["n_pp_total"]
             tc.set_option("device_build", 0)
             measured_peak = None
@@ -454,11 +505,14 @@ def run_ours(args) -> None:
         "gpu_launches": K if world == 1 else 2 * K,     # rank 0's own kernels in the timed region: forces (+ scatter when sharded)
         "clocks": clocks,
         "roofline": {"bound": "alu", "achieved": ach, "peak": peak, "unit": "TFLOP/s", "frac": ach / peak,
-                     "traffic": tr3["dram_bytes"] if tr3 else None, "kernel": "tc::forces_kernel",
+                     "traffic": tr3["dram_bytes"] if tr3 else None, "traffic_stale": tr3["traffic_stale"] if tr3 else None,
+                     "kernel": "tc::forces_kernel",
                      "peak_how": f"nominal: {N_SM} SMs x {LANES} FP32 lanes x 2 x {sm_max:.0f} MHz (DESIGN.md section 6; "
                                  "MEASURED_PEAKS.json holds HBM and bf16 figures only, no FP32 entry)",
                      "peak_measured": measured_peak, "frac_of_measured": (ach / measured_peak) if measured_peak else None,
                      "peak_measured_how": "tc_fp32_peak (include/tc_bench.h): FFMA-only microbenchmark on this device in this run",
+                     "frac_survey_flops": ((SURVEY_FLOPS_PC * st["n_pc_total"] + SURVEY_FLOPS_PP * st["n_pp_total"]) / (kernel_ms * 1e-3) / 1e12 / peak),
+                     "frac_survey_flops_how": f"the same launch counted with SURVEY.md 8(d)'s {SURVEY_FLOPS_PC} / {SURVEY_FLOPS_PP} flops per interaction",
                      "flops_per_launch": flops_rank, "flops_convention": f"{FLOPS_PC} per particle-cell, {FLOPS_PP} per particle-particle interaction "
                                                                          "(FFMA = 2, FADD/FMUL = 1, MUFU = 1); hardware counters in profiles/",
                      "algorithmic_bytes_per_launch": int(tree_bytes + 24 * n),
@@ -491,6 +545,7 @@ def run_ours(args) -> None:
                                  "pageable": {"value": inter_all / e2e_dev_pg_s, "ms_per_step": e2e_dev_pg_s * 1e3}},
         })
         extra["paper_literal"]["frac"] = extra["paper_literal"]["tflops"] / peak
+        extra["paper_setting"]["frac"] = extra["paper_setting"]["tflops"] / peak
         extra["config5"]["frac"] = extra["config5"]["tflops"] / peak
         out.update(extra)
         cb, ref, sel, ng = cpu_baseline(pos, mass, theta, eps, n_leaf)

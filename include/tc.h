@@ -134,7 +134,9 @@ int tc_forces(tc_ctx* ctx, float theta, float eps, float* acc, float* pot);
  *   "kernel_config" launch configuration of the fused kernel: 0 (default) = chosen by the mean number of particles per
  *                 group, 1 = sparse (16 warps per SM, for small groups), 2 = dense (12 warps per SM with larger
  *                 shared-memory chunks and more registers, for large groups).  Same arithmetic, same lists: results differ
- *                 by summation order only (the chunk boundaries move).
+ *                 by summation order only (the chunk boundaries move).  1 and 2 are honoured with either "stack_smem";
+ *                 0 picks the sparse build whenever "stack_smem" is 64.  Ignored while "two_pass" is 1 (that pipeline's
+ *                 kernels exist in one configuration).
  *   "shard_count", "shard_rank"   ONE force evaluation over k GPUs (tc_forces_shard below): this context is
  *                 rank shard_rank of shard_count.  Default 1 / 0.
  *   "two_pass"    0 (default: the fused kernel) or 1: the paper-literal pipeline —

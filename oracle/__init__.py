@@ -194,6 +194,44 @@ class Oracle:
         return out
 
 
+def flip_audit(o: "Oracle", theta: float, flips, groups=None, cells=None):
+    """R16 audit in SURVEY.md 8(c)'s own form: a group whose fp32-shadow walk differs from the fp64 walk is accepted only
+    if every test that was decided differently has an ABSOLUTE slack |d theta - 2 h_c| (fp64, O5) within a few fp32 ulps
+    of the coordinates that enter it:  slack <= 8 * 2^-23 * (max_k(|b_c,k| + |b_g,k|) + h_c + h_g) * max(theta, 1).
+
+    ``flips`` is the per-group flip count of ``forces(..., stats=True)`` (aligned with ``groups``, or with all groups).
+    For every group with a flip both walks are repeated; the cells that sit on a list of one walk but not of the other,
+    and whose parent does not, are exactly the tests decided differently (a parent of such a cell was opened by both
+    walks; cells below it differ only as a consequence).  Default opening rule only (R1 / R9).
+    Returns ``[(group, n_flips, [(cell, slack, bound), ...]), ...]``; the caller asserts slack <= bound and
+    len(list) == n_flips.  Bookkeeping on the oracle's own tree data; no part of the force arithmetic."""
+    assert o.open_rule == 0 and not o.group_box, "flip_audit: written for the default opening test (R1 / R9)"
+    flips = np.asarray(flips)
+    idx = np.nonzero(flips > 0)[0]
+    if idx.size == 0:
+        return []
+    c = cells if cells is not None else o.cells()
+    gcell = o.groups()
+    out = []
+    for k in idx:
+        g = int(k if groups is None else np.asarray(groups)[k])
+        c64, l64 = o.walk(g, theta, False)[:2]
+        c32, l32 = o.walk(g, theta, True)[:2]
+        cand = (set(c64.tolist()) ^ set(c32.tolist())) | (set(l64.tolist()) ^ set(l32.tolist()))
+        top = sorted(x for x in cand if int(c["parent"][x]) not in cand)
+        gc = int(gcell[g])
+        bg, hg = c["b"][gc], float(c["h"][gc])
+        rows = []
+        for x in top:
+            bc, hc = c["b"][x], float(c["h"][x])
+            d = np.maximum(0.0, np.abs(bc - bg) - hc - hg)
+            slack = abs(float(np.sqrt((d * d).sum())) * theta - 2.0 * hc)
+            bound = 8.0 * 2.0 ** -23 * (float(np.max(np.abs(bc) + np.abs(bg))) + hc + hg) * max(theta, 1.0)
+            rows.append((int(x), slack, bound))
+        out.append((g, int(flips[k]), rows))
+    return out
+
+
 def direct(pos, mass, eps: float, targets=None):
     """fp64 direct summation: (acc [n_t,3], pot [n_t])."""
     L = _load()

@@ -483,8 +483,11 @@ int forces_impl(tc_ctx* c, const char* who, float theta, float eps, float* acc, 
     c->out_cap = n;
   }
   // launch configuration of the fused kernel (tc_kernels.cu): dense from kDenseMinMean particles per group on
-  const bool dense = !c->two_pass && c->stack_smem == 256 &&
-                     (c->kernel_config == 2 || (c->kernel_config == 0 && (double)n >= kDenseMinMean * (double)c->tree.n_groups));
+  // (a forced configuration is honoured with either stack size; the automatic choice keeps the small-stack test path on
+  // the sparse build; the two-pass pipeline exists in one configuration only)
+  const bool dense = !c->two_pass &&
+                     (c->kernel_config == 2 ||
+                      (c->kernel_config == 0 && c->stack_smem == 256 && (double)n >= kDenseMinMean * (double)c->tree.n_groups));
   size_t& warps_cached = c->grid_warps[dense ? 1 : 0][c->stack_smem == 64 ? 1 : 0];
   if (!warps_cached)   // (an occupancy query: once per configuration, not per call)
     warps_cached = (size_t)(dense ? tc::dense::forces_total_warps(c->n_sm, c->stack_smem) : tc::sparse::forces_total_warps(c->n_sm, c->stack_smem));

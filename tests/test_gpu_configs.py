@@ -2,8 +2,10 @@
 
 Config 4: Plummer N = 2^20, theta in {0.3, 0.5, 0.75, 1.0} x N_leaf in {8, 16, 32}: rms relative force
 error against fp64 direct summation on 4096 sampled particles versus time.
-Config 5: two offset Plummer spheres, N = 2^24, eps = 0.005: oracle parity on sampled groups, then 10
-leapfrog KDK steps with a host tree rebuild each step (energy and momentum conservation).
+Config 5: two offset Plummer spheres, N = 2^24, eps = 0.005: oracle parity over EVERY particle at step 0 (all
+443 844 groups; the maximum error is a statement about the whole system) and on sampled groups at
+step 10, 10 leapfrog KDK steps with a host tree rebuild each step (energy and momentum conservation).
+Every comparison carries the R16 flip audit (test_gpu_parity.flip_audit).
 The tables are printed (run with -s) and written to gpurun_out/ when that directory exists.
 """
 import json
@@ -16,7 +18,7 @@ from oracle import Oracle, direct
 from paper_1005_5384_b200 import binding as B
 from paper_1005_5384_b200 import build as tc_build
 from paper_1005_5384_b200 import inputs
-from test_gpu_parity import check, rel_err
+from test_gpu_parity import check, flip_audit, rel_err
 
 pytestmark = pytest.mark.gpu
 N_GROUP = 128          # the library's default and bench.py's setting
@@ -37,6 +39,8 @@ def _dump(name, obj):
 
 def test_config4_accuracy_versus_time_1m():
     import torch
+    import bench
+    peak = bench.fp32_peak_tflops(1965.0)                 # nominal FP32 peak at the B200's maximum SM clock (bench.py)
     pos, mass, _, eps, _ = inputs.make("plummer_1m")
     n = len(mass)
     tg = inputs.sample_targets(n, 4096, seed=4)
@@ -59,12 +63,29 @@ def test_config4_accuracy_versus_time_1m():
                         ts.append(tc.stats()["t_gpu_ms"])
                     s = tc.stats()
                     e = rel_err(d_acc[torch.from_numpy(tg).cuda()].cpu().numpy().astype(np.float64), dacc)
-                    rows.append(dict(n_leaf=n_leaf, theta=theta, ms=float(np.median(ts[1:])),
+                    # the paper's device-utilisation picture versus theta (Fig. 8's axes): flop rate of
+                    # the evaluation and data rate of the walk alone (option walk_only: one more launch per point)
+                    tc.set_option("walk_only", 1)
+                    tw = []
+                    for _ in range(3):
+                        B.tc_forces(tc.ctx, theta, eps, d_acc, d_pot)
+                        tc.sync()
+                        tw.append(tc.stats()["t_gpu_ms"])
+                    sw = tc.stats()
+                    tc.set_option("walk_only", 0)
+                    ms, wms = float(np.median(ts[1:])), float(np.median(tw[1:]))
+                    rows.append(dict(n_leaf=n_leaf, theta=theta, ms=ms,
                                      rms=float(np.sqrt((e ** 2).mean())), median=float(np.median(e)),
-                                     p99=float(np.quantile(e, 0.99)), n_pc=s["n_pc_total"] / n, n_pp=s["n_pp_total"] / n))
+                                     p99=float(np.quantile(e, 0.99)), n_pc=s["n_pc_total"] / n, n_pp=s["n_pp_total"] / n,
+                                     tflops=(bench.FLOPS_PC * s["n_pc_total"] + bench.FLOPS_PP * s["n_pp_total"]) / (ms * 1e-3) / 1e12,
+                                     gflops_paper=(bench.PAPER_FLOPS_PC * s["n_pc_total"] + bench.PAPER_FLOPS_PP * s["n_pp_total"]) / (ms * 1e-3) / 1e9,
+                                     walk_ms=wms, tests=sw["n_tests_total"], opened=sw["n_opened_total"],
+                                     walk_gbs=16.0 * (sw["n_tests_total"] + sw["n_opened_total"]) / (wms * 1e-3) / 1e9))
+                    rows[-1]["frac"] = rows[-1]["tflops"] / peak
     for r in rows:
         print("config4 N_leaf={n_leaf:2d} theta={theta:4.2f}: {ms:7.3f} ms  rms={rms:.3e} median={median:.3e} "
-              "p99={p99:.3e}  p-c/particle={n_pc:7.0f} p-p/particle={n_pp:6.0f}".format(**r))
+              "p99={p99:.3e}  p-c/particle={n_pc:7.0f} p-p/particle={n_pp:6.0f}  {tflops:5.1f} TFLOP/s = {frac:.3f} of FP32 peak "
+              "({gflops_paper:7.0f} GFLOP/s in the paper's 70/38 convention)  walk {walk_ms:6.3f} ms = {walk_gbs:6.1f} GB/s".format(**r))
     _dump("config4_sweep.json", rows)
     for n_leaf in (8, 16, 32):
         rr = [r for r in rows if r["n_leaf"] == n_leaf]
@@ -77,40 +98,60 @@ def test_config4_accuracy_versus_time_1m():
 
 
 def test_config4_oracle_parity_at_every_sweep_point_1m():
-    """Oracle parity on sampled groups at ALL twelve (theta, N_leaf) points of config 4, full size."""
+    """Oracle parity at ALL twelve (theta, N_leaf) points of config 4, full size: EVERY particle at N_leaf = 16 (the
+    four theta of the headline leaf size), 2048 evenly spaced groups at N_leaf = 8 / 32, plus the paper's own setting
+    N_leaf = N_group = 64 at theta = 0.5 on 2048 groups.  Flip audit (R16) at every point."""
     pos, mass, _, eps, _ = inputs.make("plummer_1m")
-    for n_leaf in (8, 16, 32):
-        o = Oracle(pos, mass, n_leaf, N_GROUP)
-        gsel = np.arange(7 + n_leaf, o.n_groups, o.n_groups // 192, dtype=np.int64)
-        with B.TreeCode(n_group=N_GROUP) as tc:
+    rows = []
+    for n_leaf, n_group, thetas in ((8, N_GROUP, (0.3, 0.5, 0.75, 1.0)), (16, N_GROUP, (0.3, 0.5, 0.75, 1.0)),
+                                    (32, N_GROUP, (0.3, 0.5, 0.75, 1.0)), (64, 64, (0.5,))):
+        o = Oracle(pos, mass, n_leaf, n_group)
+        gsel = None if n_leaf == 16 else np.unique(np.linspace(0, o.n_groups - 1, 2048).astype(np.int64))
+        with B.TreeCode(n_group=n_group) as tc:
             tc.set_particles(pos, mass)
             tc.build(n_leaf)
-            for theta in (0.3, 0.5, 0.75, 1.0):
-                ref = o.forces(theta, eps, shadow32=True, groups=gsel)
+            for theta in thetas:
+                ref = o.forces(theta, eps, shadow32=True, groups=gsel, stats=True)
                 acc, pot = tc.forces(theta, eps)
                 n_pc, n_pp = tc.counts()
                 sel = ref["n_pc"] >= 0
+                assert gsel is not None or sel.all()
                 rel, prel = check(acc, pot, n_pc, n_pp, ref, sel)
-                print(f"config4 parity N_leaf={n_leaf:2d} theta={theta:4.2f}: {int(sel.sum())} particles of {len(gsel)} groups, "
-                      f"acc q99.9={np.quantile(rel, 0.999):.2e} max={rel.max():.2e} pot max={prel.max():.2e}")
+                fl = flip_audit(o, ref, theta, gsel, tag=f"config4 N_leaf={n_leaf} theta={theta}")
+                rows.append(dict(n_leaf=n_leaf, n_group=n_group, theta=theta, particles=int(sel.sum()),
+                                 groups=int(o.n_groups if gsel is None else len(gsel)), n_groups=int(o.n_groups),
+                                 acc_q50=float(np.median(rel)), acc_q999=float(np.quantile(rel, 0.999)), acc_max=float(rel.max()),
+                                 pot_max=float(prel.max()), flips=fl))
+                print(f"config4 parity N_leaf={n_leaf:2d} N_group={n_group:3d} theta={theta:4.2f}: {int(sel.sum())} particles of "
+                      f"{rows[-1]['groups']} / {o.n_groups} groups, acc q99.9={np.quantile(rel, 0.999):.2e} max={rel.max():.2e} "
+                      f"pot max={prel.max():.2e} flips={sum(f for _, f, _ in fl)}")
+    _dump("config4_parity.json", rows)
 
 
 def _sampled_parity(tag, pos_host, mass, d_acc, d_pot, n_pc, n_pp, theta, eps, n_leaf, n_group, n_sample, seed):
-    """Oracle (own tree on these positions) on n_sample random groups against the library's result."""
+    """Oracle (own tree on these positions) on n_sample random groups (None: ALL groups, every particle) against the
+    library's result; R16 flip audit on the groups walked."""
     o = Oracle(pos_host, mass, n_leaf, n_group)
-    gsel = np.sort(np.random.default_rng(seed).choice(o.n_groups, n_sample, replace=False)).astype(np.int64)
+    gsel = None if n_sample is None else np.sort(np.random.default_rng(seed).choice(o.n_groups, n_sample, replace=False)).astype(np.int64)
     ref = o.forces(theta, eps, shadow32=True, groups=gsel, stats=True)
     shape = (o.n_cells, o.n_leaves, o.n_groups, o.depth)
-    del o
     sel = ref["n_pc"] >= 0
+    assert n_sample is not None or sel.all()            # whole population: the oracle evaluated every particle
     rel, prel = check(d_acc.cpu().numpy(), d_pot.cpu().numpy(), n_pc, n_pp, ref, sel)
-    print(f"config5 {tag}: {int(sel.sum())} particles of {n_sample} groups, flips={int(ref['flips'].sum())}, "
-          f"acc q99.9={np.quantile(rel, 0.999):.2e} max={rel.max():.2e} pot max={prel.max():.2e}")
+    fl = flip_audit(o, ref, theta, gsel, tag=f"config5 {tag}")
+    del o
+    print(f"config5 {tag}: {int(sel.sum())} particles of {shape[2] if n_sample is None else n_sample} groups, flips={int(ref['flips'].sum())}, "
+          f"acc q50={np.median(rel):.2e} q99.9={np.quantile(rel, 0.999):.2e} max={rel.max():.2e} pot max={prel.max():.2e}")
+    _dump(f"config5_parity_{tag.replace(' ', '_').replace('(', '').replace(')', '')}.json",
+          dict(particles=int(sel.sum()), groups=int(shape[2] if n_sample is None else n_sample), n_groups=int(shape[2]),
+               interactions=int(ref["interactions"]), acc_q50=float(np.median(rel)), acc_q999=float(np.quantile(rel, 0.999)),
+               acc_max=float(rel.max()), pot_max=float(prel.max()), flips=fl))
     return shape
 
 
 def test_config5_two_plummer_16m_parity_and_leapfrog():
-    """Config 5 at full size: oracle parity at step 0 AND on the step-10 positions on 4096 sampled groups,
+    """Config 5 at full size: oracle parity at step 0 over EVERY particle (all groups) and on the step-10 positions
+     on 4096 sampled groups,
     10 KDK steps with a host tree rebuild each step (the torch harness), then the same 10 steps with the library's own
     device-side leapfrog (`tc_leapfrog`, device tree build) ending in the same state."""
     import torch
@@ -121,7 +162,7 @@ def test_config5_two_plummer_16m_parity_and_leapfrog():
     with torch.cuda.stream(st), B.TreeCode(n_group=n_group) as tc:
         tc.set_stream(st.cuda_stream)
         d_pos, d_vel, d_mass = torch.from_numpy(pos).cuda(), torch.from_numpy(vel).cuda(), torch.from_numpy(mass).cuda()
-        # ---- parity at step 0 on sampled groups (full size, the configuration the loop runs)
+        # ---- parity at step 0 over the whole population (full size, the configuration the loop runs)
         d_acc = torch.empty((n, 3), dtype=torch.float32, device="cuda")
         d_pot = torch.empty(n, dtype=torch.float32, device="cuda")
         tc.set_particles(d_pos, d_mass)
@@ -130,7 +171,7 @@ def test_config5_two_plummer_16m_parity_and_leapfrog():
         tc.sync()
         s0 = tc.stats()
         n_pc, n_pp = tc.counts()
-        shape = _sampled_parity("step 0", pos, mass, d_acc, d_pot, n_pc, n_pp, theta, eps, n_leaf, n_group, 4096, 5)
+        shape = _sampled_parity("step 0", pos, mass, d_acc, d_pot, n_pc, n_pp, theta, eps, n_leaf, n_group, None, 5)
         assert (s0["n_cells"], s0["n_leaves"], s0["n_groups"], s0["depth"]) == shape
         print(f"config5 step 0: cells={s0['n_cells']} groups={s0['n_groups']} T_host={s0['t_host_ms']:.0f} ms "
               f"T_copy={s0['t_copy_ms']:.1f} ms T_gpu={s0['t_gpu_ms']:.1f} ms interactions={s0['n_pc_total'] + s0['n_pp_total']:.3e}")

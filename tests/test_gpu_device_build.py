@@ -90,7 +90,8 @@ def test_forces_on_device_built_tree_match_oracle(name):
 
 
 def test_device_and_host_build_times_1m():
-    """Prints both build times (no assertion on a timing: the host side of the box varies from run to run)."""
+    """Prints both build times.  The host side of the box varies from run to run, so the guard is loose: the device
+    build (measured 1.1-1.3 ms) must not take more than twice the host build + copy (6-8 ms) at N = 2^20."""
     pos, mass, theta, eps, n_leaf = inputs.make("plummer_1m")
     t = {}
     for dev in (0, 1):
@@ -103,7 +104,7 @@ def test_device_and_host_build_times_1m():
                 ts.append(tc.stats()["t_host_ms"] + tc.stats()["t_copy_ms"])
             t[dev] = min(ts[1:])
     print(f"tc_build N=2^20: host {t[0]:.2f} ms (build + copy), device {t[1]:.2f} ms")
-    assert t[0] > 0 and t[1] > 0
+    assert t[0] > 0 and 0 < t[1] <= 2.0 * t[0]
 
 
 def test_device_inputs_device_build_leapfrog_matches_host_build():

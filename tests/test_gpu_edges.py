@@ -77,11 +77,13 @@ def test_theta_extremes(theta):
         check(acc, pot, n_pc, n_pp, ref)
 
 
-def test_spill_path_matches_and_is_exercised():
-    """stack_smem = 64 forces the walk stack through its global-memory spill: same result."""
+@pytest.mark.parametrize("cfg", [0, 1, 2])
+def test_spill_path_matches_and_is_exercised(cfg):
+    """stack_smem = 64 forces the walk stack through its global-memory spill: same result — in the automatic choice and in
+    each build of the fused kernel forced (kernel_config 1 = sparse, 2 = dense: both compile the spill path)."""
     pos, mass = inputs.plummer(32768, 14)
-    a0, p0, c0, d0, s0 = gpu_forces(pos, mass, 0.2, 0.01, 2, 16)
-    a1, p1, c1, d1, s1 = gpu_forces(pos, mass, 0.2, 0.01, 2, 16, opts={"stack_smem": 64})
+    a0, p0, c0, d0, s0 = gpu_forces(pos, mass, 0.2, 0.01, 2, 16, opts={"kernel_config": cfg})
+    a1, p1, c1, d1, s1 = gpu_forces(pos, mass, 0.2, 0.01, 2, 16, opts={"stack_smem": 64, "kernel_config": cfg})
     assert s1["n_spills"] > 1000 and s0["n_spills"] <= 16      # (theta = 0.2, N_leaf = 2: a handful of spills even with 256 entries)
     assert np.array_equal(c0, c1) and np.array_equal(d0, d1)
     assert s0["n_tests_total"] == s1["n_tests_total"]

@@ -1,7 +1,8 @@
 """Seeded randomised parity of the CUDA path with the fp64 oracle — `-m gpu`.
 
-compute-sanitizer is not available on the GPU pool, so out-of-range accesses and
-races of the shared-memory stack / list chunks are hunted the plain way: many small,
+compute-sanitizer is closed on the GPU pool (the refusal, verbatim, is in
+profiles/r03_sanitizer.md), so out-of-range accesses and races of the
+shared-memory stack / list chunks are hunted the plain way: many small,
 differently shaped problems (ragged sizes, degenerate geometry, duplicates, extreme
 N_leaf / N_group / theta, the stack-spill path, both tree builders, both pipelines),
 output buffers pre-filled with NaN and guarded on both sides, every result compared

@@ -71,6 +71,20 @@ def check(acc, pot, n_pc, n_pp, ref, sel=None):
     return rel, prel
 
 
+def flip_audit(o, ref, theta, groups=None, tag=""):
+    """R16 at full size: the fp32 opening decision may differ from the fp64 one only where the fp64 test is
+    decided within a few fp32 ulps of the coordinates entering it (oracle.flip_audit: SURVEY's absolute form).  Every
+    group with a flip is listed with its flipped cells, their slack |d theta - 2h| and the bound.  Needs stats=True."""
+    import oracle
+    rows = oracle.flip_audit(o, theta, ref["flips"], groups)
+    for g, f, cells in rows:
+        print(f"R16 flip audit {tag}: group {g}: {f} flipped test(s): " +
+              ", ".join(f"cell {x} slack {s:.2e} <= {b:.2e}" for x, s, b in cells))
+        assert len(cells) == f, (tag, g, f, cells)
+        assert all(s <= b for _, s, b in cells), (tag, g, cells)
+    return [(g, f, max((s / b for _, s, b in cells), default=0.0)) for g, f, cells in rows]
+
+
 # ---- config 1: Plummer N = 1024 vs oracle AND vs direct sum ------------------------------
 @pytest.mark.parametrize("n_group", [16, 64])
 @pytest.mark.parametrize("device", [False, True])
@@ -147,6 +161,7 @@ def test_config3_plummer_1m_every_particle(n_group):
           f"flips(fp32 vs fp64 decision)={flips}, acc q50={np.median(rel):.2e} q99.9={np.quantile(rel, 0.999):.2e} "
           f"max={rel.max():.2e}, pot max={prel.max():.2e}")
     assert flips <= flip_bound(o.n_groups)
+    assert sum(f for _, f, _ in flip_audit(o, ref, theta, tag=f"config3 N_group={n_group}")) == flips
     # properties that hold at any size
     assert np.isfinite(acc).all() and np.isfinite(pot).all() and (pot < 0).all()
     a64 = acc.astype(np.float64)

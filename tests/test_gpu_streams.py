@@ -39,13 +39,19 @@ def test_forces_on_default_stream_wait_for_a_late_write_of_the_positions():
         tc.build(n_leaf)
         a0, p0 = tc.forces(theta, eps)
     d_src, d_mass = torch.from_numpy(pos).cuda(), torch.from_numpy(mass).cuda()
-    d_pos = torch.zeros_like(d_src)                                  # what a too-early read would see
+    d_pos = d_src * 2.0                                              # what a too-early read would see: another (valid) system
     acc = torch.empty((n, 3), dtype=torch.float32, device="cuda")
     pot = torch.empty(n, dtype=torch.float32, device="cuda")
     torch.cuda.synchronize()
     with B.TreeCode() as tc:
         tc.use_torch_stream()
         tc.set_option("device_build", 1)                             # everything stays stream-ordered on the device
+        # one pass up front: every buffer of the context exists afterwards, so that nothing in the pass under test
+        # synchronises the device by accident (a first-use cudaMalloc) and hides a missing stream order
+        tc.set_particles(d_pos, d_mass)
+        tc.build(n_leaf)
+        B.tc_forces(tc.ctx, theta, eps, acc, pot)
+        tc.sync()
         torch.cuda._sleep(SPIN)
         d_pos.copy_(d_src)                                           # lands ~0.15 s from now
         tc.set_particles(d_pos, d_mass)

@@ -174,3 +174,23 @@ def test_fp32_boundary_contains_box_and_own_cells_always_open(n_leaf, n_group):
         cl, ll, _, _, _ = o.walk(g, 0.6, shadow32=True)
         assert not ((c["begin"][cl] < ge) & (c["begin"][cl] + c["count"][cl] > gb)).any()
         assert c["count"][cl].sum() + c["count"][ll].sum() == o.n
+
+
+def test_flip_audit_finds_exactly_the_flipped_tests_within_survey_bound():
+    """R16 in SURVEY 8(c)'s absolute form (oracle.flip_audit): for every group whose fp32-shadow walk differs from the fp64
+    one, the cells decided differently are as many as the walk counted flips, and each has a slack |d theta - 2h| within
+    8 * 2^-23 * (max_k(|b_c,k| + |b_g,k|) + h_c + h_g) * max(theta, 1).  Groups without a flip are not listed."""
+    pos, m = inputs.plummer(65536, 2)
+    O = oracle.Oracle(pos, m, 16)
+    r = O.forces(0.3, 0.01, shadow32=True, stats=True)
+    rows = oracle.flip_audit(O, 0.3, r["flips"])
+    assert int(r["flips"].sum()) >= 3                    # the case has flips to audit (5 with this seed)
+    assert sorted(g for g, _, _ in rows) == sorted(np.nonzero(r["flips"] > 0)[0].tolist())
+    for g, f, cells in rows:
+        assert len(cells) == f == int(r["flips"][g])
+        for x, slack, bound in cells:
+            assert 0.0 <= slack <= bound < 1e-4
+    # with a subset of groups the indices are mapped back to group numbers
+    sel = np.array(sorted(g for g, _, _ in rows)[:2] + [7], dtype=np.int64)
+    rs = O.forces(0.3, 0.01, shadow32=True, groups=sel, stats=True)
+    assert [g for g, _, _ in oracle.flip_audit(O, 0.3, rs["flips"], sel)] == sel[:2].tolist()
