@@ -109,10 +109,8 @@ int tc_build(tc_ctx* ctx, int n_leaf);
  * Host pointers: synchronous on return.  Device pointers: stream-ordered on the
  * context's stream (tc_set_stream); errors of the kernel surface at tc_sync().
  * eps < 1e-10 is taken as eps = 0 (coincident pairs then contribute nothing): m / eps^3 of the self pair must stay
- * finite in fp32; theta > 1e18 (theta^2 overflows fp32) is refused.  With eps > 0 every particle meets itself once
- * (the term -m_i/eps is added to phi_i and taken out again in fp32), so phi_i carries an absolute error of about
- * 6e-8 m_i/eps: negligible for N-body softening lengths (m/eps ~ 1e-4 at config 3), above the 1e-4 bar once
- * m_i/eps > ~1e3 |phi_i|.
+ * finite in fp32; theta > 1e18 (theta^2 overflows fp32) is refused.  The sums run over j != i: the pair (i, i) is excluded
+ * by index where it would occur (the rounds that stage the group's own particles), so no -m_i/eps term enters phi_i.
  * Errors: TC_ESTATE (tree not built / host-only / shard_count > 1: use tc_forces_shard), TC_EINVAL
  * (theta < 0, theta > 1e18, eps < 0, non-finite, acc NULL), TC_ECUDA, TC_EOVERFLOW.                 */
 int tc_forces(tc_ctx* ctx, float theta, float eps, float* acc, float* pot);

@@ -235,6 +235,19 @@ __device__ __forceinline__ void pp_interact(const Pos1& p, float eps2, const flo
   a.ax = __fmaf_rn(mr3, dx, a.ax); a.ay = __fmaf_rn(mr3, dy, a.ay); a.az = __fmaf_rn(mr3, dz, a.az);
 }
 
+// The same pair of interactions with one mass per half: the half whose particle IS the staged body gets mass 0 and the
+// pair (i, i) contributes exactly nothing (O6: the sums run over j != i).  eps > 0 only: with eps = 0 the pair is masked by s^2 = 0.
+__device__ __forceinline__ void pp_interact_masked(const Pos2& p, float eps2, const float4 b, float m0, float m1, Acc2& a) {
+  const f2 dx = sub2(bc(b.x), p.x), dy = sub2(bc(b.y), p.y), dz = sub2(bc(b.z), p.z);
+  const f2 s2 = fma2(dz, dz, fma2(dy, dy, fma2(dx, dx, bc(eps2))));
+  const f2 ri = pk(rsqrt_approx(lo(s2)), rsqrt_approx(hi(s2)));
+  const f2 ri2 = mul2(ri, ri);
+  const f2 mr = mul2(pk(m0, m1), ri);
+  const f2 mr3 = mul2(mr, ri2);
+  a.npot = add2(a.npot, mr);
+  a.ax = fma2(mr3, dx, a.ax); a.ay = fma2(mr3, dy, a.ay); a.az = fma2(mr3, dz, a.az);
+}
+
 // Lane mapping of one pass over m <= kPassCap particles of a group (tc_lanes.h):
 // lane = s * q + p, q = floor(32 / S); the lane's j-th particle is j * q + p, j < K.
 struct Lanes {
@@ -319,23 +332,44 @@ __device__ __forceinline__ void eval_bodies_k(const float4* __restrict__ body, i
   for (; b < end; b += sd) pp_apply<KP, ODD, kEps0>(st, eps2, b[0]);
 }
 
+// The round that stages the pass's OWN particles (at most a few per group: its own leaves): the only place where a particle can
+// meet itself.  The staged body's tree index (bidx) is compared with the lane's particles' and the self pair gets mass 0 —
+// so -m/eps never enters the fp32 potential sum (it used to be added and taken out again at write-back, which cost
+// ~6e-8 m/eps of absolute accuracy).  Plain loop: these rounds are a few per cent of the particle-particle work.
+template <int KP, bool ODD>
+__device__ __forceinline__ void eval_bodies_self_k(const float4* __restrict__ body, const int* __restrict__ bidx, int cnt, float eps2,
+                                                   const Lanes& L, PassState& st) {
+  if (!L.active) return;
+  const int me = L.tail - L.mA + L.p;              // tree index of the lane's particle 0; particle j is me + j * q
+  for (int e = L.s; e < cnt; e += L.S) {
+    const float4 b = body[e];
+    const int rel = bidx[e] - me;
+#pragma unroll
+    for (int j = 0; j < KP; j++)
+      pp_interact_masked(st.P[j], eps2, b, rel == 2 * j * L.q ? 0.f : b.w, rel == (2 * j + 1) * L.q ? 0.f : b.w, st.A[j]);
+    if (ODD) pp_interact<false>(st.p1, eps2, make_float4(b.x, b.y, b.z, rel == 2 * KP * L.q ? 0.f : b.w), st.a1);
+  }
+}
+
 // K is warp-uniform: one branch to the instantiation for this pass's particles per lane
-enum { kEvalCells = 0, kEvalMono = 1, kEvalBodies = 2 };
+enum { kEvalCells = 0, kEvalMono = 1, kEvalBodies = 2, kEvalBodiesSelf = 3 };
 template <int WHAT, bool kEps0, int K = 1>
-__device__ __forceinline__ void eval_dispatch(const void* list, int cnt, float eps2, const Lanes& L, PassState& st) {
+__device__ __forceinline__ void eval_dispatch(const void* list, int cnt, float eps2, const Lanes& L, PassState& st, const int* bidx = nullptr) {
   if (K == kMaxK || L.K == K) {
-    if (WHAT == kEvalCells) eval_cells_k<K / 2, (K & 1) != 0>(static_cast<const CellRec*>(list), cnt, eps2, L, st);
+    if (WHAT == kEvalBodiesSelf) eval_bodies_self_k<K / 2, (K & 1) != 0>(static_cast<const float4*>(list), bidx, cnt, eps2, L, st);
+    else if (WHAT == kEvalCells) eval_cells_k<K / 2, (K & 1) != 0>(static_cast<const CellRec*>(list), cnt, eps2, L, st);
     else if (WHAT == kEvalMono) eval_cells_mono_k<K / 2, (K & 1) != 0, kEps0>(static_cast<const CellRec*>(list), cnt, eps2, L, st);
     else eval_bodies_k<K / 2, (K & 1) != 0, kEps0>(static_cast<const float4*>(list), cnt, eps2, L, st);
   } else if constexpr (K < kMaxK) {
-    eval_dispatch<WHAT, kEps0, K + 1>(list, cnt, eps2, L, st);
+    eval_dispatch<WHAT, kEps0, K + 1>(list, cnt, eps2, L, st, bidx);
   }
 }
 // The tail particles (Lanes::mB of them): lane l takes list entries l, l + 32, ... and applies each to ALL tail particles in
 // scalar arithmetic.  Their accumulators are the halves of the TOP register pairs of the state (the lane table leaves
 // those pairs to the tail): unpacked to scalars for the loop, packed again after it.
 template <int MB, int WHAT, bool kEps0>
-__device__ __forceinline__ void eval_tail_m(const void* list, int cnt, float eps2, const Lanes& L, PassState& st, int lane) {
+__device__ __forceinline__ void eval_tail_m(const void* list, int cnt, float eps2, const Lanes& L, PassState& st, int lane,
+                                            const int* bidx = nullptr) {
   Pos1 p[MB];
   Acc1 a[MB];
 #pragma unroll
@@ -346,7 +380,14 @@ __device__ __forceinline__ void eval_tail_m(const void* list, int cnt, float eps
     if (j & 1) { a[j].ax = hi(a2.ax); a[j].ay = hi(a2.ay); a[j].az = hi(a2.az); a[j].npot = hi(a2.npot); }
     else { a[j].ax = lo(a2.ax); a[j].ay = lo(a2.ay); a[j].az = lo(a2.az); a[j].npot = lo(a2.npot); }
   }
-  if (WHAT == kEvalBodies) {
+  if (WHAT == kEvalBodiesSelf) {                      // (see eval_bodies_self_k: tail particle j has tree index L.tail + j)
+    for (int e = lane; e < cnt; e += 32) {
+      const float4 bb = static_cast<const float4*>(list)[e];
+      const int rel = bidx[e] - L.tail;
+#pragma unroll
+      for (int j = 0; j < MB; j++) pp_interact<kEps0>(p[j], eps2, make_float4(bb.x, bb.y, bb.z, rel == j ? 0.f : bb.w), a[j]);
+    }
+  } else if (WHAT == kEvalBodies) {
     const float4* b = static_cast<const float4*>(list) + lane;
     const float4* const end = static_cast<const float4*>(list) + cnt;
     for (; b < end; b += 32) {
@@ -377,10 +418,11 @@ __device__ __forceinline__ void eval_tail_m(const void* list, int cnt, float eps
   }
 }
 template <int WHAT, bool kEps0, int MB = 1>
-__device__ __forceinline__ void eval_tail(const void* list, int cnt, float eps2, const Lanes& L, PassState& st, int lane) {
+__device__ __forceinline__ void eval_tail(const void* list, int cnt, float eps2, const Lanes& L, PassState& st, int lane,
+                                          const int* bidx = nullptr) {
   if constexpr (kMaxTail >= 1) {
-    if (MB == kMaxTail || L.mB == MB) eval_tail_m<MB, WHAT, kEps0>(list, cnt, eps2, L, st, lane);
-    else if constexpr (MB < kMaxTail) eval_tail<WHAT, kEps0, MB + 1>(list, cnt, eps2, L, st, lane);
+    if (MB == kMaxTail || L.mB == MB) eval_tail_m<MB, WHAT, kEps0>(list, cnt, eps2, L, st, lane, bidx);
+    else if constexpr (MB < kMaxTail) eval_tail<WHAT, kEps0, MB + 1>(list, cnt, eps2, L, st, lane, bidx);
   }
 }
 
@@ -414,6 +456,9 @@ __device__ __forceinline__ void eval_leaves(BodyStage& bs, const int2* leafq, in
     for (int base = 0; base < total; base += kBodyCap) {
       const int k0 = max(0, base - off), k1 = min(n, base + kBodyCap - off);
       const int cnt = min(kBodyCap, total - base);
+      // does this round stage particles of the pass itself, [own_f, own_e)?  (warp-uniform; eps = 0 masks the pair by s^2 = 0)
+      const int own_f = L.tail - L.mA, own_e = L.tail + L.mB;
+      const bool self_round = !kEps0 && __any_sync(kFull, k1 > k0 && f + k0 < own_e && f + k1 > own_f);
 #if TC_BULK_BODIES
       if (mbar) {
         const unsigned bar = smem_u32(mbar);
@@ -430,6 +475,7 @@ __device__ __forceinline__ void eval_leaves(BodyStage& bs, const int2* leafq, in
                        : "=r"(ok) : "r"(bar), "r"(*phase) : "memory");
         } while (!ok);
         *phase ^= 1u;
+        if (self_round) { for (int k = k0; k < k1; k++) bs.bidx[off + k - base] = f + k; __syncwarp(); }
       } else
 #endif
       {
@@ -438,8 +484,13 @@ __device__ __forceinline__ void eval_leaves(BodyStage& bs, const int2* leafq, in
         for (int t = lane; t < cnt; t += 32) bs.body[t] = __ldg(part + bs.bidx[t]);
         __syncwarp();
       }
-      eval_dispatch<kEvalBodies, kEps0>(bs.body, cnt, eps2, L, st);
-      if (L.mB) eval_tail<kEvalBodies, kEps0>(bs.body, cnt, eps2, L, st, lane);
+      if (self_round) {
+        eval_dispatch<kEvalBodiesSelf, kEps0>(bs.body, cnt, eps2, L, st, bs.bidx);
+        if (L.mB) eval_tail<kEvalBodiesSelf, kEps0>(bs.body, cnt, eps2, L, st, lane, bs.bidx);
+      } else {
+        eval_dispatch<kEvalBodies, kEps0>(bs.body, cnt, eps2, L, st);
+        if (L.mB) eval_tail<kEvalBodies, kEps0>(bs.body, cnt, eps2, L, st, lane);
+      }
       __syncwarp();
     }
   }
@@ -494,7 +545,7 @@ __device__ __forceinline__ void store_particle(int t, int tq, float ax, float ay
                                                float* __restrict__ pot, int32_t* __restrict__ out_cnt, int cnt_value,
                                                int32_t* __restrict__ out_cnt2, int cnt2_value, bool self_met,
                                                float4* __restrict__ rows, int2* __restrict__ row_cnt) {
-  if (kSelf && self_met) ph += __ldg(part + t).w * rsqrt_approx(eps2);     // the particle met itself once
+  (void)eps2; (void)self_met;   // (the self pair is excluded where it would occur: eval_bodies_self_k)
   if (!kAdd && rows) {                                                     // shard: compact rows, tree order inside the group
     rows[tq] = make_float4(ax, ay, az, ph);
     if (row_cnt) row_cnt[tq] = make_int2(cnt_value, cnt2_value);
@@ -1073,6 +1124,20 @@ __device__ __forceinline__ void direct_interact(const Pos2& p, float eps2, const
   a.ax = fma2(mr3, dx, a.ax); a.ay = fma2(mr3, dy, a.ay); a.az = fma2(mr3, dz, a.az);
 }
 
+// the same pair of interactions with one mass per half (0 for the half whose target IS the source: the sum runs over j != i)
+__device__ __forceinline__ void direct_interact_masked(const Pos2& p, float eps2, const float4 b, float m0, float m1, Acc2& a) {
+  const f2 dx = sub2(bc(b.x), p.x), dy = sub2(bc(b.y), p.y), dz = sub2(bc(b.z), p.z);
+  const f2 s2 = fma2(dz, dz, fma2(dy, dy, fma2(dx, dx, bc(eps2))));
+  f2 ri = pk(rsqrt_approx(lo(s2)), rsqrt_approx(hi(s2)));
+  const f2 h = mul2(s2, bc(-0.5f));
+  ri = mul2(ri, fma2(h, mul2(ri, ri), bc(1.5f)));
+  const f2 ri2 = mul2(ri, ri);
+  const f2 mr = mul2(pk(m0, m1), ri);
+  const f2 mr3 = mul2(mr, ri2);
+  a.npot = add2(a.npot, mr);
+  a.ax = fma2(mr3, dx, a.ax); a.ay = fma2(mr3, dy, a.ay); a.az = fma2(mr3, dz, a.az);
+}
+
 template <bool kEps0>
 __global__ void __launch_bounds__(kDirThreads)
 direct_kernel(const float4* __restrict__ src, long long n, const long long* __restrict__ targets, long long n_t,
@@ -1082,7 +1147,6 @@ direct_kernel(const float4* __restrict__ src, long long n, const long long* __re
   const long long t0 = (long long)blockIdx.x * kDirTargetsPerCta + threadIdx.x;
   long long ti[4];
   Pos2 P[2];
-  float msf[4];
 #pragma unroll
   for (int j = 0; j < 4; j++) {
     const long long t = t0 + (long long)j * kDirThreads;
@@ -1092,7 +1156,6 @@ direct_kernel(const float4* __restrict__ src, long long n, const long long* __re
   for (int j = 0; j < 2; j++) {
     const float4 a = __ldg(src + (ti[2 * j] >= 0 ? ti[2 * j] : 0)), b = __ldg(src + (ti[2 * j + 1] >= 0 ? ti[2 * j + 1] : 0));
     P[j].x = add2(pk(a.x, b.x), bc(0.f)); P[j].y = add2(pk(a.y, b.y), bc(0.f)); P[j].z = add2(pk(a.z, b.z), bc(0.f));
-    msf[2 * j] = a.w; msf[2 * j + 1] = b.w;
   }
   double d[4][4];
 #pragma unroll
@@ -1112,11 +1175,25 @@ direct_kernel(const float4* __restrict__ src, long long n, const long long* __re
     Acc2 A[2];
 #pragma unroll
     for (int j = 0; j < 2; j++) A[j].ax = A[j].ay = A[j].az = A[j].npot = 0ull;
+    // A target meets itself only in the tile that holds it: there (a few tiles per thread) the source whose index is the
+    // target's gets mass 0, so -m/eps never enters the fp32 partial sum.  eps = 0 masks the pair by s^2 = 0 already.
+    const long long tbase = tl * kDirTile;
+    const bool own_tile = !kEps0 && ((ti[0] >= tbase && ti[0] < tbase + kDirTile) || (ti[1] >= tbase && ti[1] < tbase + kDirTile) ||
+                                     (ti[2] >= tbase && ti[2] < tbase + kDirTile) || (ti[3] >= tbase && ti[3] < tbase + kDirTile));
+    if (own_tile) {
+      for (int k = 0; k < kDirTile; k++) {
+        const float4 b = tile[k];
+        const long long jj = tbase + k;
+        direct_interact_masked(P[0], eps2, b, jj == ti[0] ? 0.f : b.w, jj == ti[1] ? 0.f : b.w, A[0]);
+        direct_interact_masked(P[1], eps2, b, jj == ti[2] ? 0.f : b.w, jj == ti[3] ? 0.f : b.w, A[1]);
+      }
+    } else {
 #pragma unroll 4
-    for (int k = 0; k < kDirTile; k++) {
-      const float4 b = tile[k];
-      direct_interact<kEps0>(P[0], eps2, b, A[0]);
-      direct_interact<kEps0>(P[1], eps2, b, A[1]);
+      for (int k = 0; k < kDirTile; k++) {
+        const float4 b = tile[k];
+        direct_interact<kEps0>(P[0], eps2, b, A[0]);
+        direct_interact<kEps0>(P[1], eps2, b, A[1]);
+      }
     }
 #pragma unroll
     for (int j = 0; j < 2; j++) {
@@ -1130,13 +1207,7 @@ direct_kernel(const float4* __restrict__ src, long long n, const long long* __re
   for (int j = 0; j < 4; j++) {
     if (ti[j] < 0) continue;
     const long long t = t0 + (long long)j * kDirThreads;
-    double ph = -d[j][3];
-    // the target met itself once (in exactly one source split): remove -m/eps again
-    if (!kEps0 && blockIdx.y == 0) {
-      float r = rsqrt_approx(eps2);
-      r = r * fmaf(-0.5f * eps2, r * r, 1.5f);
-      ph += (double)(msf[j] * r);
-    }
+    const double ph = -d[j][3];
     atomicAdd(acc + 3 * t + 0, d[j][0]); atomicAdd(acc + 3 * t + 1, d[j][1]); atomicAdd(acc + 3 * t + 2, d[j][2]);
     if (pot) atomicAdd(pot + t, ph);
   }

@@ -248,3 +248,28 @@ def test_both_launch_configurations_match_the_oracle(cfg):
         assert rel_err(a1.astype(np.float64), a0.astype(np.float64)).max() <= 5e-5
         with pytest.raises(B.TcError):
             tc.set_option("kernel_config", 3)
+
+
+@pytest.mark.parametrize("two_pass", [0, 1])
+def test_self_pair_is_excluded_not_cancelled_at_large_m_over_eps(two_pass):
+    """O6 sums over j != i.  With m / eps = 1e4 and |phi| ~ 1, a self term -m/eps that is added to the fp32 potential sum and
+    taken out again leaves ~6e-8 * 1e4 = 6e-4 of relative error (the library did that until round 3: this test failed);
+    excluded by index, the potential is accurate to fp32 rounding.  Tree path (fused and two-pass) and tc_direct."""
+    pos = np.array([[0.0, 0.0, 0.0], [1.0, 0.25, 0.0], [-0.5, 0.75, 0.5], [0.25, -1.0, 0.75], [0.5, 0.5, -1.25]], np.float32)
+    mass = np.array([1.0, 0.5, 2.0, 1.5, 0.75], np.float32)
+    eps = 1e-4
+    for n_leaf, n_group in ((1, 1), (2, 8), (16, 128)):
+        acc, pot, n_pc, n_pp, _ = gpu_forces(pos, mass, 0.5, eps, n_leaf, n_group, opts={"two_pass": two_pass})
+        ref = Oracle(pos, mass, n_leaf, n_group).forces(0.5, eps, shadow32=True)
+        assert np.array_equal(n_pc, ref["n_pc"]) and np.array_equal(n_pp, ref["n_pp"])
+        assert (np.abs(pot - ref["pot"]) / np.abs(ref["pot"])).max() <= 2e-6
+        assert rel_err(acc.astype(np.float64), ref["acc"]).max() <= 1e-5
+    if not two_pass:
+        with B.TreeCode() as tc:
+            tc.set_particles(pos, mass)
+            dacc, dpot = tc.direct(eps)
+            tg = np.array([3, 0, 3], np.int64)             # targets out of order, one twice
+            tacc, tpot = tc.direct(eps, tg)
+        racc, rpot = direct(pos, mass, eps)
+        assert (np.abs(dpot - rpot) / np.abs(rpot)).max() <= 1e-6 and rel_err(dacc, racc).max() <= 2e-6
+        assert np.array_equal(tpot, dpot[tg]) and np.array_equal(tacc, dacc[tg])
